@@ -1,0 +1,170 @@
+/* gsnfs.h -- C ABI of the B200-native (sm_100a) octree + RAHT hot path of GS-NFS's per-frame codec.
+ *
+ * Paper: arxiv/paper_2606_05650, "GS-NFS: Bandwidth-adaptive Streaming of Dynamic Gaussian Splats and
+ * Point Clouds"; citations are PAPER.md:L<line> of the extracted text.  Readings of passages where the
+ * paper is silent or garbled are tagged [O*]/[R*] and listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Every `d_*` pointer is CALLER-OWNED DEVICE memory (e.g. a torch tensor), 16-byte aligned.  Every
+ *    `h_*` pointer and every pointer documented "(host)" is host memory.  The library never allocates
+ *    or frees caller memory; its only state is the context's scratch, sized at gsnfs_create().
+ *  - All calls enqueue work on the given stream (a cudaStream_t passed as void*) and return without
+ *    synchronising, except the *_host frame calls, which return after their last copy completes.
+ *  - Data-dependent sizes are written to a device-resident gsnfs_counts; calls that consume them read
+ *    them on the device, so an encode can be chained with no host round trip.
+ *  - Return value: GSNFS_OK (0) or a negative gsnfs_status.  Stream corruption found on the device is
+ *    reported in gsnfs_counts.status (it cannot be known at enqueue time).
+ *  - Limits: 1 <= depth <= 21 (3*depth-bit Morton codes in 64 bits, PAPER.md:L152 [O10]);
+ *    n < 2^30; 1 <= channels <= GSNFS_MAX_CHANNELS.
+ *  - No C++ types, exceptions or torch types cross this boundary.  There is no CPU fallback.
+ */
+#ifndef GSNFS_H_
+#define GSNFS_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define GSNFS_MAX_DEPTH 21
+#define GSNFS_MAX_CHANNELS 216
+
+typedef enum gsnfs_status {
+  GSNFS_OK = 0,
+  GSNFS_E_INVALID_ARGUMENT = -1, /* NULL pointer, depth/channels/n out of range, bbox_max <= bbox_min   */
+  GSNFS_E_CAPACITY = -2,         /* n, channels or depth exceed what gsnfs_create() sized; occ too small */
+  GSNFS_E_CUDA = -3,             /* CUDA runtime error; text via gsnfs_last_error()                      */
+  GSNFS_E_CORRUPT_STREAM = -4,   /* value of gsnfs_counts.status bit 0 (set on the device by decode)     */
+  GSNFS_E_UNIMPLEMENTED = -5
+} gsnfs_status;
+
+typedef struct gsnfs_ctx gsnfs_ctx; /* opaque; owns only internal device scratch */
+typedef void* gsnfs_stream;         /* a cudaStream_t, e.g. torch.cuda.current_stream().cuda_stream */
+
+/* Device-resident result counters written by the encoder / decoder. */
+typedef struct gsnfs_counts {
+  uint32_t n_voxels;  /* N_v: occupied voxels = |L_J|                                     */
+  uint32_t occ_bytes; /* S = sum_{d<J} |L_d|: occupancy bytes emitted                     */
+  uint32_t status;    /* 0 = ok; bit 0 = corrupt stream (decode) ; bit 1 = scratch overflow */
+  uint32_t reserved;
+} gsnfs_counts;
+
+/* Dead-zone quantiser parameters (PAPER.md:L255 names the quantiser; rule is reading [R10]):
+ *   q = sign(y) * floor(|y| / qstep_c + dz_round),   y^ = sign(q) * (|q| + recon_bias*[q != 0]) * qstep_c.
+ * NULL => { 1/3, 0 }. */
+typedef struct gsnfs_quant {
+  float dz_round;
+  float recon_bias;
+} gsnfs_quant;
+
+/* ---- context ---------------------------------------------------------------------------------- */
+/* Creates a context on `device` with scratch for frames of up to max_points Gaussians, max_channels
+ * attribute channels and octree depth max_depth.  Scratch is one cudaMalloc (about
+ * max_points * (80 + 8*max_channels) bytes). */
+int gsnfs_create(gsnfs_ctx** out, int device, uint64_t max_points, int max_channels, int max_depth);
+void gsnfs_destroy(gsnfs_ctx* ctx);
+const char* gsnfs_strerror(int status);
+const char* gsnfs_last_error(const gsnfs_ctx* ctx);  /* text of the last GSNFS_E_CUDA on this context */
+const char* gsnfs_version(void);
+/* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
+uint64_t gsnfs_launch_count(const gsnfs_ctx* ctx);
+
+/* Upper bound on occupancy bytes for n points at `depth`: sum_{d<depth} min(8^d, n), rounded up to 16. */
+uint64_t gsnfs_occ_capacity(uint64_t n, int depth);
+
+/* ---- position coder, encoder side (section 2.2, Algorithm A.1) ------------------------- */
+/* fp32 positions -> breadth-first per-level occupancy bytes + Morton-sorted voxel permutation.
+ *   voxelise  [O1][O2]: v_a = clamp(floor((fp64(p_a) - fp64(lo_a)) * (2^depth / (fp64(hi_a) - fp64(lo_a)))), 0, 2^depth-1)
+ *                       with the subtraction and the product each rounded once in fp64 (no FMA).
+ *   Morton    (L136):   bit 3b = x_b, 3b+1 = y_b, 3b+2 = z_b.
+ *   sort      (L152, A.1 l.4): stable LSD radix sort of (code, original index) [O8].
+ *   unique    (L154):   voxel v = v-th run of equal codes; d_voxel_start[v] = its first sorted position.
+ *   octree    (L156-168, A.1): L_d = unique(L_{d+1} >> 3); one byte per internal node, bit i <-> child
+ *                       (node << 3) + i [O4]; level 0 first, each level contiguous, ascending code [O5].
+ * Outputs (all device): d_occ[occ_capacity] (only the first counts.occ_bytes are meaningful; the buffer
+ * is cleared by the call), d_level_sizes[depth+1] = (|L_0| .. |L_J|) [O6], d_perm[n],
+ * d_voxel_keys[n] (first N_v valid), d_voxel_start[n+1] (first N_v+1 valid; [N_v] == n), d_counts.
+ * n == 0 is valid (N_v = 0, no bytes, level sizes 0).  Non-finite positions give an unspecified (but
+ * in-range) voxel.  Errors: INVALID_ARGUMENT, CAPACITY (n/depth beyond the context, or occ_capacity <
+ * gsnfs_occ_capacity(n, depth)), CUDA. */
+int gsnfs_octree_encode(gsnfs_ctx* ctx, gsnfs_stream stream,
+                        const float* d_xyz /* n x 3 row-major */, uint64_t n,
+                        const float bbox_min[3] /* host */, const float bbox_max[3] /* host */, int depth,
+                        uint8_t* d_occ, uint64_t occ_capacity, uint32_t* d_level_sizes,
+                        uint32_t* d_perm, uint64_t* d_voxel_keys, uint32_t* d_voxel_start,
+                        gsnfs_counts* d_counts);
+
+/* Duplicate-voxel merge: merged[v][c] = mean over the Gaussians of voxel v of
+ * attr[g][c] (fp64 accumulation in sorted order, [O9]); weights[v] = count.  Rows v >= N_v untouched.
+ * N_v is read on the device from d_counts (written by gsnfs_octree_encode on the same stream). */
+int gsnfs_voxel_merge(gsnfs_ctx* ctx, gsnfs_stream stream,
+                      const float* d_attr /* n x channels row-major */, int channels, uint64_t n,
+                      const uint32_t* d_perm, const uint32_t* d_voxel_start, const gsnfs_counts* d_counts,
+                      float* d_merged /* capacity n x channels, Morton order */,
+                      uint32_t* d_weights /* capacity n */);
+
+/* ---- position coder, decoder side (section 2.3, Algorithms A.2 and A.3) ---------------- */
+/* occupancy bytes -> leaf Morton codes and integer voxel coordinates, in Morton order.
+ * level_sizes (host, depth+1 entries) is the stream header [O6]; N_v = level_sizes[depth] and
+ * occ_bytes must equal sum_{d<depth} level_sizes[d].  d_voxel_xyz is N_v x 3 (x, y, z) uint32;
+ * d_voxel_keys (N_v) may be NULL.  A zero occupancy byte or a level whose popcount sum differs from
+ * the header sets d_counts->status bit 0 [O12]; no out-of-bounds access happens either way. */
+int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream,
+                        const uint8_t* d_occ, uint64_t occ_bytes,
+                        const uint32_t* level_sizes /* host, depth+1 */, int depth,
+                        uint32_t* d_voxel_xyz, uint64_t* d_voxel_keys, gsnfs_counts* d_counts);
+
+/* ---- attribute coder: RAHT (section 3, Eq. (1), Appendix D, Algorithms A.4-A.6) ------- */
+/* Forward transform of the N_v x channels attribute rows of the Morton-sorted voxels, bottom-up over
+ * the 3*depth binary levels: siblings at level l are adjacent active entries whose codes agree above
+ * bit l-1 (A.4 l.10); a = sqrt(w0/(w0+w1)), b = sqrt(w1/(w0+w1)); low = a*y0 + b*y1 stays at the left
+ * index, high = -b*y0 + a*y1 goes to the right index (A.6 l.16-17) [R6].  The signal transformed is
+ * x_i = sqrt(w_i) * attr_i [R2]; d_weights == NULL means unit leaf weights (the paper's case).
+ * Output order ("canonical order", [R8]): row i of the Morton-sorted voxel list, row 0 = DC.
+ *   qstep (host, `channels` entries) != NULL: d_qcoeff[i][c] = sign(y) floor(|y|/qstep_c + dz_round),
+ *   saturated to int32, evaluated in fp64 from the fp32 coefficient.  d_coeff (unquantised fp32) and
+ *   d_qcoeff may each be NULL, not both; d_qcoeff requires qstep.
+ * n_voxels is the row count; if d_counts != NULL the actual N_v is read on the device from it and
+ * n_voxels is only an upper bound (rows beyond N_v are untouched). */
+int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
+                       const uint64_t* d_voxel_keys, const uint32_t* d_weights, uint64_t n_voxels,
+                       const gsnfs_counts* d_counts, int depth,
+                       const float* d_attr /* N_v x channels */, int channels,
+                       const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
+                       int32_t* d_qcoeff, float* d_coeff);
+
+/* Inverse transform (A.6 l.24-43): de-quantise (if d_qcoeff != NULL, else take d_coeff), run the same
+ * schedule top-down with low' = a*y0 - b*y1, high' = b*y0 + a*y1, then divide row i by sqrt(w_i) [R2]. */
+int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream,
+                       const uint64_t* d_voxel_keys, const uint32_t* d_weights, uint64_t n_voxels,
+                       const gsnfs_counts* d_counts, int depth,
+                       const int32_t* d_qcoeff, const float* d_coeff, int channels,
+                       const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
+                       float* d_attr_out /* N_v x channels */);
+
+/* ---- whole-frame calls on HOST buffers (copies inside; used for end-to-end timing) --------------- */
+/* encode = H2D(xyz, attr) -> octree_encode -> voxel_merge -> raht_forward(weights = counts) -> D2H.
+ * Host outputs: h_occ[occ_capacity], h_level_sizes[depth+1], h_weights[n] (first N_v valid),
+ * h_qcoeff[n x channels] (first N_v rows valid), h_counts.  Host buffers should be pinned.
+ * Returns after the results are in host memory. */
+int gsnfs_frame_encode_host(gsnfs_ctx* ctx, gsnfs_stream stream,
+                            const float* h_xyz, const float* h_attr, uint64_t n, int channels,
+                            const float bbox_min[3], const float bbox_max[3], int depth,
+                            const float* qstep, const gsnfs_quant* quant,
+                            uint8_t* h_occ, uint64_t occ_capacity, uint32_t* h_level_sizes,
+                            uint32_t* h_weights, int32_t* h_qcoeff, gsnfs_counts* h_counts);
+
+/* decode = H2D(occ, weights, qcoeff) -> octree_decode -> raht_inverse -> D2H(voxel_xyz, attr).
+ * h_weights may be NULL (unit weights).  h_voxel_xyz is N_v x 3 uint32, h_attr N_v x channels fp32. */
+int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream,
+                            const uint8_t* h_occ, uint64_t occ_bytes, const uint32_t* level_sizes, int depth,
+                            const uint32_t* h_weights, const int32_t* h_qcoeff, int channels,
+                            const float* qstep, const gsnfs_quant* quant,
+                            uint32_t* h_voxel_xyz, float* h_attr, gsnfs_counts* h_counts);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* GSNFS_H_ */

@@ -1,0 +1,306 @@
+"""Thin ctypes binding over libgsnfs.so (C ABI: include/gsnfs.h).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.  PyTorch
+supplies device memory (tensors) and the stream.  There is no CPU fallback -- if the library is
+missing or a CUDA device is absent, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_char_p, c_float, c_int, c_uint32, c_uint64, c_void_p
+
+import numpy as np
+import torch
+
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libgsnfs.so")
+_lib = None
+
+GSNFS_OK = 0
+GSNFS_E_INVALID_ARGUMENT = -1
+GSNFS_E_CAPACITY = -2
+GSNFS_E_CUDA = -3
+GSNFS_E_CORRUPT_STREAM = -4
+GSNFS_MAX_DEPTH = 21
+GSNFS_MAX_CHANNELS = 216
+
+
+class GsnfsQuant(ctypes.Structure):
+    _fields_ = [("dz_round", c_float), ("recon_bias", c_float)]
+
+
+class GsnfsCounts(ctypes.Structure):
+    _fields_ = [("n_voxels", c_uint32), ("occ_bytes", c_uint32), ("status", c_uint32), ("reserved", c_uint32)]
+
+
+class GsnfsError(RuntimeError):
+    def __init__(self, status: int, where: str, detail: str = ""):
+        self.status = status
+        super().__init__(f"{where}: {lib().gsnfs_strerror(status).decode()} ({status}) {detail}")
+
+
+_SIGNATURES = {
+    "gsnfs_create": (c_int, [POINTER(c_void_p), c_int, c_uint64, c_int, c_int]),
+    "gsnfs_destroy": (None, [c_void_p]),
+    "gsnfs_strerror": (c_char_p, [c_int]),
+    "gsnfs_last_error": (c_char_p, [c_void_p]),
+    "gsnfs_version": (c_char_p, []),
+    "gsnfs_launch_count": (c_uint64, [c_void_p]),
+    "gsnfs_occ_capacity": (c_uint64, [c_uint64, c_int]),
+    "gsnfs_octree_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, POINTER(c_float), POINTER(c_float),
+                                    c_int, c_void_p, c_uint64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "gsnfs_voxel_merge": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_uint64, c_void_p, c_void_p, c_void_p,
+                                  c_void_p, c_void_p]),
+    "gsnfs_octree_decode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, POINTER(c_uint32), c_int, c_void_p,
+                                    c_void_p, c_void_p]),
+    "gsnfs_raht_forward": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p,
+                                   c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p, c_void_p]),
+    "gsnfs_raht_inverse": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p,
+                                   c_void_p, c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p]),
+    "gsnfs_frame_encode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_int, POINTER(c_float),
+                                        POINTER(c_float), c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p,
+                                        c_uint64, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "gsnfs_frame_decode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, POINTER(c_uint32), c_int, c_void_p,
+                                        c_void_p, c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p, c_void_p,
+                                        c_void_p]),
+}
+
+
+def lib_path() -> str:
+    return _LIB_PATH
+
+
+def lib():
+    """Load libgsnfs.so (once).  Raises if it has not been built -- there is no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(_LIB_PATH):
+            raise RuntimeError(f"{_LIB_PATH} not built: run `python -m paper_2606_05650_b200.build` "
+                               "(nvcc, sm_100a).  gsnfs has no CPU fallback.")
+        L = ctypes.CDLL(_LIB_PATH)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype = res
+            fn.argtypes = args
+        _lib = L
+    return _lib
+
+
+def exported_symbols():
+    return sorted(_SIGNATURES)
+
+
+# ----------------------------------------------------------------------------- helpers
+def _dptr(t, dtype=None, name="tensor"):
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or not t.is_cuda:
+        raise TypeError(f"{name} must be a CUDA tensor")
+    if dtype is not None and t.dtype != dtype:
+        raise TypeError(f"{name} must have dtype {dtype}, got {t.dtype}")
+    if not t.is_contiguous():
+        raise ValueError(f"{name} must be contiguous")
+    return c_void_p(t.data_ptr())
+
+
+def _hptr(t, dtype, name):
+    """Host buffer (torch CPU tensor, ideally pinned)."""
+    if t is None:
+        return None
+    if not isinstance(t, torch.Tensor) or t.is_cuda or t.dtype != dtype or not t.is_contiguous():
+        raise TypeError(f"{name} must be a contiguous CPU tensor of dtype {dtype}")
+    return c_void_p(t.data_ptr())
+
+
+def _f3(v):
+    a = np.asarray(v, dtype=np.float32).reshape(3)
+    return (c_float * 3)(*a.tolist())
+
+
+def _farr(v, n):
+    if v is None:
+        return None
+    a = np.ascontiguousarray(np.asarray(v, dtype=np.float32).reshape(-1))
+    if a.shape[0] != n:
+        raise ValueError(f"expected {n} per-channel steps, got {a.shape[0]}")
+    return (c_float * n)(*a.tolist())
+
+
+def _quant(q):
+    if q is None:
+        return None
+    return ctypes.pointer(GsnfsQuant(float(q[0]), float(q[1])))
+
+
+def _stream(stream):
+    if stream is None:
+        return c_void_p(torch.cuda.current_stream().cuda_stream)
+    if isinstance(stream, torch.cuda.Stream):
+        return c_void_p(stream.cuda_stream)
+    return c_void_p(int(stream))
+
+
+def gsnfs_occ_capacity(n: int, depth: int) -> int:
+    return int(lib().gsnfs_occ_capacity(int(n), int(depth)))
+
+
+def gsnfs_version() -> str:
+    return lib().gsnfs_version().decode()
+
+
+class Context:
+    """gsnfs_ctx: owns the library's device scratch for frames up to the given sizes."""
+
+    def __init__(self, max_points: int, max_channels: int = 56, max_depth: int = GSNFS_MAX_DEPTH, device: int = 0):
+        if not torch.cuda.is_available():
+            raise RuntimeError("gsnfs needs a CUDA device (sm_100a); there is no CPU fallback")
+        h = c_void_p()
+        rc = lib().gsnfs_create(ctypes.byref(h), int(device), int(max_points), int(max_channels), int(max_depth))
+        if rc != GSNFS_OK:
+            raise GsnfsError(rc, "gsnfs_create")
+        self.handle = h
+        self.device = int(device)
+        self.max_points = int(max_points)
+        self.max_channels = int(max_channels)
+        self.max_depth = int(max_depth)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lib().gsnfs_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def launch_count(self) -> int:
+        return int(lib().gsnfs_launch_count(self.handle))
+
+    def _check(self, rc, where):
+        if rc != GSNFS_OK:
+            raise GsnfsError(rc, where, lib().gsnfs_last_error(self.handle).decode() if rc == GSNFS_E_CUDA else "")
+
+
+# ----------------------------------------------------------------------------- the ABI calls
+def gsnfs_octree_encode(ctx: Context, d_xyz, n, bbox_min, bbox_max, depth, d_occ, d_level_sizes, d_perm,
+                        d_voxel_keys, d_voxel_start, d_counts, stream=None):
+    rc = lib().gsnfs_octree_encode(
+        ctx.handle, _stream(stream), _dptr(d_xyz, torch.float32, "d_xyz"), int(n), _f3(bbox_min), _f3(bbox_max),
+        int(depth), _dptr(d_occ, torch.uint8, "d_occ"), int(d_occ.numel()),
+        _dptr(d_level_sizes, torch.int32, "d_level_sizes"), _dptr(d_perm, torch.int32, "d_perm"),
+        _dptr(d_voxel_keys, torch.int64, "d_voxel_keys"), _dptr(d_voxel_start, torch.int32, "d_voxel_start"),
+        _dptr(d_counts, torch.int32, "d_counts"))
+    ctx._check(rc, "gsnfs_octree_encode")
+
+
+def gsnfs_voxel_merge(ctx: Context, d_attr, channels, n, d_perm, d_voxel_start, d_counts, d_merged, d_weights,
+                      stream=None):
+    rc = lib().gsnfs_voxel_merge(
+        ctx.handle, _stream(stream), _dptr(d_attr, torch.float32, "d_attr"), int(channels), int(n),
+        _dptr(d_perm, torch.int32, "d_perm"), _dptr(d_voxel_start, torch.int32, "d_voxel_start"),
+        _dptr(d_counts, torch.int32, "d_counts"), _dptr(d_merged, torch.float32, "d_merged"),
+        _dptr(d_weights, torch.int32, "d_weights"))
+    ctx._check(rc, "gsnfs_voxel_merge")
+
+
+def gsnfs_octree_decode(ctx: Context, d_occ, occ_bytes, level_sizes, depth, d_voxel_xyz, d_voxel_keys, d_counts,
+                        stream=None):
+    ls = np.ascontiguousarray(np.asarray(level_sizes, dtype=np.uint32).reshape(-1))
+    if ls.shape[0] != depth + 1:
+        raise ValueError("level_sizes must have depth+1 entries")
+    arr = (c_uint32 * (depth + 1))(*ls.tolist())
+    rc = lib().gsnfs_octree_decode(
+        ctx.handle, _stream(stream), _dptr(d_occ, torch.uint8, "d_occ"), int(occ_bytes), arr, int(depth),
+        _dptr(d_voxel_xyz, torch.int32, "d_voxel_xyz"), _dptr(d_voxel_keys, torch.int64, "d_voxel_keys"),
+        _dptr(d_counts, torch.int32, "d_counts"))
+    ctx._check(rc, "gsnfs_octree_decode")
+
+
+def gsnfs_raht_forward(ctx: Context, d_voxel_keys, d_weights, n_voxels, d_counts, depth, d_attr, channels, qstep,
+                       quant, d_qcoeff, d_coeff, stream=None):
+    rc = lib().gsnfs_raht_forward(
+        ctx.handle, _stream(stream), _dptr(d_voxel_keys, torch.int64, "d_voxel_keys"),
+        _dptr(d_weights, torch.int32, "d_weights"), int(n_voxels), _dptr(d_counts, torch.int32, "d_counts"),
+        int(depth), _dptr(d_attr, torch.float32, "d_attr"), int(channels), _farr(qstep, channels), _quant(quant),
+        _dptr(d_qcoeff, torch.int32, "d_qcoeff"), _dptr(d_coeff, torch.float32, "d_coeff"))
+    ctx._check(rc, "gsnfs_raht_forward")
+
+
+def gsnfs_raht_inverse(ctx: Context, d_voxel_keys, d_weights, n_voxels, d_counts, depth, d_qcoeff, d_coeff, channels,
+                       qstep, quant, d_attr_out, stream=None):
+    rc = lib().gsnfs_raht_inverse(
+        ctx.handle, _stream(stream), _dptr(d_voxel_keys, torch.int64, "d_voxel_keys"),
+        _dptr(d_weights, torch.int32, "d_weights"), int(n_voxels), _dptr(d_counts, torch.int32, "d_counts"),
+        int(depth), _dptr(d_qcoeff, torch.int32, "d_qcoeff"), _dptr(d_coeff, torch.float32, "d_coeff"),
+        int(channels), _farr(qstep, channels), _quant(quant), _dptr(d_attr_out, torch.float32, "d_attr_out"))
+    ctx._check(rc, "gsnfs_raht_inverse")
+
+
+def gsnfs_frame_encode_host(ctx: Context, h_xyz, h_attr, n, channels, bbox_min, bbox_max, depth, qstep, quant,
+                            h_occ, h_level_sizes, h_weights, h_qcoeff, h_counts, stream=None):
+    rc = lib().gsnfs_frame_encode_host(
+        ctx.handle, _stream(stream), _hptr(h_xyz, torch.float32, "h_xyz"), _hptr(h_attr, torch.float32, "h_attr"),
+        int(n), int(channels), _f3(bbox_min), _f3(bbox_max), int(depth), _farr(qstep, channels), _quant(quant),
+        _hptr(h_occ, torch.uint8, "h_occ"), int(h_occ.numel()), _hptr(h_level_sizes, torch.int32, "h_level_sizes"),
+        _hptr(h_weights, torch.int32, "h_weights"), _hptr(h_qcoeff, torch.int32, "h_qcoeff"),
+        _hptr(h_counts, torch.int32, "h_counts"))
+    ctx._check(rc, "gsnfs_frame_encode_host")
+
+
+def gsnfs_frame_decode_host(ctx: Context, h_occ, occ_bytes, level_sizes, depth, h_weights, h_qcoeff, channels, qstep,
+                            quant, h_voxel_xyz, h_attr, h_counts, stream=None):
+    ls = np.ascontiguousarray(np.asarray(level_sizes, dtype=np.uint32).reshape(-1))
+    arr = (c_uint32 * (depth + 1))(*ls.tolist())
+    rc = lib().gsnfs_frame_decode_host(
+        ctx.handle, _stream(stream), _hptr(h_occ, torch.uint8, "h_occ"), int(occ_bytes), arr, int(depth),
+        _hptr(h_weights, torch.int32, "h_weights"), _hptr(h_qcoeff, torch.int32, "h_qcoeff"), int(channels),
+        _farr(qstep, channels), _quant(quant), _hptr(h_voxel_xyz, torch.int32, "h_voxel_xyz"),
+        _hptr(h_attr, torch.float32, "h_attr"), _hptr(h_counts, torch.int32, "h_counts"))
+    ctx._check(rc, "gsnfs_frame_decode_host")
+
+
+# ----------------------------------------------------------------------------- buffer bundle
+class FrameBuffers:
+    """Caller-owned device buffers for one frame (allocated by PyTorch; the library only fills them)."""
+
+    def __init__(self, n: int, channels: int, depth: int, device="cuda:0"):
+        dev = torch.device(device)
+        self.n, self.channels, self.depth = int(n), int(channels), int(depth)
+        cap = max(gsnfs_occ_capacity(n, depth), 16)
+        n1 = max(n, 1)
+        self.occ = torch.empty(cap, dtype=torch.uint8, device=dev)
+        self.level_sizes = torch.zeros(depth + 1, dtype=torch.int32, device=dev)
+        self.perm = torch.empty(n1, dtype=torch.int32, device=dev)
+        self.voxel_keys = torch.empty(n1, dtype=torch.int64, device=dev)
+        self.voxel_start = torch.empty(n1 + 1, dtype=torch.int32, device=dev)
+        self.counts = torch.zeros(4, dtype=torch.int32, device=dev)
+        self.merged = torch.empty((n1, channels), dtype=torch.float32, device=dev)
+        self.weights = torch.empty(n1, dtype=torch.int32, device=dev)
+        self.qcoeff = torch.empty((n1, channels), dtype=torch.int32, device=dev)
+        # decoder side
+        self.dec_xyz = torch.empty((n1, 3), dtype=torch.int32, device=dev)
+        self.dec_keys = torch.empty(n1, dtype=torch.int64, device=dev)
+        self.dec_counts = torch.zeros(4, dtype=torch.int32, device=dev)
+        self.dec_attr = torch.empty((n1, channels), dtype=torch.float32, device=dev)
+
+
+def encode_frame(ctx: Context, buf: FrameBuffers, d_xyz, d_attr, bbox_min, bbox_max, qstep, quant=None, stream=None):
+    """The encoder's three ABI calls chained on one stream with no host synchronisation."""
+    gsnfs_octree_encode(ctx, d_xyz, buf.n, bbox_min, bbox_max, buf.depth, buf.occ, buf.level_sizes, buf.perm,
+                        buf.voxel_keys, buf.voxel_start, buf.counts, stream)
+    gsnfs_voxel_merge(ctx, d_attr, buf.channels, buf.n, buf.perm, buf.voxel_start, buf.counts, buf.merged,
+                      buf.weights, stream)
+    gsnfs_raht_forward(ctx, buf.voxel_keys, buf.weights, buf.n, buf.counts, buf.depth, buf.merged, buf.channels,
+                       qstep, quant, buf.qcoeff, None, stream)
+
+
+def decode_frame(ctx: Context, buf: FrameBuffers, level_sizes, occ_bytes, qstep, quant=None, use_weights=True,
+                 stream=None):
+    """The decoder's two ABI calls.  level_sizes is the host-side stream header."""
+    nv = int(level_sizes[buf.depth])
+    gsnfs_octree_decode(ctx, buf.occ, occ_bytes, level_sizes, buf.depth, buf.dec_xyz, buf.dec_keys, buf.dec_counts,
+                        stream)
+    gsnfs_raht_inverse(ctx, buf.dec_keys, buf.weights if use_weights else None, nv, None, buf.depth, buf.qcoeff, None,
+                       buf.channels, qstep, quant, buf.dec_attr, stream)

@@ -1,0 +1,320 @@
+// C ABI of libgsnfs.so (see include/gsnfs.h): argument validation, context scratch, stage drivers.
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+
+#include "common.cuh"
+
+namespace gsnfs {
+int octree_encode_setup(gsnfs_ctx* ctx);
+
+struct Bump {
+  size_t off = 0;
+  size_t take(size_t bytes) {
+    const size_t o = off;
+    off += (bytes + 255) & ~(size_t)255;
+    return o;
+  }
+};
+}  // namespace gsnfs
+
+using namespace gsnfs;
+
+extern "C" {
+
+const char* gsnfs_version(void) { return "gsnfs-b200 0.1 (sm_100a)"; }
+
+const char* gsnfs_strerror(int status) {
+  switch (status) {
+    case GSNFS_OK: return "ok";
+    case GSNFS_E_INVALID_ARGUMENT: return "invalid argument";
+    case GSNFS_E_CAPACITY: return "capacity exceeded (context scratch or caller buffer too small)";
+    case GSNFS_E_CUDA: return "CUDA error (see gsnfs_last_error)";
+    case GSNFS_E_CORRUPT_STREAM: return "corrupt occupancy stream";
+    case GSNFS_E_UNIMPLEMENTED: return "not implemented";
+    default: return "unknown status";
+  }
+}
+
+const char* gsnfs_last_error(const gsnfs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+uint64_t gsnfs_launch_count(const gsnfs_ctx* ctx) { return ctx ? ctx->launches : 0; }
+
+uint64_t gsnfs_occ_capacity(uint64_t n, int depth) {
+  if (depth < 1 || depth > GSNFS_MAX_DEPTH) return 0;
+  uint64_t s = 0, pw = 1;
+  for (int d = 0; d < depth; ++d) {
+    s += pw < n ? pw : n;
+    if (pw < (1ull << 62)) pw <<= 3;
+  }
+  return (s + 15) & ~15ull;
+}
+
+static int create_impl(gsnfs_ctx* c) {
+  GSNFS_CUDA_OK(c, cudaSetDevice(c->device));
+  cudaDeviceProp prop;
+  GSNFS_CUDA_OK(c, cudaGetDeviceProperties(&prop, c->device));
+  c->num_sms = prop.multiProcessorCount;
+  if (!prop.cooperativeLaunch) {
+    snprintf(c->err, sizeof(c->err), "device lacks cooperative launch");
+    return GSNFS_E_CUDA;
+  }
+  const uint64_t N = c->max_points;
+  const int C = c->max_channels;
+  const uint64_t stiles = (N + kSortTile - 1) / kSortTile + 1;
+  const uint64_t otiles = (N + kOctTile - 1) / kOctTile + 1;
+  c->oct_tiles_cap = (uint32_t)otiles;
+  c->occ_cap = gsnfs_occ_capacity(N, c->max_depth) + 16;
+  c->scan_tiles_cap = (uint32_t)((c->occ_cap > N ? c->occ_cap : N) / kScanTile + 2);
+  c->raht_pool_rows = N + 8192;
+  c->raht_hdr_cap = 2 * N / kRahtTile + 4 * kRahtMaxPhases + 64;
+  c->raht_rec_cap = c->raht_hdr_cap * kRahtTile;
+
+  Bump b;
+  const size_t o_keys_a = b.take(N * 8), o_keys_b = b.take(N * 8);
+  const size_t o_pay_a = b.take(N * 4), o_pay_b = b.take(N * 4);
+  const size_t o_hist = b.take((size_t)kSortMaxPasses * 256 * 4);
+  const size_t o_status = b.take((size_t)kSortMaxPasses * stiles * 256 * 4);
+  const size_t o_ticket = b.take((size_t)kSortMaxPasses * 4);
+  const size_t o_zero_end = b.off;
+  const size_t o_ohist = b.take((size_t)kOctLevels * otiles * 4), o_obase = b.take((size_t)kOctLevels * otiles * 4);
+  const size_t o_ometa = b.take((size_t)2 * kOctLevels * 4);
+  const size_t o_ssums = b.take((size_t)c->scan_tiles_cap * 4);
+  const size_t o_wpref = b.take((N + 1) * 4);
+  const size_t o_ridx = b.take(c->raht_pool_rows * 4);
+  const size_t o_rrec = b.take(c->raht_rec_cap * sizeof(uint4));
+  const size_t o_rhdr = b.take(c->raht_hdr_cap * sizeof(RahtTileHdr));
+  const size_t o_rtp = b.take((N / kRahtTile + 2) * 4);
+  const size_t o_rplan = b.take(sizeof(RahtPlan));
+  const size_t o_rrows = b.take(c->raht_pool_rows * (size_t)C * 4);
+  const size_t o_dscan = b.take((c->occ_cap + 1) * 4);
+  const size_t o_dka = b.take((N + 1) * 8), o_dkb = b.take((N + 1) * 8);
+  c->pool_bytes = b.off;
+  GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->pool, c->pool_bytes));
+  char* p = c->pool;
+  c->keys_a = p + o_keys_a; c->keys_b = p + o_keys_b;
+  c->pay_a = (uint32_t*)(p + o_pay_a); c->pay_b = (uint32_t*)(p + o_pay_b);
+  c->hist = (uint32_t*)(p + o_hist); c->sort_status = (uint32_t*)(p + o_status);
+  c->sort_ticket = (uint32_t*)(p + o_ticket);
+  c->sort_zero_bytes = o_zero_end - o_hist;
+  c->oct_hist = (uint32_t*)(p + o_ohist); c->oct_base = (uint32_t*)(p + o_obase); c->oct_meta = (uint32_t*)(p + o_ometa);
+  c->scan_sums = (uint32_t*)(p + o_ssums);
+  c->wprefix = (uint32_t*)(p + o_wpref);
+  c->raht_idx = (uint32_t*)(p + o_ridx); c->raht_rec = (uint4*)(p + o_rrec);
+  c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
+  c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
+  c->dec_scan = (uint32_t*)(p + o_dscan); c->dec_keys_a = (uint64_t*)(p + o_dka); c->dec_keys_b = (uint64_t*)(p + o_dkb);
+  GSNFS_CUDA_OK(c, cudaMemset(c->pool, 0, o_rrows));     // everything but the big row pool
+  int rc = octree_encode_setup(c);
+  if (rc != GSNFS_OK) return rc;
+  return raht_setup(c);
+}
+
+int gsnfs_create(gsnfs_ctx** out, int device, uint64_t max_points, int max_channels, int max_depth) {
+  if (!out) return GSNFS_E_INVALID_ARGUMENT;
+  *out = nullptr;
+  if (max_points == 0 || max_points >= (1ull << 30) || max_channels < 1 || max_channels > GSNFS_MAX_CHANNELS ||
+      max_depth < 1 || max_depth > GSNFS_MAX_DEPTH)
+    return GSNFS_E_INVALID_ARGUMENT;
+  gsnfs_ctx* c = (gsnfs_ctx*)calloc(1, sizeof(gsnfs_ctx));
+  if (!c) return GSNFS_E_CAPACITY;
+  c->device = device;
+  c->max_points = max_points;
+  c->max_channels = max_channels;
+  c->max_depth = max_depth;
+  const int rc = create_impl(c);
+  if (rc != GSNFS_OK) {
+    fprintf(stderr, "gsnfs_create failed: %s\n", c->err);
+    if (c->pool) cudaFree(c->pool);
+    free(c);
+    return rc;
+  }
+  *out = c;
+  return GSNFS_OK;
+}
+
+void gsnfs_destroy(gsnfs_ctx* ctx) {
+  if (!ctx) return;
+  cudaSetDevice(ctx->device);
+  if (ctx->pool) cudaFree(ctx->pool);
+  if (ctx->fpool) cudaFree(ctx->fpool);
+  free(ctx);
+}
+
+int gsnfs_octree_encode(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_xyz, uint64_t n, const float bbox_min[3],
+                        const float bbox_max[3], int depth, uint8_t* d_occ, uint64_t occ_capacity,
+                        uint32_t* d_level_sizes, uint32_t* d_perm, uint64_t* d_voxel_keys, uint32_t* d_voxel_start,
+                        gsnfs_counts* d_counts) {
+  if (!ctx || !bbox_min || !bbox_max || !d_occ || !d_level_sizes || !d_voxel_start || !d_counts ||
+      (n && (!d_xyz || !d_perm || !d_voxel_keys)))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (depth < 1 || depth > GSNFS_MAX_DEPTH || n >= (1ull << 30)) return GSNFS_E_INVALID_ARGUMENT;
+  double lo[3], scale[3];
+  for (int a = 0; a < 3; ++a) {
+    const double l = (double)bbox_min[a], h = (double)bbox_max[a];
+    if (!(h > l) || !isfinite(l) || !isfinite(h)) return GSNFS_E_INVALID_ARGUMENT;
+    lo[a] = l;
+    scale[a] = ldexp(1.0, depth) / (h - l);          // [O2] computed once on the host in fp64
+  }
+  if (n > ctx->max_points || depth > ctx->max_depth) return GSNFS_E_CAPACITY;
+  if (occ_capacity < gsnfs_occ_capacity(n, depth) || (occ_capacity & 3)) return GSNFS_E_CAPACITY;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return run_octree_encode(ctx, (cudaStream_t)stream, d_xyz, (uint32_t)n, lo, scale, depth, d_occ, occ_capacity,
+                           d_level_sizes, d_perm, d_voxel_keys, d_voxel_start, d_counts);
+}
+
+int gsnfs_voxel_merge(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr, int channels, uint64_t n,
+                      const uint32_t* d_perm, const uint32_t* d_voxel_start, const gsnfs_counts* d_counts,
+                      float* d_merged, uint32_t* d_weights) {
+  if (!ctx || !d_voxel_start || !d_counts || (n && (!d_attr || !d_perm || !d_merged || !d_weights)))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (channels < 1 || channels > GSNFS_MAX_CHANNELS || n >= (1ull << 30)) return GSNFS_E_INVALID_ARGUMENT;
+  if (n > ctx->max_points) return GSNFS_E_CAPACITY;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return run_voxel_merge(ctx, (cudaStream_t)stream, d_attr, channels, (uint32_t)n, d_perm, d_voxel_start, d_counts,
+                         d_merged, d_weights);
+}
+
+int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_occ, uint64_t occ_bytes,
+                        const uint32_t* level_sizes, int depth, uint32_t* d_voxel_xyz, uint64_t* d_voxel_keys,
+                        gsnfs_counts* d_counts) {
+  if (!ctx || !level_sizes || !d_counts) return GSNFS_E_INVALID_ARGUMENT;
+  if (depth < 1 || depth > GSNFS_MAX_DEPTH) return GSNFS_E_INVALID_ARGUMENT;
+  if (level_sizes[depth] && (!d_occ || !d_voxel_xyz)) return GSNFS_E_INVALID_ARGUMENT;
+  if (depth > ctx->max_depth) return GSNFS_E_CAPACITY;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return run_octree_decode(ctx, (cudaStream_t)stream, d_occ, occ_bytes, level_sizes, depth, d_voxel_xyz, d_voxel_keys,
+                           d_counts);
+}
+
+static int raht_check(gsnfs_ctx* ctx, const uint64_t* keys, uint64_t n, int depth, int channels) {
+  if (!ctx || (n && !keys)) return GSNFS_E_INVALID_ARGUMENT;
+  if (depth < 1 || depth > GSNFS_MAX_DEPTH || channels < 1 || channels > GSNFS_MAX_CHANNELS || n >= (1ull << 30))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (n > ctx->max_points || channels > ctx->max_channels) return GSNFS_E_CAPACITY;
+  return GSNFS_OK;
+}
+
+int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_weights,
+                       uint64_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_attr, int channels,
+                       const float* qstep, const gsnfs_quant* quant, int32_t* d_qcoeff, float* d_coeff) {
+  int rc = raht_check(ctx, d_voxel_keys, n_voxels, depth, channels);
+  if (rc != GSNFS_OK) return rc;
+  if (n_voxels && (!d_attr || (!d_qcoeff && !d_coeff) || (d_qcoeff && !qstep))) return GSNFS_E_INVALID_ARGUMENT;
+  if (qstep)
+    for (int c = 0; c < channels; ++c)
+      if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return run_raht(ctx, (cudaStream_t)stream, false, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth, d_attr,
+                  nullptr, channels, qstep, quant, d_qcoeff, d_coeff);
+}
+
+int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_weights,
+                       uint64_t n_voxels, const gsnfs_counts* d_counts, int depth, const int32_t* d_qcoeff,
+                       const float* d_coeff, int channels, const float* qstep, const gsnfs_quant* quant,
+                       float* d_attr_out) {
+  int rc = raht_check(ctx, d_voxel_keys, n_voxels, depth, channels);
+  if (rc != GSNFS_OK) return rc;
+  if (n_voxels && (!d_attr_out || (!d_qcoeff && !d_coeff) || (d_qcoeff && !qstep))) return GSNFS_E_INVALID_ARGUMENT;
+  if (qstep)
+    for (int c = 0; c < channels; ++c)
+      if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return run_raht(ctx, (cudaStream_t)stream, true, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth, d_coeff,
+                  d_qcoeff, channels, d_qcoeff ? qstep : nullptr, quant, nullptr, d_attr_out);
+}
+
+// ---- whole-frame calls on host buffers -----------------------------------------------------------
+static int frame_pool(gsnfs_ctx* c) {
+  if (c->fpool) return GSNFS_OK;
+  const uint64_t N = c->max_points;
+  const size_t C = (size_t)c->max_channels;
+  Bump b;
+  const size_t o_xyz = b.take(N * 12), o_attr = b.take(N * C * 4), o_mrg = b.take(N * C * 4), o_q = b.take(N * C * 4);
+  const size_t o_occ = b.take(c->occ_cap), o_lev = b.take(256), o_perm = b.take(N * 4), o_vk = b.take(N * 8);
+  const size_t o_vs = b.take((N + 1) * 4), o_w = b.take(N * 4), o_vx = b.take(N * 12), o_cnt = b.take(256);
+  c->fpool_bytes = b.off;
+  GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->fpool, c->fpool_bytes));
+  char* p = c->fpool;
+  c->f_xyz = (float*)(p + o_xyz); c->f_attr = (float*)(p + o_attr); c->f_merged = (float*)(p + o_mrg);
+  c->f_q = (int32_t*)(p + o_q); c->f_occ = (uint8_t*)(p + o_occ); c->f_levels = (uint32_t*)(p + o_lev);
+  c->f_perm = (uint32_t*)(p + o_perm); c->f_vkeys = (uint64_t*)(p + o_vk); c->f_vstart = (uint32_t*)(p + o_vs);
+  c->f_weights = (uint32_t*)(p + o_w); c->f_vxyz = (uint32_t*)(p + o_vx); c->f_counts = (gsnfs_counts*)(p + o_cnt);
+  return GSNFS_OK;
+}
+
+int gsnfs_frame_encode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
+                            int channels, const float bbox_min[3], const float bbox_max[3], int depth,
+                            const float* qstep, const gsnfs_quant* quant, uint8_t* h_occ, uint64_t occ_capacity,
+                            uint32_t* h_level_sizes, uint32_t* h_weights, int32_t* h_qcoeff, gsnfs_counts* h_counts) {
+  if (!ctx || !h_occ || !h_level_sizes || !h_counts || !qstep || (n && (!h_xyz || !h_attr || !h_weights || !h_qcoeff)))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (n > ctx->max_points || channels > ctx->max_channels || channels < 1) return GSNFS_E_CAPACITY;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  int rc = frame_pool(ctx);
+  if (rc != GSNFS_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint64_t cap = gsnfs_occ_capacity(n, depth);
+  if (cap == 0 || occ_capacity < cap || cap > ctx->occ_cap) return depth < 1 || depth > GSNFS_MAX_DEPTH ? GSNFS_E_INVALID_ARGUMENT : GSNFS_E_CAPACITY;
+  const size_t C = (size_t)channels;
+  if (n) {
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_xyz, h_xyz, n * 12, cudaMemcpyHostToDevice, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_attr, h_attr, n * C * 4, cudaMemcpyHostToDevice, st));
+  }
+  rc = gsnfs_octree_encode(ctx, stream, ctx->f_xyz, n, bbox_min, bbox_max, depth, ctx->f_occ, cap, ctx->f_levels,
+                           ctx->f_perm, ctx->f_vkeys, ctx->f_vstart, ctx->f_counts);
+  if (rc != GSNFS_OK) return rc;
+  rc = gsnfs_voxel_merge(ctx, stream, ctx->f_attr, channels, n, ctx->f_perm, ctx->f_vstart, ctx->f_counts, ctx->f_merged,
+                         ctx->f_weights);
+  if (rc != GSNFS_OK) return rc;
+  rc = gsnfs_raht_forward(ctx, stream, ctx->f_vkeys, ctx->f_weights, n, ctx->f_counts, depth, ctx->f_merged, channels,
+                          qstep, quant, ctx->f_q, nullptr);
+  if (rc != GSNFS_OK) return rc;
+  // header first: the sizes of the remaining copies depend on it
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_counts, ctx->f_counts, sizeof(gsnfs_counts), cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_level_sizes, ctx->f_levels, sizeof(uint32_t) * (depth + 1), cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  const uint64_t nv = h_counts->n_voxels, ob = h_counts->occ_bytes;
+  if (nv) {
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_occ, ctx->f_occ, ob, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_weights, ctx->f_weights, nv * 4, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_qcoeff, ctx->f_q, nv * C * 4, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  }
+  return GSNFS_OK;
+}
+
+int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
+                            const uint32_t* level_sizes, int depth, const uint32_t* h_weights, const int32_t* h_qcoeff,
+                            int channels, const float* qstep, const gsnfs_quant* quant, uint32_t* h_voxel_xyz,
+                            float* h_attr, gsnfs_counts* h_counts) {
+  if (!ctx || !level_sizes || !h_counts || !qstep) return GSNFS_E_INVALID_ARGUMENT;
+  if (depth < 1 || depth > GSNFS_MAX_DEPTH) return GSNFS_E_INVALID_ARGUMENT;
+  const uint64_t nv = level_sizes[depth];
+  if (nv && (!h_occ || !h_qcoeff || !h_voxel_xyz || !h_attr)) return GSNFS_E_INVALID_ARGUMENT;
+  if (nv > ctx->max_points || channels > ctx->max_channels || channels < 1 || occ_bytes + 1 > ctx->occ_cap)
+    return GSNFS_E_CAPACITY;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  int rc = frame_pool(ctx);
+  if (rc != GSNFS_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const size_t C = (size_t)channels;
+  if (nv) {
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_occ, h_occ, occ_bytes, cudaMemcpyHostToDevice, st));
+    if (h_weights) GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_weights, h_weights, nv * 4, cudaMemcpyHostToDevice, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_q, h_qcoeff, nv * C * 4, cudaMemcpyHostToDevice, st));
+  }
+  rc = gsnfs_octree_decode(ctx, stream, ctx->f_occ, occ_bytes, level_sizes, depth, ctx->f_vxyz, ctx->f_vkeys, ctx->f_counts);
+  if (rc != GSNFS_OK) return rc;
+  rc = gsnfs_raht_inverse(ctx, stream, ctx->f_vkeys, h_weights ? ctx->f_weights : nullptr, nv, nullptr, depth, ctx->f_q,
+                          nullptr, channels, qstep, quant, ctx->f_attr);
+  if (rc != GSNFS_OK) return rc;
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_counts, ctx->f_counts, sizeof(gsnfs_counts), cudaMemcpyDeviceToHost, st));
+  if (nv) {
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_voxel_xyz, ctx->f_vxyz, nv * 12, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_attr, ctx->f_attr, nv * C * 4, cudaMemcpyDeviceToHost, st));
+  }
+  GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  return GSNFS_OK;
+}
+
+}  // extern "C"

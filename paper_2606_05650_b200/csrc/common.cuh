@@ -1,0 +1,211 @@
+// Internal definitions shared by the gsnfs CUDA translation units (sm_100a only).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+
+#include "gsnfs.h"
+
+namespace gsnfs {
+
+constexpr int kRahtTile = 256;       // entries per RAHT tile (rows staged in shared memory)
+constexpr int kRahtMaxPhases = 30;   // >= worst-case number of tile phases
+constexpr int kSortItems = 16;       // keys per thread in a onesweep tile
+constexpr int kSortThreads = 256;
+constexpr int kSortTile = kSortItems * kSortThreads;
+constexpr int kSortMaxPasses = 8;    // ceil(63 / 8)
+constexpr int kOctTile = 2048;       // sorted keys per octree-build tile
+constexpr int kOctLevels = 24;       // >= GSNFS_MAX_DEPTH + 2
+constexpr int kScanTile = 2048;
+
+struct SortPlan {
+  int passes;
+  int shift[kSortMaxPasses];
+  int bits[kSortMaxPasses];
+};
+
+// Per-tile header of the RAHT schedule (one per tile per phase).
+struct __align__(16) RahtTileHdr {
+  uint16_t lev_end[64];   // lev_end[l-1] = number of local merges with level <= l  (l = 1..64)
+  uint32_t pendmask[8];   // bit k set: entry k of the tile stays pending after this phase
+  uint32_t pend_off;      // exclusive prefix of pending counts over the phase's earlier tiles
+  uint32_t npend;
+  uint32_t nent;          // valid entries in the tile
+  uint32_t nmerge;
+};
+static_assert(sizeof(RahtTileHdr) == 176, "RahtTileHdr layout");
+
+// Device-resident description of the phase structure (data dependent).
+struct RahtPlan {
+  uint32_t nphases;
+  uint32_t overflow;
+  uint32_t M[kRahtMaxPhases + 2];     // active entries of phase p (1-based); M[1] = N_v
+  uint32_t poff[kRahtMaxPhases + 2];  // row offset of phase p (p >= 2) in the idx / pending-row pools
+  uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
+};
+
+struct Region {
+  void* p;
+  size_t bytes;
+};
+
+}  // namespace gsnfs
+
+struct gsnfs_ctx {
+  int device;
+  int num_sms;
+  uint64_t max_points;
+  int max_channels;
+  int max_depth;
+  uint64_t launches;
+  char err[256];
+
+  char* pool;
+  size_t pool_bytes;
+
+  // sort + octree build
+  void* keys_a;            // max_points x 8
+  void* keys_b;            // max_points x 8
+  uint32_t* pay_a;
+  uint32_t* pay_b;
+  uint32_t* hist;          // kSortMaxPasses x 256
+  uint32_t* sort_status;   // kSortMaxPasses x tiles x 256
+  uint32_t* sort_ticket;   // kSortMaxPasses
+  size_t sort_zero_bytes;  // hist..ticket are contiguous; cleared by one memset
+  uint32_t* oct_hist;      // kOctLevels x oct_tiles (level-major)
+  uint32_t* oct_base;      // kOctLevels x oct_tiles
+  uint32_t* oct_meta;      // level sizes [kOctLevels] + level offsets [kOctLevels]
+  uint32_t oct_tiles_cap;
+
+  // generic scan scratch
+  uint32_t* scan_sums;     // per-tile sums
+  uint32_t scan_tiles_cap;
+
+  // RAHT
+  uint32_t* wprefix;       // max_points + 1
+  uint32_t* raht_idx;      // idx pool for phases >= 2
+  uint4* raht_rec;         // merge records
+  gsnfs::RahtTileHdr* raht_hdr;
+  uint32_t* raht_tile_pend;
+  gsnfs::RahtPlan* raht_plan;
+  float* raht_rows;        // pending-row pool (phases >= 2)
+  uint64_t raht_pool_rows; // capacity (rows) of raht_idx / raht_rows
+  uint64_t raht_rec_cap;
+  uint64_t raht_hdr_cap;
+  float* qparams;          // 2 x max_channels doubles (inv step / step) stored as double
+  int raht_grid_sched, raht_grid_fwd, raht_grid_inv;
+
+  // decode
+  uint32_t* dec_scan;      // exclusive popcount scan over the stream (one per byte)
+  uint64_t* dec_keys_a;    // ping-pong level key lists
+  uint64_t* dec_keys_b;
+  uint64_t occ_cap;
+
+  // host-frame staging (allocated on first use)
+  char* fpool;
+  size_t fpool_bytes;
+  float* f_xyz;
+  float* f_attr;
+  float* f_merged;
+  int32_t* f_q;
+  uint8_t* f_occ;
+  uint32_t* f_levels;
+  uint32_t* f_perm;
+  uint64_t* f_vkeys;
+  uint32_t* f_vstart;
+  uint32_t* f_weights;
+  uint32_t* f_vxyz;
+  gsnfs_counts* f_counts;
+};
+
+namespace gsnfs {
+
+#define GSNFS_CUDA_OK(ctx, expr)                                                              \
+  do {                                                                                        \
+    cudaError_t e__ = (expr);                                                                 \
+    if (e__ != cudaSuccess) {                                                                 \
+      snprintf((ctx)->err, sizeof((ctx)->err), "%s:%d %s: %s", __FILE__, __LINE__, #expr,     \
+               cudaGetErrorString(e__));                                                      \
+      return GSNFS_E_CUDA;                                                                    \
+    }                                                                                         \
+  } while (0)
+
+#define GSNFS_LAUNCH_CHECK(ctx)                 \
+  do {                                          \
+    (ctx)->launches++;                          \
+    GSNFS_CUDA_OK(ctx, cudaPeekAtLastError());  \
+  } while (0)
+
+__device__ __forceinline__ int msb64(unsigned long long x) { return 63 - __clzll((long long)x); }
+__device__ __forceinline__ unsigned lanemask_lt() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_lt;" : "=r"(m));
+  return m;
+}
+__device__ __forceinline__ unsigned lanemask_le() {
+  unsigned m;
+  asm("mov.u32 %0, %%lanemask_le;" : "=r"(m));
+  return m;
+}
+__device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
+  uint32_t v;
+  asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_volatile_u32(uint32_t* p, uint32_t v) {
+  asm volatile("st.volatile.global.u32 [%0], %1;" ::"l"(p), "r"(v) : "memory");
+}
+
+// Exclusive scan of one value per thread over a 256-thread block.  `total` (optional) gets the sum.
+__device__ __forceinline__ uint32_t block_excl_scan_256(uint32_t v, uint32_t* s_warp /*>= 9*/, uint32_t* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  uint32_t inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) {
+    uint32_t t = __shfl_up_sync(0xffffffffu, inc, o);
+    if (lane >= o) inc += t;
+  }
+  if (lane == 31) s_warp[warp] = inc;
+  __syncthreads();
+  if (warp == 0) {
+    uint32_t w = lane < 8 ? s_warp[lane] : 0;
+    uint32_t winc = w;
+#pragma unroll
+    for (int o = 1; o < 8; o <<= 1) {
+      uint32_t t = __shfl_up_sync(0xffffffffu, winc, o);
+      if (lane >= o) winc += t;
+    }
+    if (lane < 8) s_warp[lane] = winc - w;
+    if (lane == 7) s_warp[8] = winc;
+  }
+  __syncthreads();
+  uint32_t res = inc - v + s_warp[warp];
+  if (total) *total = s_warp[8];
+  __syncthreads();
+  return res;
+}
+
+// ---- entry points of the stage drivers (one per .cu) -------------------------------------------
+int run_octree_encode(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint32_t n, const double lo[3],
+                      const double scale[3], int depth, uint8_t* d_occ, uint64_t occ_capacity,
+                      uint32_t* d_level_sizes, uint32_t* d_perm, uint64_t* d_voxel_keys,
+                      uint32_t* d_voxel_start, gsnfs_counts* d_counts);
+int run_voxel_merge(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, int channels, uint32_t n,
+                    const uint32_t* d_perm, const uint32_t* d_voxel_start, const gsnfs_counts* d_counts,
+                    float* d_merged, uint32_t* d_weights);
+int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uint64_t occ_bytes,
+                      const uint32_t* level_sizes, int depth, uint32_t* d_voxel_xyz, uint64_t* d_voxel_keys,
+                      gsnfs_counts* d_counts);
+int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_keys, const uint32_t* d_weights,
+             uint32_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_in_f,
+             const int32_t* d_in_q, int channels, const float* qstep, const gsnfs_quant* quant,
+             int32_t* d_out_q, float* d_out_f);
+int raht_setup(gsnfs_ctx* ctx);   // occupancy queries + attributes, called from gsnfs_create
+
+// generic exclusive scan of uint32 (weights) with the element count read on the device
+int run_scan_u32(gsnfs_ctx* ctx, cudaStream_t st, const uint32_t* d_in, uint32_t* d_out /* n+1 */,
+                 uint32_t n_cap, const uint32_t* d_n /* may be NULL => n_cap */);
+// exclusive scan of popcount(byte)
+int run_scan_popc8(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_in, uint32_t* d_out /* n+1 */, uint32_t n);
+
+}  // namespace gsnfs

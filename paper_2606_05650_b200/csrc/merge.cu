@@ -1,0 +1,90 @@
+// Duplicate-voxel merge as a segmented reduction: the attributes of the
+// Gaussians that fall into one voxel are replaced by their arithmetic mean [O9]; weight = count.
+// Rows are gathered through the sorted permutation; a voxel holding one Gaussian (the common case)
+// is a straight 16-byte-vector row copy, so the kernel is a 2 x 4C bytes/voxel HBM stream.
+#include <type_traits>
+
+#include "common.cuh"
+
+namespace gsnfs {
+
+// VEC = 4: channels % 4 == 0, rows moved as float4 (rows are then 16-byte aligned);  VEC = 1: any C.
+// Layout: threadIdx.x = vector lane inside a row (16 lanes), threadIdx.y = row slot; each thread keeps
+// ROWS independent rows in flight to cover the start -> perm -> row dependent-load chain.
+template <int VEC, int ROWS>
+__global__ void __launch_bounds__(256) merge_kernel(const float* __restrict__ attr, int C,
+                                                    const uint32_t* __restrict__ perm,
+                                                    const uint32_t* __restrict__ vstart,
+                                                    const gsnfs_counts* __restrict__ counts,
+                                                    float* __restrict__ merged, uint32_t* __restrict__ weights) {
+  using VecT = typename std::conditional<VEC == 4, float4, float>::type;
+  const uint32_t nv = counts->n_voxels;
+  const int cv = C / VEC;                       // vectors per row
+  const int lane = threadIdx.x;                 // 0..15
+  const uint32_t rows_per_block = 16 * ROWS;
+  for (uint32_t r0 = blockIdx.x * rows_per_block; r0 < nv; r0 += gridDim.x * rows_per_block) {
+    uint32_t s[ROWS], e[ROWS], g[ROWS];
+#pragma unroll
+    for (int k = 0; k < ROWS; ++k) {
+      const uint32_t v = r0 + threadIdx.y + 16 * k;
+      s[k] = v < nv ? vstart[v] : 0u;
+      e[k] = v < nv ? vstart[v + 1] : 0u;
+    }
+#pragma unroll
+    for (int k = 0; k < ROWS; ++k) g[k] = (e[k] > s[k]) ? perm[s[k]] : 0u;
+    for (int c = lane; c < cv; c += 16) {
+      VecT x[ROWS];
+#pragma unroll
+      for (int k = 0; k < ROWS; ++k)
+        if (e[k] > s[k]) x[k] = reinterpret_cast<const VecT*>(attr + (size_t)g[k] * C)[c];
+#pragma unroll
+      for (int k = 0; k < ROWS; ++k) {
+        const uint32_t v = r0 + threadIdx.y + 16 * k;
+        if (e[k] <= s[k]) continue;
+        const uint32_t cnt = e[k] - s[k];
+        if (cnt > 1) {                           // rare: fp64 accumulation in sorted order, then mean
+          if constexpr (VEC == 4) {
+            double a0 = x[k].x, a1 = x[k].y, a2 = x[k].z, a3 = x[k].w;
+            for (uint32_t q = s[k] + 1; q < e[k]; ++q) {
+              const float4 y = reinterpret_cast<const float4*>(attr + (size_t)perm[q] * C)[c];
+              a0 += y.x; a1 += y.y; a2 += y.z; a3 += y.w;
+            }
+            const double inv = (double)cnt;
+            x[k] = make_float4((float)(a0 / inv), (float)(a1 / inv), (float)(a2 / inv), (float)(a3 / inv));
+          } else {
+            double a0 = x[k];
+            for (uint32_t q = s[k] + 1; q < e[k]; ++q) a0 += attr[(size_t)perm[q] * C + c];
+            x[k] = (float)(a0 / (double)cnt);
+          }
+        }
+        reinterpret_cast<VecT*>(merged + (size_t)v * C)[c] = x[k];
+      }
+    }
+    if (lane == 0) {
+#pragma unroll
+      for (int k = 0; k < ROWS; ++k) {
+        const uint32_t v = r0 + threadIdx.y + 16 * k;
+        if (v < nv) weights[v] = e[k] - s[k];
+      }
+    }
+  }
+}
+
+int run_voxel_merge(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, int channels, uint32_t n,
+                    const uint32_t* d_perm, const uint32_t* d_voxel_start, const gsnfs_counts* d_counts,
+                    float* d_merged, uint32_t* d_weights) {
+  if (n == 0) return GSNFS_OK;
+  constexpr int ROWS = 4;
+  const dim3 block(16, 16);
+  const uint32_t blocks_needed = (n + 16 * ROWS - 1) / (16 * ROWS);
+  const uint32_t gcap = (uint32_t)ctx->num_sms * 32u;
+  const int grid = (int)(blocks_needed < gcap ? blocks_needed : gcap);
+  if (channels % 4 == 0)
+    merge_kernel<4, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, d_merged, d_weights);
+  else
+    merge_kernel<1, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, d_merged, d_weights);
+  GSNFS_LAUNCH_CHECK(ctx);
+  return GSNFS_OK;
+}
+
+}  // namespace gsnfs

@@ -1,0 +1,463 @@
+// Encoder-side position coder: voxelise + Morton (K1/K2), onesweep LSD radix sort (K3), and a fused
+// unique + all-levels octree build that emits the breadth-first occupancy stream (K4, K6, K7, K8).
+//
+// What differs from the paper's design (section 2.2, Alg. A.1): the paper builds L_d level by
+// level with J `unique` launches and then runs J OccKernel launches with a binary search per parent.
+// Here one pass over the sorted codes does all levels at once.  With h_i = msb(code[i-1] ^ code[i]), sorted
+// entry i starts a new node at every depth d >= J - floor(h_i / 3) (and at no depth if it is a duplicate),
+// so |L_d|, the index of every node inside its level and each parent's occupancy bits all follow from
+// per-level prefix counts of those flags.  The bytes produced are exactly Alg. A.1's.
+#include "common.cuh"
+
+namespace gsnfs {
+
+// ------------------------------------------------------------------------------------------------
+// K1 + K2: voxelise, Morton-encode, and accumulate the digit histograms of every radix pass.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint64_t spread3(uint32_t v) {   // 21 bits -> every third bit
+  uint64_t x = v & 0x1fffffu;
+  x = (x | (x << 32)) & 0x001f00000000ffffull;
+  x = (x | (x << 16)) & 0x001f0000ff0000ffull;
+  x = (x | (x << 8)) & 0x100f00f00f00f00full;
+  x = (x | (x << 4)) & 0x10c30c30c30c30c3ull;
+  x = (x | (x << 2)) & 0x1249249249249249ull;
+  return x;
+}
+
+struct VoxParams {
+  double lo[3];
+  double scale[3];
+  double vmax;
+};
+
+__device__ __forceinline__ uint32_t voxel_coord(float p, double lo, double scale, double vmax) {
+  // [O2]: one rounding for the subtraction, one for the product, no contraction into an FMA.
+  const double t = __dsub_rn((double)p, lo);
+  const double u = __dmul_rn(t, scale);
+  double v = floor(u);
+  v = (u < 0.0) ? 0.0 : fmin(v, vmax);      // NaN -> fmin returns vmax: in range, unspecified
+  return (uint32_t)v;
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(256) voxelize_kernel(const float* __restrict__ xyz, uint32_t n, VoxParams vp,
+                                                       SortPlan plan, KeyT* __restrict__ keys,
+                                                       uint32_t* __restrict__ ghist) {
+  __shared__ uint32_t s_hist[kSortMaxPasses][256];
+  for (int i = threadIdx.x; i < kSortMaxPasses * 256; i += 256) (&s_hist[0][0])[i] = 0;
+  __syncthreads();
+  for (uint32_t i = blockIdx.x * 256 + threadIdx.x; i < n; i += gridDim.x * 256) {
+    const float px = xyz[3 * (size_t)i], py = xyz[3 * (size_t)i + 1], pz = xyz[3 * (size_t)i + 2];
+    const uint32_t vx = voxel_coord(px, vp.lo[0], vp.scale[0], vp.vmax);
+    const uint32_t vy = voxel_coord(py, vp.lo[1], vp.scale[1], vp.vmax);
+    const uint32_t vz = voxel_coord(pz, vp.lo[2], vp.scale[2], vp.vmax);
+    const uint64_t key = spread3(vx) | (spread3(vy) << 1) | (spread3(vz) << 2);
+    keys[i] = (KeyT)key;
+    for (int p = 0; p < plan.passes; ++p) {
+      const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
+      atomicAdd(&s_hist[p][d], 1u);
+    }
+  }
+  __syncthreads();
+  for (int i = threadIdx.x; i < plan.passes * 256; i += 256) {
+    const uint32_t c = (&s_hist[0][0])[i];
+    if (c) atomicAdd(&ghist[i], c);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// K3: one onesweep pass (stable LSD radix sort, 8-bit digits): warp-level match_any ranking into
+// shared-memory warp histograms, per-digit decoupled look-back across tiles for the global offsets,
+// shared-memory staged scatter so that global writes are coalesced per digit run.
+// ------------------------------------------------------------------------------------------------
+constexpr uint32_t kFlagAgg = 1u << 30, kFlagInc = 2u << 30, kValMask = (1u << 30) - 1u;
+
+template <typename KeyT>
+__global__ void __launch_bounds__(kSortThreads) onesweep_kernel(
+    const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ pay_in, KeyT* __restrict__ keys_out,
+    uint32_t* __restrict__ pay_out, uint32_t n, int shift, int bits, const uint32_t* __restrict__ ghist,
+    uint32_t* status, uint32_t* ticket) {
+  constexpr int WARPS = kSortThreads / 32;
+  extern __shared__ __align__(16) unsigned char s_dyn[];
+  KeyT* s_keys = reinterpret_cast<KeyT*>(s_dyn);
+  uint32_t* s_pay = reinterpret_cast<uint32_t*>(s_dyn + sizeof(KeyT) * kSortTile);
+  __shared__ uint32_t s_whist[WARPS][257];
+  __shared__ uint32_t s_dstart[256];
+  __shared__ uint32_t s_goff[256];
+  __shared__ uint32_t s_scan[9];
+  __shared__ uint32_t s_tile;
+
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid == 0) s_tile = atomicAdd(ticket, 1u);
+  for (int i = tid; i < WARPS * 257; i += kSortThreads) (&s_whist[0][0])[i] = 0;
+  __syncthreads();
+  const uint32_t tile = s_tile;
+  const uint32_t base = tile * (uint32_t)kSortTile;
+  const uint32_t mask = (1u << bits) - 1u;
+
+  KeyT key[kSortItems];
+  uint32_t pay[kSortItems];
+  uint32_t rank[kSortItems];
+  const uint32_t wbase = base + warp * (kSortItems * 32) + lane;
+#pragma unroll
+  for (int j = 0; j < kSortItems; ++j) {
+    const uint32_t idx = wbase + j * 32;
+    const bool valid = idx < n;
+    key[j] = valid ? keys_in[idx] : (KeyT)~(KeyT)0;
+    pay[j] = valid ? (pay_in ? pay_in[idx] : idx) : 0xffffffffu;
+  }
+  // global digit base for this pass (exclusive scan of the pass histogram)
+  uint32_t gbase = block_excl_scan_256(ghist[tid], s_scan, nullptr);
+
+#pragma unroll
+  for (int j = 0; j < kSortItems; ++j) {
+    const bool valid = (wbase + j * 32) < n;
+    const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
+    const unsigned peers = __match_any_sync(0xffffffffu, d);
+    const unsigned lt = peers & lanemask_lt();
+    const uint32_t prev = s_whist[warp][d];
+    __syncwarp();
+    if (lt == 0) s_whist[warp][d] = prev + __popc(peers);
+    __syncwarp();
+    rank[j] = prev + __popc(lt);
+  }
+  __syncthreads();
+
+  // thread d: exclusive prefix over warps of digit d, tile count of digit d
+  uint32_t count = 0;
+#pragma unroll
+  for (int w = 0; w < WARPS; ++w) {
+    const uint32_t c = s_whist[w][tid];
+    s_whist[w][tid] = count;
+    count += c;
+  }
+  // publish the aggregate early, then resolve the exclusive prefix by look-back
+  uint32_t* my_status = status + (size_t)tile * 256 + tid;
+  if (tile == 0) {
+    st_volatile_u32(my_status, kFlagInc | count);
+  } else {
+    st_volatile_u32(my_status, kFlagAgg | count);
+  }
+  const uint32_t dstart = block_excl_scan_256(count, s_scan, nullptr);
+  uint32_t excl = 0;
+  if (tile > 0) {
+    int t = (int)tile - 1;
+    while (true) {
+      const uint32_t* ps = status + (size_t)t * 256 + tid;
+      uint32_t s;
+      do { s = ld_volatile_u32(ps); } while ((s & ~kValMask) == 0u);
+      excl += s & kValMask;
+      if (s & kFlagInc) break;
+      --t;
+    }
+    st_volatile_u32(my_status, kFlagInc | (excl + count));
+  }
+  s_dstart[tid] = dstart;
+  s_goff[tid] = gbase + excl - dstart;      // global position = s_goff[d] + tile-local sorted position
+  __syncthreads();
+
+#pragma unroll
+  for (int j = 0; j < kSortItems; ++j) {
+    const bool valid = (wbase + j * 32) < n;
+    if (valid) {
+      const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
+      const uint32_t pos = s_dstart[d] + s_whist[warp][d] + rank[j];
+      s_keys[pos] = key[j];
+      s_pay[pos] = pay[j];
+    }
+  }
+  __syncthreads();
+  const uint32_t cnt = min((uint32_t)kSortTile, n - base);
+  for (uint32_t i = tid; i < cnt; i += kSortThreads) {
+    const KeyT k = s_keys[i];
+    const uint32_t d = (uint32_t)(k >> shift) & mask;
+    const uint32_t o = s_goff[d] + i;
+    keys_out[o] = k;
+    pay_out[o] = s_pay[i];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// K4 + K6 + K7 + K8: unique + all-levels octree build over the sorted codes.
+//   t(i) = number of depths at which sorted entry i starts a node:
+//          i = 0: J + 1 (depths 0..J); duplicate of i-1: 0; else floor(h_i / 3) + 1 (depths J - floor(h_i/3) .. J).
+//   flag_d(i) = t(i) >= J - d + 1.
+// ------------------------------------------------------------------------------------------------
+template <typename KeyT>
+__device__ __forceinline__ int start_levels(const KeyT* __restrict__ keys, uint32_t i, uint32_t n, int J,
+                                            uint64_t* key_out) {
+  if (i >= n) { *key_out = 0; return 0; }
+  const uint64_t k = (uint64_t)keys[i];
+  *key_out = k;
+  if (i == 0) return J + 1;
+  const uint64_t x = k ^ (uint64_t)keys[i - 1];
+  if (x == 0) return 0;
+  return msb64(x) / 3 + 1;
+}
+
+// per-tile counts c_d(tile) for d = 0..J, level-major layout hist[d * ntiles + tile]
+template <typename KeyT>
+__global__ void __launch_bounds__(256) octree_count_kernel(const KeyT* __restrict__ keys, uint32_t n, int J,
+                                                           uint32_t ntiles, uint32_t* __restrict__ hist) {
+  __shared__ uint32_t s_cnt[kOctLevels];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (tid < kOctLevels) s_cnt[tid] = 0;
+  __syncthreads();
+  const uint32_t base = blockIdx.x * (uint32_t)kOctTile + warp * 256;
+  uint32_t mine = 0;   // lane d accumulates level d
+  for (int it = 0; it < 8; ++it) {
+    uint64_t k;
+    const int t = start_levels(keys, base + it * 32 + lane, n, J, &k);
+    for (int d = 0; d <= J; ++d) {
+      const unsigned b = __ballot_sync(0xffffffffu, t >= J - d + 1);
+      if (lane == d) mine += __popc(b);
+    }
+  }
+  if (lane <= J) atomicAdd(&s_cnt[lane], mine);
+  __syncthreads();
+  if (tid <= J) hist[(size_t)tid * ntiles + blockIdx.x] = s_cnt[tid];
+}
+
+// one CTA: per level exclusive scan over tiles; level sizes, stream offsets, counts.
+__global__ void __launch_bounds__(1024) octree_scan_kernel(const uint32_t* __restrict__ hist,
+                                                           uint32_t* __restrict__ tbase, uint32_t ntiles, int J,
+                                                           uint32_t n, uint32_t* __restrict__ meta,
+                                                           uint32_t* __restrict__ d_level_sizes,
+                                                           uint32_t* __restrict__ d_voxel_start,
+                                                           gsnfs_counts* __restrict__ d_counts) {
+  __shared__ uint32_t s_size[kOctLevels];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int d = warp; d <= J; d += 32) {        // warp per level
+    uint32_t carry = 0;
+    for (uint32_t b = 0; b < ntiles; b += 32) {
+      const uint32_t t = b + lane;
+      const uint32_t v = t < ntiles ? hist[(size_t)d * ntiles + t] : 0u;
+      uint32_t inc = v;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        uint32_t x = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += x;
+      }
+      if (t < ntiles) tbase[(size_t)d * ntiles + t] = carry + inc - v;
+      carry += __shfl_sync(0xffffffffu, inc, 31);
+    }
+    if (lane == 0) s_size[d] = carry;
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    uint32_t off = 0;
+    for (int d = 0; d <= J; ++d) {
+      meta[d] = s_size[d];
+      meta[kOctLevels + d] = off;       // stream offset of level d (valid for d < J; off[J] = S)
+      d_level_sizes[d] = s_size[d];
+      if (d < J) off += s_size[d];
+    }
+    d_counts->n_voxels = s_size[J];
+    d_counts->occ_bytes = n ? off : 0u;
+    d_counts->status = 0;
+    d_counts->reserved = 0;
+    d_voxel_start[s_size[J]] = n;
+  }
+}
+
+template <typename KeyT>
+__global__ void __launch_bounds__(256) octree_emit_kernel(const KeyT* __restrict__ keys, uint32_t n, int J,
+                                                          uint32_t ntiles, const uint32_t* __restrict__ hist,
+                                                          const uint32_t* __restrict__ tbase,
+                                                          const uint32_t* __restrict__ meta,
+                                                          uint8_t* __restrict__ occ,
+                                                          uint64_t* __restrict__ voxel_keys,
+                                                          uint32_t* __restrict__ voxel_start) {
+  extern __shared__ __align__(16) unsigned char s_dyn[];
+  uint32_t* s_stage = reinterpret_cast<uint32_t*>(s_dyn);        // staged occupancy bytes, as words
+  __shared__ uint32_t s_wcnt[8][kOctLevels];   // per-warp per-level counts -> exclusive over warps
+  __shared__ uint32_t s_cnt[kOctLevels];       // c_d(tile)
+  __shared__ uint32_t s_base[kOctLevels];      // nodes of level d started before this tile
+  __shared__ uint32_t s_soff[kOctLevels + 1];  // staging offset (bytes) of level e, e < J
+  __shared__ uint32_t s_loff[kOctLevels];      // stream offset of level e
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const uint32_t tile = blockIdx.x;
+
+  if (tid <= J) {
+    s_cnt[tid] = hist[(size_t)tid * ntiles + tile];
+    s_base[tid] = tbase[(size_t)tid * ntiles + tile];
+    s_loff[tid] = meta[kOctLevels + tid];
+  }
+  __syncthreads();
+  if (tid == 0) {
+    uint32_t o = 0;
+    for (int e = 0; e < J; ++e) { s_soff[e] = o; o += (s_cnt[e] + 1 + 3) & ~3u; }   // word-aligned per level
+    s_soff[J] = o;
+  }
+  __syncthreads();
+  const uint32_t stage_words = s_soff[J] >> 2;
+  for (uint32_t i = tid; i < stage_words; i += 256) s_stage[i] = 0;
+
+  // pass 1: t values into registers, per-warp per-level counts
+  const uint32_t base = tile * (uint32_t)kOctTile + warp * 256;
+  int tt[8];
+  uint64_t kk[8];
+  uint32_t mine = 0;
+#pragma unroll
+  for (int it = 0; it < 8; ++it) {
+    tt[it] = start_levels(keys, base + it * 32 + lane, n, J, &kk[it]);
+    for (int d = 0; d <= J; ++d) {
+      const unsigned b = __ballot_sync(0xffffffffu, tt[it] >= J - d + 1);
+      if (lane == d) mine += __popc(b);
+    }
+  }
+  if (lane <= J) s_wcnt[warp][lane] = mine;
+  __syncthreads();
+  if (tid <= J) {                      // exclusive prefix over warps for level tid
+    uint32_t run = 0;
+    for (int w = 0; w < 8; ++w) { const uint32_t c = s_wcnt[w][tid]; s_wcnt[w][tid] = run; run += c; }
+  }
+  __syncthreads();
+
+  // pass 2: ranks, voxel list, staged occupancy bits
+  uint32_t run = (lane <= J) ? s_wcnt[warp][lane] : 0u;   // lane d: level-d starts in this tile before this warp-iteration
+#pragma unroll
+  for (int it = 0; it < 8; ++it) {
+    const uint32_t i = base + it * 32 + lane;
+    const int t = tt[it];
+    const uint64_t k = kk[it];
+    uint32_t prev_incl = 0;            // tile-local inclusive rank at depth d-1
+    for (int d = 0; d <= J; ++d) {
+      const bool f = t >= J - d + 1;
+      const unsigned b = __ballot_sync(0xffffffffu, f);
+      const uint32_t run_d = __shfl_sync(0xffffffffu, run, d);
+      const uint32_t incl = run_d + __popc(b & lanemask_le());
+      if (f && d >= 1) {
+        // this entry starts a node at depth d; its parent is the prev_incl-th slot of depth d-1
+        const uint32_t digit = (uint32_t)(k >> (3 * (J - d))) & 7u;
+        const uint32_t sb = s_soff[d - 1] + prev_incl;
+        atomicOr(&s_stage[sb >> 2], (1u << digit) << (8 * (sb & 3u)));
+      }
+      if (f && d == J) {
+        const uint32_t v = s_base[J] + incl - 1;
+        voxel_keys[v] = k;
+        voxel_start[v] = i;
+      }
+      if (lane == d) run += __popc(b);
+      prev_incl = incl;
+    }
+  }
+  __syncthreads();
+
+  // flush: slot s of level e is stream byte loff[e] + base[e] - 1 + s, s = 0..c_e.  Slots 0 and c_e may be
+  // shared with neighbouring tiles; any global word holding such a byte (or a byte outside this tile's
+  // range of this level) is merged with atomicOr, fully interior words are stored whole.
+  uint32_t* occ_w = reinterpret_cast<uint32_t*>(occ);
+  for (int e = 0; e < J; ++e) {
+    const uint32_t c = s_cnt[e];
+    const int64_t g0 = (int64_t)s_loff[e] + (int64_t)s_base[e] - 1;    // stream byte of slot 0 (may be -1 at tile 0)
+    const int64_t g1 = g0 + c;
+    const int64_t w0 = (g0 < 0 ? 0 : g0) >> 2, w1 = g1 >> 2;
+    const uint8_t* sbytes = reinterpret_cast<const uint8_t*>(s_stage) + s_soff[e];
+    for (int64_t w = w0 + tid; w <= w1; w += 256) {
+      uint32_t val = 0;
+      bool interior = true;
+#pragma unroll
+      for (int bb = 0; bb < 4; ++bb) {
+        const int64_t s = (w << 2) + bb - g0;
+        if (s >= 0 && s <= (int64_t)c) val |= (uint32_t)sbytes[s] << (8 * bb);
+        if (s < 1 || s > (int64_t)c - 1) interior = false;
+      }
+      if (interior) occ_w[w] = val;
+      else if (val) atomicOr(&occ_w[w], val);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+static SortPlan make_sort_plan(int depth) {
+  SortPlan p{};
+  const int total = 3 * depth;
+  p.passes = (total + 7) / 8;
+  int shift = 0;
+  for (int i = 0; i < p.passes; ++i) {           // spread the bits evenly over the passes
+    const int b = (total - shift + (p.passes - i) - 1) / (p.passes - i);
+    p.shift[i] = shift;
+    p.bits[i] = b;
+    shift += b;
+  }
+  return p;
+}
+
+template <typename KeyT>
+static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint32_t n, const VoxParams& vp,
+                       int depth, uint8_t* d_occ, uint64_t occ_capacity, uint32_t* d_level_sizes, uint32_t* d_perm,
+                       uint64_t* d_voxel_keys, uint32_t* d_voxel_start, gsnfs_counts* d_counts) {
+  const SortPlan plan = make_sort_plan(depth);
+  const uint32_t stiles = (n + kSortTile - 1) / kSortTile;
+  KeyT* ka = reinterpret_cast<KeyT*>(ctx->keys_a);
+  KeyT* kb = reinterpret_cast<KeyT*>(ctx->keys_b);
+
+  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->hist, 0, ctx->sort_zero_bytes, st));
+  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(d_occ, 0, occ_capacity, st));
+  if (n) {
+    const uint32_t vwant = (n + 1023u) / 1024u, vcap = (uint32_t)ctx->num_sms * 8u;
+    const int vgrid = (int)(vwant < vcap ? vwant : vcap);
+    voxelize_kernel<KeyT><<<vgrid, 256, 0, st>>>(d_xyz, n, vp, plan, ka, ctx->hist);
+    GSNFS_LAUNCH_CHECK(ctx);
+    const size_t smem = (sizeof(KeyT) + 4) * (size_t)kSortTile;
+    const uint32_t status_stride = (uint32_t)((ctx->max_points + kSortTile - 1) / kSortTile) * 256;
+    const KeyT* kin = ka;
+    KeyT* kout = kb;
+    const uint32_t* pin = nullptr;
+    for (int p = 0; p < plan.passes; ++p) {
+      uint32_t* pout = (p == plan.passes - 1) ? d_perm : ((p & 1) ? ctx->pay_b : ctx->pay_a);
+      onesweep_kernel<KeyT><<<stiles, kSortThreads, smem, st>>>(
+          kin, pin, kout, pout, n, plan.shift[p], plan.bits[p], ctx->hist + p * 256,
+          ctx->sort_status + (size_t)p * status_stride, ctx->sort_ticket + p);
+      GSNFS_LAUNCH_CHECK(ctx);
+      pin = pout;
+      const KeyT* t = kin;
+      kin = kout;
+      kout = const_cast<KeyT*>(t);
+    }
+    const KeyT* sorted = kin;
+    const uint32_t otiles = (n + kOctTile - 1) / kOctTile;
+    octree_count_kernel<KeyT><<<otiles, 256, 0, st>>>(sorted, n, depth, otiles, ctx->oct_hist);
+    GSNFS_LAUNCH_CHECK(ctx);
+    octree_scan_kernel<<<1, 1024, 0, st>>>(ctx->oct_hist, ctx->oct_base, otiles, depth, n, ctx->oct_meta,
+                                           d_level_sizes, d_voxel_start, d_counts);
+    GSNFS_LAUNCH_CHECK(ctx);
+    const size_t esmem = (size_t)depth * (kOctTile + 4);
+    octree_emit_kernel<KeyT><<<otiles, 256, esmem, st>>>(sorted, n, depth, otiles, ctx->oct_hist, ctx->oct_base,
+                                                         ctx->oct_meta, d_occ, d_voxel_keys, d_voxel_start);
+    GSNFS_LAUNCH_CHECK(ctx);
+  } else {
+    GSNFS_CUDA_OK(ctx, cudaMemsetAsync(d_level_sizes, 0, sizeof(uint32_t) * (depth + 1), st));
+    GSNFS_CUDA_OK(ctx, cudaMemsetAsync(d_counts, 0, sizeof(gsnfs_counts), st));
+    GSNFS_CUDA_OK(ctx, cudaMemsetAsync(d_voxel_start, 0, sizeof(uint32_t), st));
+  }
+  return GSNFS_OK;
+}
+
+int octree_encode_setup(gsnfs_ctx* ctx) {
+  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(onesweep_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)((8 + 4) * kSortTile)));
+  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(onesweep_kernel<uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)((4 + 4) * kSortTile)));
+  const int esmem = GSNFS_MAX_DEPTH * (kOctTile + 4);
+  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(octree_emit_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, esmem));
+  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(octree_emit_kernel<uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, esmem));
+  return GSNFS_OK;
+}
+
+int run_octree_encode(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint32_t n, const double lo[3],
+                      const double scale[3], int depth, uint8_t* d_occ, uint64_t occ_capacity,
+                      uint32_t* d_level_sizes, uint32_t* d_perm, uint64_t* d_voxel_keys, uint32_t* d_voxel_start,
+                      gsnfs_counts* d_counts) {
+  VoxParams vp;
+  for (int a = 0; a < 3; ++a) { vp.lo[a] = lo[a]; vp.scale[a] = scale[a]; }
+  vp.vmax = (double)((1u << depth) - 1u);
+  if (3 * depth <= 32)
+    return encode_impl<uint32_t>(ctx, st, d_xyz, n, vp, depth, d_occ, occ_capacity, d_level_sizes, d_perm,
+                                 d_voxel_keys, d_voxel_start, d_counts);
+  return encode_impl<uint64_t>(ctx, st, d_xyz, n, vp, depth, d_occ, occ_capacity, d_level_sizes, d_perm,
+                               d_voxel_keys, d_voxel_start, d_counts);
+}
+
+}  // namespace gsnfs

@@ -1,0 +1,348 @@
+"""GPU parity: the CUDA path (through the C ABI) against the fp64 oracle, element by element, on the
+same seeded inputs.  Tolerances are BASELINE.json north_star's:
+  occupancy bytes, level sizes, perm, voxel keys, decoded voxels: bit-exact;
+  unquantised RAHT coefficients: per-channel relative L2 <= 1e-5;
+  quantised coefficients: >= 99.99 % identical, the rest off by exactly 1;
+  decoded attributes: max abs error <= 1e-4 x channel range (same quantised input on both sides).
+"""
+import numpy as np
+import pytest
+import torch
+
+from oracle import gsnfs_oracle as orc
+from paper_2606_05650_b200 import synth
+
+pytestmark = pytest.mark.gpu
+
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_05650_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx_small(B):
+    c = B.Context(max_points=120_000, max_channels=64, max_depth=21)
+    yield c
+    c.close()
+
+
+@pytest.fixture(scope="module")
+def ctx_big(B):
+    c = B.Context(max_points=3_000_000, max_channels=56, max_depth=21)
+    yield c
+    c.close()
+
+
+def _t(a, dtype=None):
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.to(DEV)
+
+
+def gpu_position_encode(B, ctx, fr):
+    buf = B.FrameBuffers(fr.n, fr.channels, fr.depth, DEV)
+    d_xyz = _t(fr.xyz) if fr.n else torch.empty((1, 3), dtype=torch.float32, device=DEV)
+    B.gsnfs_octree_encode(ctx, d_xyz, fr.n, fr.bbox_min, fr.bbox_max, fr.depth, buf.occ, buf.level_sizes, buf.perm,
+                          buf.voxel_keys, buf.voxel_start, buf.counts)
+    torch.cuda.synchronize()
+    cnt = buf.counts.cpu().numpy().astype(np.int64)
+    nv, ob = int(cnt[0]), int(cnt[1])
+    return buf, {
+        "n_voxels": nv, "occ_bytes": ob, "status": int(cnt[2]),
+        "occ": buf.occ[:ob].cpu().numpy(),
+        "level_sizes": buf.level_sizes.cpu().numpy().astype(np.int64),
+        "perm": buf.perm[:fr.n].cpu().numpy().astype(np.int64),
+        "voxel_keys": buf.voxel_keys[:nv].cpu().numpy().astype(np.uint64),
+        "voxel_start": buf.voxel_start[:nv + 1].cpu().numpy().astype(np.int64),
+    }
+
+
+def check_position(got, ref, n):
+    assert got["n_voxels"] == len(ref["voxel_keys"])
+    assert got["level_sizes"].tolist() == ref["level_sizes"].tolist()
+    assert got["occ_bytes"] == len(ref["occ"])
+    assert np.array_equal(got["occ"], ref["occ"])
+    assert np.array_equal(got["perm"], ref["perm"][:n])
+    assert np.array_equal(got["voxel_keys"], ref["voxel_keys"])
+    assert np.array_equal(got["voxel_start"], ref["voxel_start"])
+
+
+def rel_l2(got, ref):
+    num = np.sqrt(((got.astype(np.float64) - ref) ** 2).sum(axis=0))
+    den = np.sqrt((ref ** 2).sum(axis=0))
+    den = np.where(den > 0, den, 1.0)
+    return num / den
+
+
+def check_quantised(q_gpu, q_ref):
+    diff = q_gpu.astype(np.int64) - q_ref
+    nz = diff != 0
+    frac = nz.mean() if diff.size else 0.0
+    assert frac <= 1e-4, f"{frac:.3e} of quantised coefficients differ"
+    assert np.all(np.abs(diff[nz]) == 1)
+    return frac
+
+
+def full_pipeline_check(B, ctx, fr, dz=None, check_decode=True):
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep,
+                           dz_round=orc.DZ_ROUND_DEFAULT if dz is None else float(np.float32(dz)))
+    buf, got = gpu_position_encode(B, ctx, fr)
+    check_position(got, ref, fr.n)
+    nv = got["n_voxels"]
+    d_attr = _t(fr.attr)
+    B.gsnfs_voxel_merge(ctx, d_attr, fr.channels, fr.n, buf.perm, buf.voxel_start, buf.counts, buf.merged, buf.weights)
+    torch.cuda.synchronize()
+    merged = buf.merged[:nv].cpu().numpy()
+    assert np.array_equal(buf.weights[:nv].cpu().numpy().astype(np.int64), ref["weights"])
+    ch_range = (fr.qstep.astype(np.float64) * fr.qdiv)[None, :]
+    assert np.all(np.abs(merged - ref["merged"]) <= 1e-6 * ch_range + 1e-7 * np.abs(ref["merged"]))
+    single = ref["weights"] == 1
+    assert np.array_equal(merged[single], ref["merged"][single].astype(np.float32))   # copies are bit exact
+    # forward: unquantised + quantised in one call, counts chained on the device
+    coeff = torch.empty((max(fr.n, 1), fr.channels), dtype=torch.float32, device=DEV)
+    quant = None if dz is None else (dz, 0.0)
+    B.gsnfs_raht_forward(ctx, buf.voxel_keys, buf.weights, fr.n, buf.counts, fr.depth, buf.merged, fr.channels,
+                         fr.qstep, quant, buf.qcoeff, coeff)
+    torch.cuda.synchronize()
+    Y = coeff[:nv].cpu().numpy()
+    q = buf.qcoeff[:nv].cpu().numpy()
+    err = rel_l2(Y, ref["coeff"])
+    assert err.max() <= 1e-5, f"coefficient rel L2 {err.max():.3e}"
+    frac = check_quantised(q, ref["qcoeff"])
+    if not check_decode:
+        return frac
+    # decode: position stream from the GPU encoder (bit-exact to the oracle's), coefficients = the ORACLE's
+    dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], fr.depth)
+    assert ok
+    buf.qcoeff[:nv].copy_(_t(ref["qcoeff"].astype(np.int32)))
+    B.decode_frame(ctx, buf, ref["level_sizes"], len(ref["occ"]), fr.qstep, quant)
+    torch.cuda.synchronize()
+    assert int(buf.dec_counts.cpu()[2]) == 0
+    assert np.array_equal(buf.dec_keys[:nv].cpu().numpy().astype(np.uint64), dk)
+    assert np.array_equal(buf.dec_xyz[:nv].cpu().numpy().astype(np.uint64), dc)
+    ref_attr = orc.raht_inverse(orc.dequantize(ref["qcoeff"], fr.qstep), dk, ref["weights"], fr.depth)
+    got_attr = buf.dec_attr[:nv].cpu().numpy().astype(np.float64)
+    assert np.all(np.abs(got_attr - ref_attr) <= 1e-4 * ch_range)
+    return frac
+
+
+# ----------------------------------------------------------------------------------------------
+def test_library_loaded_is_in_tree(B):
+    assert B.lib_path().endswith("paper_2606_05650_b200/libgsnfs.so")
+    assert "sm_100a" in B.gsnfs_version()
+
+
+def test_config1_full_pipeline(B, ctx_small):
+    full_pipeline_check(B, ctx_small, synth.make_frame(1))
+
+
+def test_config2_full_pipeline(B, ctx_small):
+    full_pipeline_check(B, ctx_small, synth.make_frame(2))
+
+
+@pytest.mark.parametrize("n,depth,channels", [(20_000, 5, 56), (5_000, 3, 56), (30_000, 6, 12), (3_000, 4, 7), (999, 2, 3)])
+def test_dense_duplicates(B, ctx_small, n, depth, channels):
+    # heavy duplicate merging, weights up to hundreds, vector (C%4==0) and scalar channel paths
+    full_pipeline_check(B, ctx_small, synth.make_dense_frame(n=n, depth=depth, channels=channels, seed=n))
+
+
+@pytest.mark.parametrize("dz", [0.0, 0.5])
+def test_quantiser_rounding_offsets(B, ctx_small, dz):
+    full_pipeline_check(B, ctx_small, synth.make_frame(1, n_override=4000), dz=dz)
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 3, 255, 256, 257, 4095, 4096, 4097])
+def test_tiny_and_tile_edges(B, ctx_small, n):
+    fr = synth.make_uniform_frame(n, depth=9, channels=8, seed=100 + n)
+    if n == 0:
+        buf, got = gpu_position_encode(B, ctx_small, fr)
+        assert got["n_voxels"] == 0 and got["occ_bytes"] == 0 and got["level_sizes"].tolist() == [0] * 10
+        return
+    full_pipeline_check(B, ctx_small, fr)
+
+
+def test_all_points_in_one_voxel(B, ctx_small):
+    fr = synth.make_uniform_frame(500, depth=6, channels=8, seed=5)
+    fr.xyz[:] = np.array([0.3, 0.6, 0.9], dtype=np.float32)
+    full_pipeline_check(B, ctx_small, fr)
+
+
+@pytest.mark.parametrize("J", [1, 2, 3, 4])
+def test_full_cube(B, ctx_small, J):
+    side = 1 << J
+    g = (np.arange(side) + 0.5) / side
+    xyz = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3).astype(np.float32)
+    rng = np.random.default_rng(J)
+    xyz = xyz[rng.permutation(xyz.shape[0])]
+    attr = rng.normal(0, 1, (xyz.shape[0], 4)).astype(np.float32)
+    fr = synth.Frame("cube", xyz, attr, synth.qstep_from_range(attr, 256), J, 256, np.zeros(3, np.float32), np.ones(3, np.float32))
+    full_pipeline_check(B, ctx_small, fr)
+    buf, got = gpu_position_encode(B, ctx_small, fr)
+    assert np.all(got["occ"] == 0xFF) and got["occ_bytes"] == (8 ** J - 1) // 7
+
+
+def test_deep_octree_and_cuboid_bbox(B, ctx_small):
+    # depth 21 (63-bit codes), non-cubic bounding box, points on and outside the box faces
+    rng = np.random.default_rng(21)
+    n = 20_000
+    lo = np.array([-1.0, 0.5, 10.0], np.float32)
+    hi = np.array([3.0, 0.75, 12.0], np.float32)
+    xyz = (lo + rng.uniform(0, 1, (n, 3)) * (hi - lo)).astype(np.float32)
+    xyz[:50] = lo
+    xyz[50:100] = hi
+    xyz[100:150] = hi + 1.0
+    xyz[150:200] = lo - 1.0
+    attr = rng.normal(0, 1, (n, 16)).astype(np.float32)
+    for depth in (21, 11, 10):
+        fr = synth.Frame("deep", xyz, attr, synth.qstep_from_range(attr, 256), depth, 256, lo, hi)
+        full_pipeline_check(B, ctx_small, fr)
+
+
+def test_presorted_and_reversed_input(B, ctx_small):
+    fr = synth.make_frame(1)
+    pos = orc.position_encode(fr.xyz, fr.bbox_min, fr.bbox_max, fr.depth)
+    for order in (pos["perm"], pos["perm"][::-1].copy()):
+        fr2 = synth.Frame("sorted", np.ascontiguousarray(fr.xyz[order]), np.ascontiguousarray(fr.attr[order]),
+                          fr.qstep, fr.depth, fr.qdiv, fr.bbox_min, fr.bbox_max)
+        full_pipeline_check(B, ctx_small, fr2, check_decode=False)
+
+
+def test_unit_weights_paper_mode(B, ctx_small):
+    # d_weights == NULL: the paper's unit leaf weights
+    fr = synth.make_frame(1, n_override=6000)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep, unit_weights=True)
+    buf, got = gpu_position_encode(B, ctx_small, fr)
+    nv = got["n_voxels"]
+    merged = _t(ref["merged"].astype(np.float32))
+    coeff = torch.empty((nv, fr.channels), dtype=torch.float32, device=DEV)
+    B.gsnfs_raht_forward(ctx_small, buf.voxel_keys, None, nv, None, fr.depth, merged, fr.channels, None, None, None, coeff)
+    back = torch.empty_like(coeff)
+    B.gsnfs_raht_inverse(ctx_small, buf.voxel_keys, None, nv, None, fr.depth, None, coeff, fr.channels, None, None, back)
+    torch.cuda.synchronize()
+    ref_Y = orc.raht_forward(ref["merged"].astype(np.float32), ref["voxel_keys"], np.ones(nv, np.int64), fr.depth)
+    assert rel_l2(coeff.cpu().numpy(), ref_Y).max() <= 1e-5
+    rng_c = (fr.qstep.astype(np.float64) * fr.qdiv)[None, :]
+    assert np.all(np.abs(back.cpu().numpy() - ref["merged"]) <= 1e-4 * rng_c)     # perfect reconstruction
+
+
+def test_corrupt_stream_is_flagged(B, ctx_small):
+    fr = synth.make_frame(1, n_override=3000)
+    ref = orc.position_encode(fr.xyz, fr.bbox_min, fr.bbox_max, fr.depth)
+    buf = B.FrameBuffers(fr.n, fr.channels, fr.depth, DEV)
+    occ = ref["occ"].copy()
+    occ[len(occ) // 2] = 0
+    buf.occ[:len(occ)].copy_(_t(occ))
+    B.gsnfs_octree_decode(ctx_small, buf.occ, len(occ), ref["level_sizes"], fr.depth, buf.dec_xyz, buf.dec_keys, buf.dec_counts)
+    torch.cuda.synchronize()
+    assert int(buf.dec_counts.cpu()[2]) & 1
+    sizes = ref["level_sizes"].copy()
+    sizes[fr.depth] -= 1
+    buf.occ[:len(occ)].copy_(_t(ref["occ"]))
+    B.gsnfs_octree_decode(ctx_small, buf.occ, len(ref["occ"]), sizes, fr.depth, buf.dec_xyz, buf.dec_keys, buf.dec_counts)
+    torch.cuda.synchronize()
+    assert int(buf.dec_counts.cpu()[2]) & 1
+
+
+def test_argument_errors(B, ctx_small):
+    fr = synth.make_frame(1, n_override=100)
+    buf = B.FrameBuffers(fr.n, fr.channels, fr.depth, DEV)
+    d_xyz = _t(fr.xyz)
+    with pytest.raises(B.GsnfsError) as e:
+        B.gsnfs_octree_encode(ctx_small, d_xyz, fr.n, fr.bbox_min, fr.bbox_max, 22, buf.occ, buf.level_sizes, buf.perm,
+                              buf.voxel_keys, buf.voxel_start, buf.counts)
+    assert e.value.status == B.GSNFS_E_INVALID_ARGUMENT
+    with pytest.raises(B.GsnfsError) as e:
+        B.gsnfs_octree_encode(ctx_small, d_xyz, fr.n, fr.bbox_max, fr.bbox_min, fr.depth, buf.occ, buf.level_sizes,
+                              buf.perm, buf.voxel_keys, buf.voxel_start, buf.counts)
+    assert e.value.status == B.GSNFS_E_INVALID_ARGUMENT
+    with pytest.raises(B.GsnfsError) as e:
+        B.gsnfs_octree_encode(ctx_small, d_xyz, 10**6, fr.bbox_min, fr.bbox_max, fr.depth, buf.occ, buf.level_sizes,
+                              buf.perm, buf.voxel_keys, buf.voxel_start, buf.counts)
+    assert e.value.status == B.GSNFS_E_CAPACITY
+
+
+# ----------------------------------------------------------------------------------------------
+# BASELINE.json's full sizes, in the launch configuration bench.py times
+# ----------------------------------------------------------------------------------------------
+def test_config3_headline_full_compare(B, ctx_big):
+    frac = full_pipeline_check(B, ctx_big, synth.make_frame(3))
+    print(f"config3: fraction of quantised coefficients off by one = {frac:.3e}")
+
+
+def test_config4_large_position_exact_and_raht_properties(B, ctx_big):
+    fr = synth.make_frame(4)
+    ref = orc.position_encode(fr.xyz, fr.bbox_min, fr.bbox_max, fr.depth)
+    buf, got = gpu_position_encode(B, ctx_big, fr)
+    check_position(got, ref, fr.n)
+    nv = got["n_voxels"]
+    d_attr = _t(fr.attr)
+    B.gsnfs_voxel_merge(ctx_big, d_attr, fr.channels, fr.n, buf.perm, buf.voxel_start, buf.counts, buf.merged, buf.weights)
+    coeff = torch.empty((fr.n, fr.channels), dtype=torch.float32, device=DEV)
+    B.gsnfs_raht_forward(ctx_big, buf.voxel_keys, buf.weights, fr.n, buf.counts, fr.depth, buf.merged, fr.channels,
+                         fr.qstep, None, buf.qcoeff, coeff)
+    torch.cuda.synchronize()
+    merged = buf.merged[:nv].double()
+    w = buf.weights[:nv].double()
+    Y = coeff[:nv].double()
+    # properties that hold at any size: DC = sum(w a)/sqrt(W); Parseval on sqrt(w)-scaled inputs
+    dc_ref = (w[:, None] * merged).sum(0) / torch.sqrt(w.sum())
+    scale = torch.sqrt((w[:, None] * merged ** 2).sum(0))
+    assert torch.all((Y[0] - dc_ref).abs() <= 2e-6 * scale)
+    assert torch.allclose((Y ** 2).sum(0), (w[:, None] * merged ** 2).sum(0), rtol=1e-5)
+    # sampled coefficients, one by one, from the closed form over Morton-prefix ranges (fp64, numpy)
+    M = ref["voxel_keys"]
+    mg = merged.cpu().numpy()
+    wn = ref["weights"].astype(np.float64)
+    P = np.concatenate([[0.0], np.cumsum(wn)])
+    Yn = Y.cpu().numpy()
+    rng = np.random.default_rng(0)
+    h_all = np.floor(np.log2((M[1:] ^ M[:-1]).astype(np.float64))).astype(np.int64)
+    cand = np.concatenate([rng.integers(1, nv, 300), 1 + np.argsort(h_all)[-40:]])      # random + the top of the tree
+    for i in cand.tolist():
+        h = int(M[i] ^ M[i - 1]).bit_length() - 1
+        lo = np.searchsorted(M, (M[i] >> np.uint64(h + 1)) << np.uint64(h + 1))
+        hi = np.searchsorted(M, ((M[i] >> np.uint64(h)) + np.uint64(1)) << np.uint64(h))
+        W0, W1 = P[i] - P[lo], P[hi] - P[i]
+        T0 = (wn[lo:i, None] * mg[lo:i]).sum(0)
+        T1 = (wn[i:hi, None] * mg[i:hi]).sum(0)
+        yref = np.sqrt(W0 / (W0 + W1)) * T1 / np.sqrt(W1) - np.sqrt(W1 / (W0 + W1)) * T0 / np.sqrt(W0)
+        tol = 2e-6 * (np.abs(T1) / np.sqrt(W1) + np.abs(T0) / np.sqrt(W0)) + 1e-6
+        assert np.all(np.abs(Yn[i] - yref) <= tol), i
+    # decode round trip on the GPU's own stream: voxels bit-exact, attributes within quantisation error
+    B.decode_frame(ctx_big, buf, got["level_sizes"], got["occ_bytes"], fr.qstep, None)
+    torch.cuda.synchronize()
+    assert int(buf.dec_counts.cpu()[2]) == 0
+    assert torch.equal(buf.dec_keys[:nv], buf.voxel_keys[:nv])
+    dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], fr.depth)
+    assert np.array_equal(buf.dec_xyz[:nv].cpu().numpy().astype(np.uint64), dc)
+
+
+def test_host_frame_calls_roundtrip(B, ctx_small):
+    fr = synth.make_frame(1)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    n, C = fr.n, fr.channels
+    cap = B.gsnfs_occ_capacity(n, fr.depth)
+    pin = lambda *s, dt: torch.empty(s, dtype=dt).pin_memory()
+    h_xyz, h_attr = torch.from_numpy(fr.xyz).pin_memory(), torch.from_numpy(fr.attr).pin_memory()
+    h_occ, h_lev = pin(cap, dt=torch.uint8), pin(fr.depth + 1, dt=torch.int32)
+    h_w, h_q, h_cnt = pin(n, dt=torch.int32), pin(n, C, dt=torch.int32), pin(4, dt=torch.int32)
+    B.gsnfs_frame_encode_host(ctx_small, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep, None,
+                              h_occ, h_lev, h_w, h_q, h_cnt)
+    nv, ob = int(h_cnt[0]), int(h_cnt[1])
+    assert nv == len(ref["voxel_keys"]) and np.array_equal(h_occ[:ob].numpy(), ref["occ"])
+    assert h_lev.numpy().tolist() == ref["level_sizes"].tolist()
+    check_quantised(h_q[:nv].numpy(), ref["qcoeff"])
+    h_vx, h_out, h_cnt2 = pin(n, 3, dt=torch.int32), pin(n, C, dt=torch.float32), pin(4, dt=torch.int32)
+    B.gsnfs_frame_decode_host(ctx_small, h_occ, ob, h_lev.numpy(), fr.depth, h_w, h_q, C, fr.qstep, None, h_vx, h_out, h_cnt2)
+    assert int(h_cnt2[2]) == 0
+    dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], fr.depth)
+    assert np.array_equal(h_vx[:nv].numpy().astype(np.uint64), dc)
+    # reconstruction error bounded by the quantiser: compare against the merged attributes loosely
+    rng_c = (fr.qstep.astype(np.float64) * fr.qdiv)[None, :]
+    assert np.max(np.abs(h_out[:nv].numpy() - ref["merged"]) / rng_c) < 0.05
