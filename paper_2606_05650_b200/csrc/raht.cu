@@ -80,7 +80,7 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
       const uint32_t vidx = valid ? (idx_p ? idx_p[ks + tid] : ks + tid) : 0xffffffffu;
       const uint64_t mk = valid ? keys[vidx] : ~0ull;
       s_key[tid] = mk;
-      s_vidx[tid] = vidx;
+      if (valid) s_vidx[tid] = vidx;                 // slot cnt is written by thread 0 below
       for (int i = tid; i < 8 * 64; i += 256) (&s_wl[0][0])[i] = 0;
       if (tid == 0) {
         const bool has_next = ks + cnt < M;
