@@ -1,0 +1,343 @@
+#!/usr/bin/env python
+"""bench.py -- encode + decode of one synthetic 3DGS frame (octree + RAHT hot path) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path over one frame: gsnfs_octree_encode -> gsnfs_voxel_merge ->
+gsnfs_raht_forward (encode), the decoder's header read-back, then gsnfs_octree_decode ->
+gsnfs_raht_inverse (decode).  `value` is whole-job Mgaussians/s with inputs resident in HBM; `e2e` is the
+same metric through the *_host ABI calls with pinned host buffers (H2D/D2H inside the timed region).
+Multi-GPU: frames are independent (intra-only codec) => replicas only, one frame stream per
+rank, no collective on the data path ("scaling": "weak").  `--impl reference` times the fp64 oracle on the
+host cores (a deliberately slow baseline, not the target).
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "encode+decode Mgaussians/s per frame (octree+RAHT)"
+UNIT = "Mgaussians/s"
+
+
+def load_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """Samples nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index: int):
+        self.gpu = gpu_index
+        self.rows = []
+        self.proc = None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                          "-i", str(self.gpu), "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[1]))
+                mx.append(float(r[2]))
+                for k, nm in enumerate(names):
+                    if r[5 + k].lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                continue
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+# ------------------------------------------------------------------------------------------------
+def algorithmic_bytes(n, nv, s_occ, channels, depth):
+    """SURVEY.md section 8(d) / DESIGN.md 'Algorithmic bytes': what each kernel must move, per launch."""
+    k = 4 if 3 * depth <= 32 else 8
+    passes = (3 * depth + 7) // 8
+    c4 = 4 * channels
+    return {
+        "voxelize_morton_hist": 12 * n + k * n,
+        "onesweep_pass": 2 * (k + 4) * n,
+        "octree_count": k * n,
+        "octree_emit": k * n + 12 * nv + s_occ,
+        "merge": 4 * n + 8 * nv + c4 * n + c4 * nv + 4 * nv,
+        "raht_schedule": 12 * nv + 16 * nv,
+        "raht_forward": c4 * nv + c4 * nv + 16 * nv,
+        "raht_inverse": c4 * nv + c4 * nv + 16 * nv,
+        "scan_reduce": None, "scan_sums": None, "scan_down": None,   # used twice with different inputs
+        "expand_children": (s_occ + 4 * s_occ + 8 * (s_occ + nv) + 12 * nv) / max(depth, 1),
+        "_sort_total": k * n + passes * 2 * (k + 4) * n, "_passes": passes,
+    }
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2606_05650_b200 import binding as B, synth
+
+    torch.cuda.set_device(local_rank)
+    dev = f"cuda:{local_rank}"
+    fr = synth.make_frame(args.config)
+    n, C, J = fr.n, fr.channels, fr.depth
+    ctx = B.Context(max_points=n, max_channels=C, max_depth=J, device=local_rank)
+    buf = B.FrameBuffers(n, C, J, dev)
+    d_xyz = torch.from_numpy(fr.xyz).to(dev)
+    d_attr = torch.from_numpy(fr.attr).to(dev)
+    h_hdr = torch.empty(J + 1 + 4, dtype=torch.int32).pin_memory()
+    stream = torch.cuda.current_stream()
+
+    def step():
+        B.encode_frame(ctx, buf, d_xyz, d_attr, fr.bbox_min, fr.bbox_max, fr.qstep)
+        # the decoder needs the stream header (level sizes) on the host: read it back like a receiver would
+        h_hdr[:J + 1].copy_(buf.level_sizes, non_blocking=True)
+        h_hdr[J + 1:].copy_(buf.counts, non_blocking=True)
+        stream.synchronize()
+        levels = h_hdr[:J + 1].numpy()
+        B.decode_frame(ctx, buf, levels, int(h_hdr[J + 2]), fr.qstep)
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    barrier()
+    nv, s_occ = int(h_hdr[J + 1]), int(h_hdr[J + 2])
+
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    l0 = ctx.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+    e1.record(stream)
+    barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = ctx.launch_count() - l0
+    clocks = sampler.stop()
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * n / (ms_step * 1e-3) / 1e6
+
+    # ---- stage split (encode / decode) and per-kernel durations, live, on the same stream
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+    enc_ms, dec_ms = [], []
+    for _ in range(args.steps):
+        ev[0].record(stream)
+        B.encode_frame(ctx, buf, d_xyz, d_attr, fr.bbox_min, fr.bbox_max, fr.qstep)
+        ev[1].record(stream)
+        B.decode_frame(ctx, buf, h_hdr[:J + 1].numpy(), s_occ, fr.qstep)
+        ev[2].record(stream)
+        torch.cuda.synchronize()
+        enc_ms.append(ev[0].elapsed_time(ev[1]))
+        dec_ms.append(ev[1].elapsed_time(ev[2]))
+    ctx.profile_start(8192)
+    for _ in range(args.steps):
+        step()
+    prof = ctx.profile_stop()
+
+    peak, peak_src = load_peaks()
+    ab = algorithmic_bytes(n, nv, s_occ, C, J)
+    kernels = {}
+    for name, (cnt, tot_ms) in prof.items():
+        avg_us = tot_ms / cnt * 1e3
+        b = ab.get(name)
+        kernels[name] = {"launches_per_step": cnt / args.steps, "avg_us": round(avg_us, 2),
+                         "ms_per_step": round(tot_ms / args.steps, 4),
+                         "alg_GBps": round(b / (avg_us * 1e-6) / 1e9, 1) if b else None}
+    dom = max((k for k in kernels if ab.get(k)), key=lambda k: kernels[k]["ms_per_step"])
+    traffic = None
+    tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    if os.path.exists(tpath):
+        try:
+            traffic = json.load(open(tpath)).get(f"config{args.config}", {}).get(dom)
+        except Exception:
+            traffic = None
+    roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["alg_GBps"], "peak": peak, "unit": "GB/s",
+                "frac": round(kernels[dom]["alg_GBps"] / peak, 4), "traffic": traffic, "peak_source": peak_src,
+                "alg_bytes_per_launch": ab[dom]}
+    sort_ms = kernels.get("onesweep_pass", {}).get("ms_per_step", 0.0)
+    sort_frac = (ab["_sort_total"] / (sort_ms * 1e-3) / 1e9 / peak) if sort_ms else None
+
+    # ---- end to end through the host-buffer ABI calls (pinned host memory, copies inside the timed region)
+    e2e = None
+    if rank == 0 or world > 1:
+        cap = B.gsnfs_occ_capacity(n, J)
+        pin = lambda *s, dt: torch.empty(s, dtype=dt).pin_memory()
+        h_xyz, h_attr = torch.from_numpy(fr.xyz).pin_memory(), torch.from_numpy(fr.attr).pin_memory()
+        h_occ, h_lev = pin(cap, dt=torch.uint8), pin(J + 1, dt=torch.int32)
+        h_w, h_q, h_cnt = pin(n, dt=torch.int32), pin(n, C, dt=torch.int32), pin(4, dt=torch.int32)
+        h_vx, h_out, h_cnt2 = pin(n, 3, dt=torch.int32), pin(n, C, dt=torch.float32), pin(4, dt=torch.int32)
+
+        def e2e_step():
+            B.gsnfs_frame_encode_host(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None,
+                                      h_occ, h_lev, h_w, h_q, h_cnt)
+            B.gsnfs_frame_decode_host(ctx, h_occ, int(h_cnt[1]), h_lev.numpy(), J, h_w, h_q, C, fr.qstep, None,
+                                      h_vx, h_out, h_cnt2)
+
+        for _ in range(2):
+            e2e_step()
+        barrier()
+        ks = max(2, min(args.steps, 10))
+        e0.record(stream)
+        for _ in range(ks):
+            e2e_step()
+        e1.record(stream)
+        barrier()
+        ms_e = e0.elapsed_time(e1)
+        if world > 1:
+            t = torch.tensor([ms_e], dtype=torch.float64, device=dev)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e = float(t.item())
+        ms_e /= ks
+        nv_e = int(h_cnt[0])
+        h2d = n * 12 + n * C * 4 + int(h_cnt[1]) + nv_e * 4 + nv_e * C * 4
+        d2h = 16 + 4 * (J + 1) + int(h_cnt[1]) + nv_e * 4 + nv_e * C * 4 + 16 + nv_e * 12 + nv_e * C * 4
+        e2e = {"value": round(world * n / (ms_e * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_e, 4),
+               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ks}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        cpu = oracle_time(fr, sample_n=None)
+    ctx.close()
+    if rank != 0:
+        return
+    out = {
+        "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 4), "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config - 1}]: N={n} Gaussians, C={C} fp32 channels, "
+                               f"octree depth {J}, qstep=range/{fr.qdiv}, seed per synth.make_frame({args.config})",
+                   "n_gaussians": n, "n_voxels": nv, "occ_bytes": s_occ, "channels": C, "depth": J,
+                   "replicas": world, "l2_policy": "inputs larger than L2 (236 MB frame vs 126 MB L2); "
+                   "intermediates stay wherever the pipeline leaves them"},
+        "encode_ms": round(float(np.median(enc_ms)), 4), "decode_ms": round(float(np.median(dec_ms)), 4),
+        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "gpu_launches_per_step": launches / args.steps,
+        "roofline": roofline,
+        "sort": {"alg_bytes": ab["_sort_total"], "ms_per_step": sort_ms, "passes": ab["_passes"],
+                 "frac_of_peak": round(sort_frac, 4) if sort_frac else None},
+        "kernels": kernels, "cpu_baseline": cpu,
+    }
+    print(json.dumps(out))
+
+
+# ------------------------------------------------------------------------------------------------
+def oracle_time(fr, sample_n=None, steps=1):
+    """Times the fp64 oracle, as it stands, on this box's host cores (single thread: numpy)."""
+    from oracle import gsnfs_oracle as orc
+    xyz, attr = fr.xyz, fr.attr
+    if sample_n is not None and sample_n < fr.n:
+        xyz, attr = xyz[:sample_n], attr[:sample_n]
+    n = xyz.shape[0]
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        enc = orc.encode_frame(xyz, attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+        dec = orc.decode_frame(enc["occ"], enc["level_sizes"], fr.depth, enc["qcoeff"], fr.qstep, enc["weights"])
+    dt = (time.perf_counter() - t0) / steps
+    assert dec["ok"]
+    return {"value": round(n / dt / 1e6, 5), "unit": UNIT, "cores": 1, "kind": "oracle",
+            "sample": f"first {n} of {fr.n} Gaussians of the same frame, encode+decode, {steps} step(s), "
+                      f"{dt:.2f} s/step", "ms_per_step": round(dt * 1e3, 2)}
+
+
+def run_reference(args, rank, world):
+    if rank != 0:
+        return
+    from paper_2606_05650_b200 import synth
+    fr = synth.make_frame(args.config)
+    total = args.steps + args.warmup
+    # bounded sample: the whole run should end within a few minutes (~15 us per Gaussian per step)
+    budget_s = 150.0
+    sample_n = int(min(fr.n, max(10_000, budget_s / max(total, 1) / 16e-6)))
+    for _ in range(args.warmup):
+        oracle_time(fr, sample_n)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        r = oracle_time(fr, sample_n)
+    dt = (time.perf_counter() - t0) / args.steps
+    val = round(sample_n / dt / 1e6, 5)
+    cpu = {"value": val, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": r["sample"]}
+    out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+           "warmup": args.warmup, "ms_per_step": round(dt * 1e3, 3), "higher_is_better": True, "scaling": "weak",
+           "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+           "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (bounded sample of {sample_n} Gaussians per step)",
+                      "n_gaussians": sample_n, "channels": fr.channels, "depth": fr.depth},
+           "cpu_baseline": cpu,
+           "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(out))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); 3 = headline 1M frame")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank, world)
+        return
+    if world > 1:
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        dist.init_process_group("nccl")
+    run_ours(args, rank, world, local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

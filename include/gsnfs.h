@@ -71,6 +71,13 @@ const char* gsnfs_version(void);
 /* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
 uint64_t gsnfs_launch_count(const gsnfs_ctx* ctx);
 
+/* Per-kernel device timing.  gsnfs_profile_start(): from now on every kernel this context launches is
+ * bracketed by a CUDA event pair on its stream (up to max_records launches).  gsnfs_profile_stop():
+ * synchronises the device, stops recording and writes one text line per kernel name into `out` (host):
+ * "<name> <launches> <total_ms>\n".  Used by bench.py for the live roofline figures. */
+int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records);
+int gsnfs_profile_stop(gsnfs_ctx* ctx, char* out /* host */, uint64_t out_cap);
+
 /* Upper bound on occupancy bytes for n points at `depth`: sum_{d<depth} min(8^d, n), rounded up to 16. */
 uint64_t gsnfs_occ_capacity(uint64_t n, int depth);
 

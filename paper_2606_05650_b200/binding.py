@@ -47,6 +47,8 @@ _SIGNATURES = {
     "gsnfs_version": (c_char_p, []),
     "gsnfs_launch_count": (c_uint64, [c_void_p]),
     "gsnfs_occ_capacity": (c_uint64, [c_uint64, c_int]),
+    "gsnfs_profile_start": (c_int, [c_void_p, c_int]),
+    "gsnfs_profile_stop": (c_int, [c_void_p, c_char_p, c_uint64]),
     "gsnfs_octree_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, POINTER(c_float), POINTER(c_float),
                                     c_int, c_void_p, c_uint64, c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "gsnfs_voxel_merge": (c_int, [c_void_p, c_void_p, c_void_p, c_int, c_uint64, c_void_p, c_void_p, c_void_p,
@@ -177,6 +179,19 @@ class Context:
 
     def launch_count(self) -> int:
         return int(lib().gsnfs_launch_count(self.handle))
+
+    def profile_start(self, max_records: int = 4096):
+        self._check(lib().gsnfs_profile_start(self.handle, int(max_records)), "gsnfs_profile_start")
+
+    def profile_stop(self):
+        """-> {kernel name: (launches, total_ms)}; synchronises the device."""
+        buf = ctypes.create_string_buffer(1 << 14)
+        self._check(lib().gsnfs_profile_stop(self.handle, buf, len(buf)), "gsnfs_profile_stop")
+        out = {}
+        for line in buf.value.decode().splitlines():
+            name, cnt, ms = line.split()
+            out[name] = (int(cnt), float(ms))
+        return out
 
     def _check(self, rc, where):
         if rc != GSNFS_OK:

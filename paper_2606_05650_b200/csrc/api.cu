@@ -135,9 +135,57 @@ int gsnfs_create(gsnfs_ctx** out, int device, uint64_t max_points, int max_chann
 void gsnfs_destroy(gsnfs_ctx* ctx) {
   if (!ctx) return;
   cudaSetDevice(ctx->device);
+  for (int i = 0; i < ctx->prof_cap; ++i) { cudaEventDestroy(ctx->prof[i].a); cudaEventDestroy(ctx->prof[i].b); }
+  free(ctx->prof);
   if (ctx->pool) cudaFree(ctx->pool);
   if (ctx->fpool) cudaFree(ctx->fpool);
   free(ctx);
+}
+
+int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records) {
+  if (!ctx || max_records < 1) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  if (max_records > ctx->prof_cap) {
+    ProfRec* np = (ProfRec*)realloc(ctx->prof, sizeof(ProfRec) * (size_t)max_records);
+    if (!np) return GSNFS_E_CAPACITY;
+    ctx->prof = np;
+    for (int i = ctx->prof_cap; i < max_records; ++i) {
+      GSNFS_CUDA_OK(ctx, cudaEventCreate(&ctx->prof[i].a));
+      GSNFS_CUDA_OK(ctx, cudaEventCreate(&ctx->prof[i].b));
+      ctx->prof_cap = i + 1;
+    }
+  }
+  ctx->prof_n = 0;
+  ctx->prof_on = 1;
+  return GSNFS_OK;
+}
+
+int gsnfs_profile_stop(gsnfs_ctx* ctx, char* out, uint64_t out_cap) {
+  if (!ctx || !out || out_cap < 2) return GSNFS_E_INVALID_ARGUMENT;
+  ctx->prof_on = 0;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_CUDA_OK(ctx, cudaDeviceSynchronize());
+  // aggregate by kernel name (names are string literals; compare by content)
+  struct Agg { const char* name; int count; double ms; };
+  Agg agg[64];
+  int na = 0;
+  for (int i = 0; i < ctx->prof_n; ++i) {
+    float ms = 0.f;
+    GSNFS_CUDA_OK(ctx, cudaEventElapsedTime(&ms, ctx->prof[i].a, ctx->prof[i].b));
+    int k = 0;
+    for (; k < na; ++k) if (strcmp(agg[k].name, ctx->prof[i].name) == 0) break;
+    if (k == na) { if (na == 64) continue; agg[na].name = ctx->prof[i].name; agg[na].count = 0; agg[na].ms = 0.0; ++na; }
+    agg[k].count++;
+    agg[k].ms += ms;
+  }
+  size_t off = 0;
+  out[0] = 0;
+  for (int k = 0; k < na; ++k) {
+    const int w = snprintf(out + off, (size_t)out_cap - off, "%s %d %.6f\n", agg[k].name, agg[k].count, agg[k].ms);
+    if (w < 0 || (size_t)w >= (size_t)out_cap - off) return GSNFS_E_CAPACITY;
+    off += (size_t)w;
+  }
+  return GSNFS_OK;
 }
 
 int gsnfs_octree_encode(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_xyz, uint64_t n, const float bbox_min[3],

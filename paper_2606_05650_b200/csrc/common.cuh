@@ -44,9 +44,9 @@ struct RahtPlan {
   uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
 };
 
-struct Region {
-  void* p;
-  size_t bytes;
+struct ProfRec {
+  const char* name;
+  cudaEvent_t a, b;
 };
 
 }  // namespace gsnfs
@@ -59,6 +59,12 @@ struct gsnfs_ctx {
   int max_depth;
   uint64_t launches;
   char err[256];
+
+  // optional per-kernel timing (gsnfs_profile_start/stop): one event pair per launch
+  int prof_on;
+  int prof_n;
+  int prof_cap;
+  gsnfs::ProfRec* prof;
 
   char* pool;
   size_t pool_bytes;
@@ -130,10 +136,23 @@ namespace gsnfs {
     }                                                                                         \
   } while (0)
 
-#define GSNFS_LAUNCH_CHECK(ctx)                 \
-  do {                                          \
-    (ctx)->launches++;                          \
-    GSNFS_CUDA_OK(ctx, cudaPeekAtLastError());  \
+// Bracket every kernel launch: GSNFS_KERNEL(ctx, st, "name") before, GSNFS_LAUNCH_CHECK(ctx, st) after.
+#define GSNFS_KERNEL(ctx, st, kname)                                         \
+  do {                                                                       \
+    if ((ctx)->prof_on && (ctx)->prof_n < (ctx)->prof_cap) {                 \
+      (ctx)->prof[(ctx)->prof_n].name = (kname);                             \
+      cudaEventRecord((ctx)->prof[(ctx)->prof_n].a, (st));                   \
+    }                                                                        \
+  } while (0)
+
+#define GSNFS_LAUNCH_CHECK(ctx, st)                                          \
+  do {                                                                       \
+    (ctx)->launches++;                                                       \
+    if ((ctx)->prof_on && (ctx)->prof_n < (ctx)->prof_cap) {                 \
+      cudaEventRecord((ctx)->prof[(ctx)->prof_n].b, (st));                   \
+      (ctx)->prof_n++;                                                       \
+    }                                                                        \
+    GSNFS_CUDA_OK(ctx, cudaPeekAtLastError());                               \
   } while (0)
 
 __device__ __forceinline__ int msb64(unsigned long long x) { return 63 - __clzll((long long)x); }

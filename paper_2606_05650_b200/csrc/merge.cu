@@ -79,11 +79,12 @@ int run_voxel_merge(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, int ch
   const uint32_t blocks_needed = (n + 16 * ROWS - 1) / (16 * ROWS);
   const uint32_t gcap = (uint32_t)ctx->num_sms * 32u;
   const int grid = (int)(blocks_needed < gcap ? blocks_needed : gcap);
+  GSNFS_KERNEL(ctx, st, "merge");
   if (channels % 4 == 0)
     merge_kernel<4, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, d_merged, d_weights);
   else
     merge_kernel<1, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, d_merged, d_weights);
-  GSNFS_LAUNCH_CHECK(ctx);
+  GSNFS_LAUNCH_CHECK(ctx, st);
   return GSNFS_OK;
 }
 

@@ -70,16 +70,18 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
   uint32_t status = 0;
   if (nv == 0) {
     if (occ_bytes != 0) status = 1;
+    GSNFS_KERNEL(ctx, st, "decode_init");
     decode_init_kernel<<<1, 1, 0, st>>>(ctx->dec_keys_a, d_counts, 0, (uint32_t)occ_bytes, status);
-    GSNFS_LAUNCH_CHECK(ctx);
+    GSNFS_LAUNCH_CHECK(ctx, st);
     return GSNFS_OK;
   }
   if (sum != occ_bytes || level_sizes[0] != 1) status = 1;    // header inconsistent with the stream [O12]
   for (int d = 0; d <= depth; ++d)
     if (level_sizes[d] > ctx->max_points) return GSNFS_E_CAPACITY;
   if (occ_bytes + 1 > ctx->occ_cap) return GSNFS_E_CAPACITY;
+  GSNFS_KERNEL(ctx, st, "decode_init");
   decode_init_kernel<<<1, 1, 0, st>>>(ctx->dec_keys_a, d_counts, nv, (uint32_t)occ_bytes, status);
-  GSNFS_LAUNCH_CHECK(ctx);
+  GSNFS_LAUNCH_CHECK(ctx, st);
   if (status) return GSNFS_OK;        // reported through d_counts->status; nothing decoded
   int rc = run_scan_popc8(ctx, st, d_occ, ctx->dec_scan, (uint32_t)occ_bytes);
   if (rc != GSNFS_OK) return rc;
@@ -89,6 +91,7 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
   for (int d = 0; d < depth; ++d) {
     const uint32_t m_d = level_sizes[d], m_next = level_sizes[d + 1];
     const uint32_t grid = (m_d + 255) / 256;
+    GSNFS_KERNEL(ctx, st, "expand_children");
     if (d == depth - 1) {
       expand_children_kernel<true><<<grid, 256, 0, st>>>(cur, d_occ + off, ctx->dec_scan + off, m_d, m_next,
                                                          d_voxel_keys, d_voxel_xyz, d_counts);
@@ -96,7 +99,7 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
       expand_children_kernel<false><<<grid, 256, 0, st>>>(cur, d_occ + off, ctx->dec_scan + off, m_d, m_next, nxt,
                                                           nullptr, d_counts);
     }
-    GSNFS_LAUNCH_CHECK(ctx);
+    GSNFS_LAUNCH_CHECK(ctx, st);
     off += m_d;
     uint64_t* t = cur; cur = nxt; nxt = t;
   }

@@ -398,8 +398,9 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
   if (n) {
     const uint32_t vwant = (n + 1023u) / 1024u, vcap = (uint32_t)ctx->num_sms * 8u;
     const int vgrid = (int)(vwant < vcap ? vwant : vcap);
+    GSNFS_KERNEL(ctx, st, "voxelize_morton_hist");
     voxelize_kernel<KeyT><<<vgrid, 256, 0, st>>>(d_xyz, n, vp, plan, ka, ctx->hist);
-    GSNFS_LAUNCH_CHECK(ctx);
+    GSNFS_LAUNCH_CHECK(ctx, st);
     const size_t smem = (sizeof(KeyT) + 4) * (size_t)kSortTile;
     const uint32_t status_stride = (uint32_t)((ctx->max_points + kSortTile - 1) / kSortTile) * 256;
     const KeyT* kin = ka;
@@ -407,10 +408,11 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
     const uint32_t* pin = nullptr;
     for (int p = 0; p < plan.passes; ++p) {
       uint32_t* pout = (p == plan.passes - 1) ? d_perm : ((p & 1) ? ctx->pay_b : ctx->pay_a);
+      GSNFS_KERNEL(ctx, st, "onesweep_pass");
       onesweep_kernel<KeyT><<<stiles, kSortThreads, smem, st>>>(
           kin, pin, kout, pout, n, plan.shift[p], plan.bits[p], ctx->hist + p * 256,
           ctx->sort_status + (size_t)p * status_stride, ctx->sort_ticket + p);
-      GSNFS_LAUNCH_CHECK(ctx);
+      GSNFS_LAUNCH_CHECK(ctx, st);
       pin = pout;
       const KeyT* t = kin;
       kin = kout;
@@ -418,15 +420,18 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
     }
     const KeyT* sorted = kin;
     const uint32_t otiles = (n + kOctTile - 1) / kOctTile;
+    GSNFS_KERNEL(ctx, st, "octree_count");
     octree_count_kernel<KeyT><<<otiles, 256, 0, st>>>(sorted, n, depth, otiles, ctx->oct_hist);
-    GSNFS_LAUNCH_CHECK(ctx);
+    GSNFS_LAUNCH_CHECK(ctx, st);
+    GSNFS_KERNEL(ctx, st, "octree_scan");
     octree_scan_kernel<<<1, 1024, 0, st>>>(ctx->oct_hist, ctx->oct_base, otiles, depth, n, ctx->oct_meta,
                                            d_level_sizes, d_voxel_start, d_counts);
-    GSNFS_LAUNCH_CHECK(ctx);
+    GSNFS_LAUNCH_CHECK(ctx, st);
     const size_t esmem = (size_t)depth * (kOctTile + 4);
+    GSNFS_KERNEL(ctx, st, "octree_emit");
     octree_emit_kernel<KeyT><<<otiles, 256, esmem, st>>>(sorted, n, depth, otiles, ctx->oct_hist, ctx->oct_base,
                                                          ctx->oct_meta, d_occ, d_voxel_keys, d_voxel_start);
-    GSNFS_LAUNCH_CHECK(ctx);
+    GSNFS_LAUNCH_CHECK(ctx, st);
   } else {
     GSNFS_CUDA_OK(ctx, cudaMemsetAsync(d_level_sizes, 0, sizeof(uint32_t) * (depth + 1), st));
     GSNFS_CUDA_OK(ctx, cudaMemsetAsync(d_counts, 0, sizeof(gsnfs_counts), st));

@@ -523,8 +523,9 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
     void* args[] = {(void*)&d_keys, (void*)&P, (void*)&n_voxels, (void*)&n_dev, (void*)&ctx->raht_idx,
                     (void*)&ctx->raht_rec, (void*)&ctx->raht_hdr, (void*)&ctx->raht_tile_pend, (void*)&ctx->raht_plan,
                     (void*)&pool_rows, (void*)&hdr_cap};
+    GSNFS_KERNEL(ctx, st, "raht_schedule");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)raht_schedule_kernel, dim3(grid), dim3(256), args, 0, st));
-    ctx->launches++;
+    GSNFS_LAUNCH_CHECK(ctx, st);
   }
   QStepParams qs;
   for (int c = 0; c < GSNFS_MAX_CHANNELS; ++c) qs.step[c] = (qstep && c < channels) ? qstep[c] : 1.0f;
@@ -542,8 +543,9 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
     void* fn = vec4 ? (void*)raht_forward_kernel<4> : (void*)raht_forward_kernel<1>;
     int rc = vec4 ? coop_grid(ctx, raht_forward_kernel<4>, smem, want, &grid) : coop_grid(ctx, raht_forward_kernel<1>, smem, want, &grid);
     if (rc != GSNFS_OK) return rc;
+    GSNFS_KERNEL(ctx, st, "raht_forward");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, st));
-    ctx->launches++;
+    GSNFS_LAUNCH_CHECK(ctx, st);
   } else {
     void* args[] = {(void*)&d_in_q, (void*)&d_in_f, (void*)&d_weights, (void*)&ctx->raht_rows, (void*)&ctx->raht_rec,
                     (void*)&ctx->raht_hdr, (void*)&ctx->raht_plan, (void*)&channels, (void*)&levels, (void*)&qs, (void*)&bias,
@@ -551,8 +553,9 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
     void* fn = vec4 ? (void*)raht_inverse_kernel<4> : (void*)raht_inverse_kernel<1>;
     int rc = vec4 ? coop_grid(ctx, raht_inverse_kernel<4>, smem, want, &grid) : coop_grid(ctx, raht_inverse_kernel<1>, smem, want, &grid);
     if (rc != GSNFS_OK) return rc;
+    GSNFS_KERNEL(ctx, st, "raht_inverse");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, st));
-    ctx->launches++;
+    GSNFS_LAUNCH_CHECK(ctx, st);
   }
   return GSNFS_OK;
 }

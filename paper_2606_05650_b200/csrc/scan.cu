@@ -138,12 +138,15 @@ static int run_scan(gsnfs_ctx* ctx, cudaStream_t st, Loader ld, uint32_t* d_out,
                     const uint32_t* d_n) {
   const uint32_t ntiles = n_cap / kScanTile + 1;
   if (ntiles > ctx->scan_tiles_cap) return GSNFS_E_CAPACITY;
+  GSNFS_KERNEL(ctx, st, "scan_reduce");
   scan_reduce_kernel<Loader><<<ntiles, 256, 0, st>>>(ld, n_cap, d_n, ctx->scan_sums);
-  GSNFS_LAUNCH_CHECK(ctx);
+  GSNFS_LAUNCH_CHECK(ctx, st);
+  GSNFS_KERNEL(ctx, st, "scan_sums");
   scan_sums_kernel<<<1, 1024, 0, st>>>(ctx->scan_sums, ntiles);
-  GSNFS_LAUNCH_CHECK(ctx);
+  GSNFS_LAUNCH_CHECK(ctx, st);
+  GSNFS_KERNEL(ctx, st, "scan_down");
   scan_down_kernel<Loader><<<ntiles, 256, 0, st>>>(ld, n_cap, d_n, ctx->scan_sums, d_out);
-  GSNFS_LAUNCH_CHECK(ctx);
+  GSNFS_LAUNCH_CHECK(ctx, st);
   return GSNFS_OK;
 }
 
