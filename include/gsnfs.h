@@ -78,6 +78,11 @@ uint64_t gsnfs_launch_count(const gsnfs_ctx* ctx);
 int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records);
 int gsnfs_profile_stop(gsnfs_ctx* ctx, char* out /* host */, uint64_t out_cap);
 
+/* Diagnostics: synchronises and copies the RAHT phase plan of the last forward/inverse call to host:
+ * uint32 nphases, overflow, M[32], poff[32], toff[32]; uint64 t_sched[32], t_xform[32] (globaltimer ns at
+ * the end of each phase). */
+int gsnfs_debug_read_plan(gsnfs_ctx* ctx, void* h_out /* host */, uint64_t bytes);
+
 /* Upper bound on occupancy bytes for n points at `depth`: sum_{d<depth} min(8^d, n), rounded up to 16. */
 uint64_t gsnfs_occ_capacity(uint64_t n, int depth);
 

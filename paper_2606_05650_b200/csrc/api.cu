@@ -79,11 +79,12 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_ohist = b.take((size_t)kOctLevels * otiles * 4), o_obase = b.take((size_t)kOctLevels * otiles * 4);
   const size_t o_ometa = b.take((size_t)2 * kOctLevels * 4);
   const size_t o_ssums = b.take((size_t)c->scan_tiles_cap * 4);
-  const size_t o_wpref = b.take((N + 1) * 4);
-  const size_t o_ridx = b.take(c->raht_pool_rows * 4);
+  c->raht_bsum_cap = (uint32_t)(c->raht_hdr_cap / 256 + 2 * kRahtMaxPhases + 8);
+  const size_t o_ridx = b.take(c->raht_rec_cap * 4), o_rpw = b.take(c->raht_rec_cap * 4);
+  const size_t o_rbs = b.take((size_t)c->raht_bsum_cap * 4);
   const size_t o_rrec = b.take(c->raht_rec_cap * sizeof(uint4));
   const size_t o_rhdr = b.take(c->raht_hdr_cap * sizeof(RahtTileHdr));
-  const size_t o_rtp = b.take((N / kRahtTile + 2) * 4);
+  const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
   const size_t o_rplan = b.take(sizeof(RahtPlan));
   const size_t o_rrows = b.take(c->raht_pool_rows * (size_t)C * 4);
   const size_t o_dscan = b.take((c->occ_cap + 1) * 4);
@@ -98,8 +99,8 @@ static int create_impl(gsnfs_ctx* c) {
   c->sort_zero_bytes = o_zero_end - o_hist;
   c->oct_hist = (uint32_t*)(p + o_ohist); c->oct_base = (uint32_t*)(p + o_obase); c->oct_meta = (uint32_t*)(p + o_ometa);
   c->scan_sums = (uint32_t*)(p + o_ssums);
-  c->wprefix = (uint32_t*)(p + o_wpref);
-  c->raht_idx = (uint32_t*)(p + o_ridx); c->raht_rec = (uint4*)(p + o_rrec);
+  c->raht_idx = (uint32_t*)(p + o_ridx); c->raht_pw = (uint32_t*)(p + o_rpw); c->raht_bsum = (uint32_t*)(p + o_rbs);
+  c->raht_rec = (uint4*)(p + o_rrec);
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
   c->dec_scan = (uint32_t*)(p + o_dscan); c->dec_keys_a = (uint64_t*)(p + o_dka); c->dec_keys_b = (uint64_t*)(p + o_dkb);
@@ -140,6 +141,15 @@ void gsnfs_destroy(gsnfs_ctx* ctx) {
   if (ctx->pool) cudaFree(ctx->pool);
   if (ctx->fpool) cudaFree(ctx->fpool);
   free(ctx);
+}
+
+int gsnfs_debug_read_plan(gsnfs_ctx* ctx, void* h_out, uint64_t bytes) {
+  if (!ctx || !h_out) return GSNFS_E_INVALID_ARGUMENT;
+  if (bytes > sizeof(RahtPlan)) bytes = sizeof(RahtPlan);
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_CUDA_OK(ctx, cudaDeviceSynchronize());
+  GSNFS_CUDA_OK(ctx, cudaMemcpy(h_out, ctx->raht_plan, bytes, cudaMemcpyDeviceToHost));
+  return GSNFS_OK;
 }
 
 int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records) {

@@ -26,11 +26,11 @@ struct SortPlan {
 
 // Per-tile header of the RAHT schedule (one per tile per phase).
 struct __align__(16) RahtTileHdr {
-  uint16_t lev_end[64];   // lev_end[l-1] = number of local merges with level <= l  (l = 1..64)
+  uint16_t lev_end[64];   // lev_end[s] = end (exclusive) of the s-th non-empty level's records, s < nseg
   uint32_t pendmask[8];   // bit k set: entry k of the tile stays pending after this phase
   uint32_t pend_off;      // exclusive prefix of pending counts over the phase's earlier tiles
   uint32_t npend;
-  uint32_t nent;          // valid entries in the tile
+  uint32_t nent;          // valid entries in the tile | nseg << 16
   uint32_t nmerge;
 };
 static_assert(sizeof(RahtTileHdr) == 176, "RahtTileHdr layout");
@@ -42,6 +42,8 @@ struct RahtPlan {
   uint32_t M[kRahtMaxPhases + 2];     // active entries of phase p (1-based); M[1] = N_v
   uint32_t poff[kRahtMaxPhases + 2];  // row offset of phase p (p >= 2) in the idx / pending-row pools
   uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
+  unsigned long long t_sched[kRahtMaxPhases + 2];  // globaltimer (ns) at the end of each phase, CTA 0 (diagnostics)
+  unsigned long long t_xform[kRahtMaxPhases + 2];
 };
 
 struct ProfRec {
@@ -88,8 +90,10 @@ struct gsnfs_ctx {
   uint32_t scan_tiles_cap;
 
   // RAHT
-  uint32_t* wprefix;       // max_points + 1
-  uint32_t* raht_idx;      // idx pool for phases >= 2
+  uint32_t* raht_idx;      // pending-entry first-voxel indices, tile strided (raht_hdr_cap x kRahtTile)
+  uint32_t* raht_pw;       // pending-entry node weights, same indexing
+  uint32_t* raht_bsum;     // pending counts summed per 256 tiles
+  uint32_t raht_bsum_cap;
   uint4* raht_rec;         // merge records
   gsnfs::RahtTileHdr* raht_hdr;
   uint32_t* raht_tile_pend;
@@ -165,6 +169,11 @@ __device__ __forceinline__ unsigned lanemask_le() {
   unsigned m;
   asm("mov.u32 %0, %%lanemask_le;" : "=r"(m));
   return m;
+}
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
 }
 __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
   uint32_t v;

@@ -29,6 +29,18 @@ struct QStepParams {
   float step[GSNFS_MAX_CHANNELS];
 };
 
+// ---- small PTX helpers -----------------------------------------------------------------------------
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(s), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) {
+  const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
 __device__ __forceinline__ uint32_t lower_bound_u64(const uint64_t* a, uint32_t lo, uint32_t hi, uint64_t x) {
   while (lo < hi) {                      // first index in [lo, hi) with a[idx] >= x, else hi
     const uint32_t mid = (lo + hi) >> 1;
@@ -37,60 +49,174 @@ __device__ __forceinline__ uint32_t lower_bound_u64(const uint64_t* a, uint32_t 
   return lo;
 }
 
+// Block-wide search in the exclusive prefix E of vals[0..n) (all vals > 0 where it matters): returns the
+// index i and E(i) with E(i) <= target < E(i+1), and the grand total.  All 256 threads must call it.
+struct PrefixHit { uint32_t idx, before, total; };
+__device__ PrefixHit block_prefix_find(const uint32_t* vals, uint32_t n, uint32_t target, uint32_t* s_scan /*9*/,
+                                       uint32_t* s_hit /*2*/) {
+  uint32_t running = 0;
+  if (threadIdx.x == 0) { s_hit[0] = 0; s_hit[1] = 0; }
+  __syncthreads();
+  for (uint32_t base = 0; base < n; base += 256) {
+    const uint32_t i = base + threadIdx.x;
+    const uint32_t v = i < n ? ((const volatile uint32_t*)vals)[i] : 0u;
+    uint32_t tot;
+    const uint32_t ex = block_excl_scan_256(v, s_scan, &tot) + running;
+    if (v && ex <= target && target < ex + v) { s_hit[0] = i; s_hit[1] = ex; }
+    running += tot;
+  }
+  __syncthreads();
+  PrefixHit h;
+  h.idx = s_hit[0]; h.before = s_hit[1]; h.total = running;
+  __syncthreads();
+  return h;
+}
+
 // ------------------------------------------------------------------------------------------------
-// Schedule ("prelude"): all phases in one cooperative launch.
+// Schedule ("prelude"): all phases in one cooperative launch, one grid-wide barrier per phase.
+//
+// Phase p works on a list of M_p nodes (phase 1: the voxels), each with the index of its first voxel
+// (vidx), its weight and -- through vidx -- its Morton code.  Tile t of the phase:
+//   * finds, for every entry k > 0 of the tile, whether its butterfly is local (both sibling ranges, found
+//     by binary search of the Morton prefixes, end inside the tile or at a tile edge whose neighbour has a
+//     higher differing bit); computes W0, W1 from a tile-local weight prefix and a = sqrt(W0/(W0+W1)), b;
+//   * sorts the local butterflies by level into records {k | left<<8 | level<<16, a, b, vidx};
+//   * emits the pending entries (vidx, weight of the merged node) tile-strided for the next phase, their
+//     count, and adds the count into a per-256-tiles bucket sum.
+// After the barrier, phase p+1 maps its entry index to (source tile, rank) through the bucket sums and
+// the per-tile counts, so the pending lists never have to be compacted.
 // ------------------------------------------------------------------------------------------------
+struct SchedPools {
+  uint4* rec;            // (toff + tile) * T + j
+  RahtTileHdr* hdr;      // toff + tile
+  uint32_t* pend_vidx;   // (toff + tile) * T + rank
+  uint32_t* pend_w;      // same indexing
+  uint32_t* tile_pend;   // toff + tile
+  uint32_t* bsum;        // boff + tile / 256
+  uint32_t hdr_cap;
+  uint32_t bsum_cap;
+  uint32_t pool_rows;    // capacity of the pending-row pool used by the transform kernels
+};
+
 __global__ void __launch_bounds__(256) raht_schedule_kernel(
-    const uint64_t* __restrict__ keys, const uint32_t* __restrict__ P, uint32_t n_host,
-    const uint32_t* __restrict__ n_dev, uint32_t* __restrict__ idx_pool, uint4* __restrict__ rec,
-    RahtTileHdr* __restrict__ hdr, uint32_t* __restrict__ tile_pend, RahtPlan* __restrict__ plan,
-    uint32_t pool_rows, uint32_t hdr_cap) {
+    const uint64_t* __restrict__ keys, const uint32_t* __restrict__ weights, uint32_t n_host,
+    const uint32_t* __restrict__ n_dev, SchedPools sp, RahtPlan* __restrict__ plan) {
   cg::grid_group grid = cg::this_grid();
   __shared__ uint64_t s_key[T];
-  __shared__ uint32_t s_vidx[T + 1];
+  __shared__ uint32_t s_wpre[T + 1];       // tile-local exclusive prefix of the entry weights
+  __shared__ uint32_t s_E[T + 1];          // exclusive prefix of source-tile pending counts
   __shared__ uint16_t s_wl[8][64];
   __shared__ uint32_t s_tot[64];
   __shared__ uint32_t s_lstart[64];
+  __shared__ uint16_t s_segend[64];
+  __shared__ uint32_t s_nseg;
   __shared__ uint32_t s_pmask[8];
   __shared__ uint64_t s_edge[2];
-  __shared__ uint32_t s_red[9];
+  __shared__ uint32_t s_scan[9];
+  __shared__ uint32_t s_hit[2];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const uint32_t Nv = n_dev ? min(*n_dev, n_host) : n_host;
-  uint32_t M = Nv, poff = 0, toff = 0;
+  uint32_t M = Nv, toff = 0, boff = 0;
+  uint32_t toff_prev = 0, boff_prev = 0, ntiles_prev = 0, poff = 0;
   int p = 1;
   if (blockIdx.x == 0 && tid == 0) {
-    plan->M[1] = Nv; plan->poff[1] = 0; plan->toff[1] = 0; plan->overflow = 0; plan->nphases = 1;
+    plan->M[0] = 0; plan->M[1] = Nv; plan->poff[1] = 0; plan->toff[1] = 0; plan->overflow = 0; plan->nphases = 1;
+    plan->t_sched[0] = globaltimer_ns();
   }
   while (true) {
     const uint32_t ntiles = (M + T - 1) / T;
-    const uint32_t poff_next = (p == 1) ? 0u : poff + M;
-    const uint32_t* idx_p = (p == 1) ? nullptr : idx_pool + poff;
-    if (toff + ntiles > hdr_cap) {               // uniform over the grid
+    const uint32_t nb = (ntiles + 255) / 256;
+    const uint32_t nb_prev = (ntiles_prev + 255) / 256;
+    if (toff + ntiles > sp.hdr_cap || boff + nb > sp.bsum_cap) {      // uniform over the grid
       if (blockIdx.x == 0 && tid == 0) plan->overflow = 1;
       break;
     }
-    if (blockIdx.x == 0 && tid == 0) { plan->M[p + 1] = 0; plan->poff[p + 1] = poff_next; plan->toff[p + 1] = toff + ntiles; }
+    // side job (p >= 2): exclusive offsets of the previous phase's pending lists -> its tile headers
+    if (p >= 2) {
+      for (uint32_t b = blockIdx.x; b < nb_prev; b += gridDim.x) {
+        uint32_t part = 0;
+        for (uint32_t i = tid; i < b; i += 256) part += ((const volatile uint32_t*)sp.bsum)[boff_prev + i];
+        part = __reduce_add_sync(0xffffffffu, part);
+        if (lane == 0) s_scan[warp] = part;
+        __syncthreads();
+        uint32_t bpre = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) bpre += s_scan[w];
+        __syncthreads();
+        const uint32_t t = b * 256 + tid;
+        const uint32_t v = t < ntiles_prev ? ((const volatile uint32_t*)sp.tile_pend)[toff_prev + t] : 0u;
+        const uint32_t ex = block_excl_scan_256(v, s_scan, nullptr);
+        if (t < ntiles_prev) sp.hdr[toff_prev + t].pend_off = bpre + ex;
+      }
+    }
 
-    // ---- step A: per tile, find the butterflies local to the tile and sort them by level
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const uint32_t ks = tile * T;
       const uint32_t cnt = min((uint32_t)T, M - ks);
       const bool valid = (uint32_t)tid < cnt;
-      const uint32_t vidx = valid ? (idx_p ? idx_p[ks + tid] : ks + tid) : 0xffffffffu;
-      const uint64_t mk = valid ? keys[vidx] : ~0ull;
+      const bool has_prev = ks > 0, has_next = ks + cnt < M;
+      uint32_t vidx = 0xffffffffu, went = 0;
+      uint64_t mk = ~0ull;
+      if (p == 1) {
+        if (valid) { vidx = ks + tid; mk = keys[vidx]; went = weights ? weights[vidx] : 1u; }
+        if (tid == 0) {
+          s_edge[0] = has_prev ? keys[ks - 1] : 0ull;
+          s_edge[1] = has_next ? keys[ks + cnt] : 0ull;
+        }
+      } else {
+        // entry (ks + k) of this phase = rank-th pending entry of source tile t: E(t) <= ks + k < E(t+1)
+        const PrefixHit hb = block_prefix_find(sp.bsum + boff_prev, nb_prev, ks, s_scan, s_hit);
+        const uint32_t tb = hb.idx * 256;
+        const uint32_t nin = min(256u, ntiles_prev - tb);
+        const PrefixHit ht = block_prefix_find(sp.tile_pend + toff_prev + tb, nin, ks - hb.before, s_scan, s_hit);
+        const uint32_t t0 = tb + ht.idx;                 // source tile holding entry ks
+        const uint32_t e0 = hb.before + ht.before;       // E(t0)
+        {
+          const uint32_t t = t0 + tid;
+          const uint32_t v = t < ntiles_prev ? ((const volatile uint32_t*)sp.tile_pend)[toff_prev + t] : 0u;
+          uint32_t tot;
+          const uint32_t ex = block_excl_scan_256(v, s_scan, &tot);
+          s_E[tid] = e0 + ex;
+          if (tid == 0) s_E[T] = e0 + tot;
+        }
+        __syncthreads();
+        if (valid) {
+          const uint32_t gk = ks + tid;
+          uint32_t lo = 0, hi = T;                       // last i in [0, T] with s_E[i] <= gk
+          while (lo < hi) { const uint32_t mid = (lo + hi + 1) >> 1; if (s_E[mid] <= gk) lo = mid; else hi = mid - 1; }
+          const size_t src = (size_t)(toff_prev + t0 + lo) * T + (gk - s_E[lo]);
+          vidx = ((const volatile uint32_t*)sp.pend_vidx)[src];
+          went = ((const volatile uint32_t*)sp.pend_w)[src];
+          mk = keys[vidx];
+        }
+        if (tid == 0) {
+          uint64_t kp = 0, kn = 0;
+          if (has_prev) {                                // entry ks - 1: rank-1 in t0, or the last of tile t0-1
+            const uint32_t r0 = ks - e0;
+            const size_t src = r0 > 0 ? (size_t)(toff_prev + t0) * T + (r0 - 1)
+                                      : (size_t)(toff_prev + t0 - 1) * T +
+                                            (((const volatile uint32_t*)sp.tile_pend)[toff_prev + t0 - 1] - 1);
+            kp = keys[((const volatile uint32_t*)sp.pend_vidx)[src]];
+          }
+          if (has_next) {
+            const uint32_t gk = ks + cnt;
+            uint32_t lo = 0, hi = T;
+            while (lo < hi) { const uint32_t mid = (lo + hi + 1) >> 1; if (s_E[mid] <= gk) lo = mid; else hi = mid - 1; }
+            kn = keys[((const volatile uint32_t*)sp.pend_vidx)[(size_t)(toff_prev + t0 + lo) * T + (gk - s_E[lo])]];
+          }
+          s_edge[0] = kp; s_edge[1] = kn;
+        }
+      }
       s_key[tid] = mk;
-      if (valid) s_vidx[tid] = vidx;                 // slot cnt is written by thread 0 below
       for (int i = tid; i < 8 * 64; i += 256) (&s_wl[0][0])[i] = 0;
-      if (tid == 0) {
-        const bool has_next = ks + cnt < M;
-        const uint32_t vend = has_next ? (idx_p ? idx_p[ks + cnt] : ks + cnt) : Nv;
-        s_vidx[cnt] = vend;                                        // cnt <= T: slot T exists
-        s_edge[0] = ks > 0 ? keys[idx_p ? idx_p[ks - 1] : ks - 1] : 0ull;
-        s_edge[1] = has_next ? keys[vend] : 0ull;
+      {
+        uint32_t tot;
+        const uint32_t ex = block_excl_scan_256(went, s_scan, &tot);     // (contains the barriers)
+        s_wpre[tid] = ex;
+        if (tid == 0) s_wpre[T] = tot;
       }
       __syncthreads();
-      const bool has_prev = ks > 0, has_next = ks + cnt < M;
       const uint64_t x_first = s_edge[0] ^ s_key[0];
       const uint64_t x_end = s_edge[1] ^ s_key[cnt - 1];
       const int hfirst = has_prev ? (x_first ? msb64(x_first) : 0) : 64;
@@ -109,9 +235,10 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
         local = (l > 0 || hfirst > h) && (r < cnt || hend > h);
         if (local) {
           level = h + 1;
-          const uint32_t vk = s_vidx[tid], vl = s_vidx[l], vr = s_vidx[r];
-          const double w0 = P ? (double)(P[vk] - P[vl]) : (double)(vk - vl);
-          const double w1 = P ? (double)(P[vr] - P[vk]) : (double)(vr - vk);
+          const uint32_t pk = s_wpre[tid];
+          const uint32_t pr = (r == cnt) ? s_wpre[T] : s_wpre[r];       // entries >= cnt carry weight 0
+          const double w0 = (double)(pk - s_wpre[l]);
+          const double w1 = (double)(pr - pk);
           fa = (float)sqrt(w0 / (w0 + w1));
           fb = (float)sqrt(w1 / (w0 + w1));
         }
@@ -130,7 +257,7 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
         s_tot[tid] = run;
       }
       __syncthreads();
-      if (warp == 0) {                                             // exclusive scan of 64 level totals
+      if (warp == 0) {                      // exclusive scan of the 64 level totals + compact list of non-empty levels
         const uint32_t t0 = s_tot[2 * lane], t1 = s_tot[2 * lane + 1];
         uint32_t inc = t0 + t1;
 #pragma unroll
@@ -138,9 +265,15 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
         const uint32_t ex = inc - (t0 + t1);
         s_lstart[2 * lane] = ex;
         s_lstart[2 * lane + 1] = ex + t0;
+        const unsigned b0 = __ballot_sync(0xffffffffu, t0 > 0), b1 = __ballot_sync(0xffffffffu, t1 > 0);
+        const uint32_t pos = __popc(b0 & lanemask_lt()) + __popc(b1 & lanemask_lt());
+        if (t0 > 0) s_segend[pos] = (uint16_t)(ex + t0);
+        if (t1 > 0) s_segend[pos + (t0 > 0 ? 1 : 0)] = (uint16_t)(ex + t0 + t1);
+        if (lane == 0) s_nseg = __popc(b0) + __popc(b1);
       }
       __syncthreads();
-      RahtTileHdr* h_out = hdr + toff + tile;
+      const size_t tbase = (size_t)(toff + tile) * T;
+      RahtTileHdr* h_out = sp.hdr + toff + tile;
       if (local) {
         const uint32_t j = s_lstart[level - 1] + s_wl[warp][level - 1] + __popc(lt);
         uint4 rr;
@@ -148,58 +281,60 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
         rr.y = __float_as_uint(fa);
         rr.z = __float_as_uint(fb);
         rr.w = vidx;
-        rec[(size_t)(toff + tile) * T + j] = rr;
+        sp.rec[tbase + j] = rr;
       }
-      if (tid < 64) h_out->lev_end[tid] = (uint16_t)(s_lstart[tid] + s_tot[tid]);
-      if (tid < 8) h_out->pendmask[tid] = s_pmask[tid];
-      if (tid == 0) {
-        uint32_t np = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) np += __popc(s_pmask[w]);
-        h_out->npend = np;
-        h_out->nent = cnt;
-        h_out->nmerge = cnt - np;
-        h_out->pend_off = 0;
-        tile_pend[tile] = np;
-      }
-      __syncthreads();
-    }
-    grid.sync();
-
-    // ---- step B: offsets of the pending entries, next phase's index list
-    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      uint32_t part = 0;
-      for (uint32_t t = tid; t < tile; t += 256) part += tile_pend[t];
-      part = __reduce_add_sync(0xffffffffu, part);
-      if (lane == 0) s_red[warp] = part;
-      if (tid < 8) s_pmask[tid] = hdr[toff + tile].pendmask[tid];
-      __syncthreads();
-      uint32_t pend_off = 0;
-#pragma unroll
-      for (int w = 0; w < 8; ++w) pend_off += s_red[w];
-      uint32_t before = 0, np = 0;
+      uint32_t np = 0, before = 0;
 #pragma unroll
       for (int w = 0; w < 8; ++w) { const uint32_t c = __popc(s_pmask[w]); if (w < warp) before += c; np += c; }
-      const uint32_t ks = tile * T;
-      const bool pend = (s_pmask[warp] >> lane) & 1u;
-      const bool fits = (uint64_t)poff_next + pend_off + np <= pool_rows;
-      if (pend && fits) {
+      if (valid && !local) {
+        // pending node = this entry plus everything merged into it: up to the next pending entry
         const uint32_t rank = before + __popc(s_pmask[warp] & lanemask_lt());
-        idx_pool[poff_next + pend_off + rank] = idx_p ? idx_p[ks + tid] : ks + tid;
+        uint32_t nxt = cnt;                                          // next pending entry after tid
+        {
+          unsigned m = s_pmask[warp] & ~lanemask_le();
+          int w = warp;
+          while (m == 0 && ++w < 8) m = s_pmask[w];
+          if (m) nxt = (uint32_t)(w * 32 + __ffs(m) - 1);
+        }
+        const uint32_t pn = (nxt >= cnt) ? s_wpre[T] : s_wpre[nxt];
+        sp.pend_vidx[tbase + rank] = vidx;
+        sp.pend_w[tbase + rank] = pn - s_wpre[tid];
       }
+      if (tid < 64) h_out->lev_end[tid] = tid < (int)s_nseg ? s_segend[tid] : (uint16_t)0;
+      if (tid < 8) h_out->pendmask[tid] = s_pmask[tid];
       if (tid == 0) {
-        hdr[toff + tile].pend_off = pend_off;
-        if (!fits) plan->overflow = 1;
-        if (tile == ntiles - 1) plan->M[p + 1] = pend_off + np;
+        h_out->npend = np;
+        h_out->nent = cnt | (s_nseg << 16);
+        h_out->nmerge = cnt - np;
+        h_out->pend_off = 0;
+        sp.tile_pend[toff + tile] = np;
+        atomicAdd(&sp.bsum[boff + tile / 256], np);
       }
       __syncthreads();
     }
     grid.sync();
-    const uint32_t M_next = *((volatile uint32_t*)&plan->M[p + 1]);
-    const uint32_t ovf = *((volatile uint32_t*)&plan->overflow);
-    if (M_next <= 1 || ovf || p + 1 > kRahtMaxPhases) break;
+    uint32_t part = 0;
+    for (uint32_t i = tid; i < nb; i += 256) part += ((const volatile uint32_t*)sp.bsum)[boff + i];
+    part = __reduce_add_sync(0xffffffffu, part);
+    if (lane == 0) s_scan[warp] = part;
+    __syncthreads();
+    uint32_t M_next = 0;
+#pragma unroll
+    for (int w = 0; w < 8; ++w) M_next += s_scan[w];
+    __syncthreads();
+    const uint32_t poff_next = (p == 1) ? 0u : poff + M;
+    if (blockIdx.x == 0 && tid == 0) {
+      plan->M[p + 1] = M_next; plan->poff[p + 1] = poff_next; plan->toff[p + 1] = toff + ntiles;
+      plan->t_sched[p] = globaltimer_ns();
+    }
+    if ((uint64_t)poff_next + M_next > sp.pool_rows) {
+      if (blockIdx.x == 0 && tid == 0) plan->overflow = 1;
+      break;
+    }
+    if (M_next <= 1 || p + 1 > kRahtMaxPhases) break;
+    toff_prev = toff; boff_prev = boff; ntiles_prev = ntiles;
     poff = poff_next;
-    toff += ntiles;
+    toff += ntiles; boff += nb;
     M = M_next;
     ++p;
   }
@@ -258,19 +393,47 @@ __device__ __forceinline__ void store_coeff(const float* row_s, int c, int C, si
   }
 }
 
+// Per-tile metadata staged in shared memory (double buffered: the next tile's is prefetched).
+struct __align__(16) TileMeta {
+  uint4 rec[T];
+  RahtTileHdr hdr;
+  uint32_t w[T];          // leaf weights of the tile's rows (phase 1 with weights only)
+};
+
+__device__ __forceinline__ void prefetch_meta(TileMeta* m, const uint4* rec, const RahtTileHdr* hdr,
+                                              const uint32_t* weights, size_t tglob, uint32_t ks, uint32_t cnt) {
+  const int tid = threadIdx.x;
+  cp_async16(&m->rec[tid], rec + tglob * T + tid);
+  if (tid < (int)(sizeof(RahtTileHdr) / 16))
+    cp_async16(reinterpret_cast<uint4*>(&m->hdr) + tid, reinterpret_cast<const uint4*>(hdr + tglob) + tid);
+  if (weights && (uint32_t)tid < cnt) cp_async4(&m->w[tid], weights + ks + tid);
+}
+
+template <int VEC>
+__device__ __forceinline__ void stage_rows_contig(float* s_rows, const float* src, uint32_t nrows, int C) {
+  if constexpr (VEC == 4) {
+    const uint32_t tot = nrows * (uint32_t)(C / 4);
+    const float4* g = reinterpret_cast<const float4*>(src);
+    float4* s = reinterpret_cast<float4*>(s_rows);
+    for (uint32_t i = threadIdx.x; i < tot; i += 256) cp_async16(s + i, g + i);
+  } else {
+    const uint32_t tot = nrows * (uint32_t)C;
+    for (uint32_t i = threadIdx.x; i < tot; i += 256) cp_async4(s_rows + i, src + i);
+  }
+}
+
 template <int VEC>
 __global__ void __launch_bounds__(256) raht_forward_kernel(
     const float* __restrict__ attr_in, const uint32_t* __restrict__ weights, float* __restrict__ pool,
-    const uint4* __restrict__ rec, const RahtTileHdr* __restrict__ hdr, const RahtPlan* __restrict__ plan, int C,
-    int levels, QStepParams qs, int has_q, double dz, int32_t* __restrict__ out_q, float* __restrict__ out_f) {
+    const uint4* __restrict__ rec, const RahtTileHdr* __restrict__ hdr, RahtPlan* __restrict__ plan, int C,
+    QStepParams qs, int has_q, double dz, int32_t* __restrict__ out_q, float* __restrict__ out_f) {
   using V = typename RowVec<VEC>::type;
   cg::grid_group grid = cg::this_grid();
   extern __shared__ __align__(16) unsigned char s_dyn[];
-  float* s_rows = reinterpret_cast<float*>(s_dyn);                      // T x C
-  double* s_qinv = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C);   // C
-  __shared__ uint4 s_rec[T];
-  __shared__ RahtTileHdr s_hdr;
-  __shared__ uint16_t s_plist[T];
+  float* s_rows = reinterpret_cast<float*>(s_dyn);                                // T x C
+  TileMeta* s_meta = reinterpret_cast<TileMeta*>(s_dyn + sizeof(float) * T * C);  // x 2
+  double* s_qinv = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C + 2 * sizeof(TileMeta));
+  __shared__ uint32_t s_dst[T];     // destination row: out row (finished) or pool row | 0x80000000 (pending)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int hw = tid >> 4, l16 = tid & 15;
@@ -279,104 +442,113 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
   if (!has_q) out_q = nullptr;
   const uint32_t nph = plan->nphases;
   if (plan->overflow) return;                                           // uniform: no grid.sync mismatch
+  if (blockIdx.x == 0 && tid == 0) plan->t_xform[0] = globaltimer_ns();
   for (uint32_t p = 1; p <= nph; ++p) {
     const uint32_t M = plan->M[p], Mnext = plan->M[p + 1];
     const uint32_t ntiles = (M + T - 1) / T, toff = plan->toff[p];
     const float* src = (p == 1) ? attr_in : pool + (size_t)plan->poff[p] * C;
     float* dstp = pool + (size_t)plan->poff[p + 1] * C;
+    const uint32_t* wts = (p == 1) ? weights : nullptr;
+    int cur = 0;
+    if (blockIdx.x < ntiles) {
+      const uint32_t ks = blockIdx.x * T;
+      prefetch_meta(&s_meta[0], rec, hdr, wts, (size_t)toff + blockIdx.x, ks, min((uint32_t)T, M - ks));
+    }
+    cp_async_commit();
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const uint32_t ks = tile * T;
-      if (tid < (int)(sizeof(RahtTileHdr) / 4))
-        reinterpret_cast<uint32_t*>(&s_hdr)[tid] = reinterpret_cast<const uint32_t*>(hdr + toff + tile)[tid];
-      __syncthreads();
-      const uint32_t nent = s_hdr.nent, nmerge = s_hdr.nmerge, npend = s_hdr.npend;
-      if ((uint32_t)tid < nmerge) s_rec[tid] = rec[(size_t)(toff + tile) * T + tid];
-      {
-        const V* g = reinterpret_cast<const V*>(src + (size_t)ks * C);
-        V* s = reinterpret_cast<V*>(s_rows);
-        const uint32_t tot = nent * cv;
-        for (uint32_t i = tid; i < tot; i += 256) s[i] = g[i];
+      const uint32_t nent = min((uint32_t)T, M - ks);
+      TileMeta* mt = &s_meta[cur];
+      stage_rows_contig<VEC>(s_rows, src + (size_t)ks * C, nent, C);
+      cp_async_commit();
+      const uint32_t tnext = tile + gridDim.x;
+      if (tnext < ntiles) {
+        const uint32_t ksn = tnext * T;
+        prefetch_meta(&s_meta[cur ^ 1], rec, hdr, wts, (size_t)toff + tnext, ksn, min((uint32_t)T, M - ksn));
       }
-      {   // list of pending entries in order
-        const uint32_t pm = s_hdr.pendmask[warp];
+      cp_async_commit();
+      asm volatile("cp.async.wait_group 1;" ::: "memory");      // meta(cur) + rows(cur) landed; meta(next) may be in flight
+      __syncthreads();
+      const uint32_t nmerge = mt->hdr.nmerge, nseg = mt->hdr.nent >> 16;
+      {   // destination of every entry, in natural order
+        const uint32_t pm = mt->hdr.pendmask[warp];
         uint32_t before = 0;
 #pragma unroll
-        for (int w = 0; w < 8; ++w) if (w < warp) before += __popc(s_hdr.pendmask[w]);
-        if ((pm >> lane) & 1u) s_plist[before + __popc(pm & lanemask_lt())] = (uint16_t)tid;
+        for (int w = 0; w < 8; ++w) if (w < warp) before += __popc(mt->hdr.pendmask[w]);
+        if ((pm >> lane) & 1u) s_dst[tid] = 0x80000000u | (mt->hdr.pend_off + before + __popc(pm & lanemask_lt()));
+        if ((uint32_t)tid < nmerge) { const uint4 rr = mt->rec[tid]; s_dst[rr.x & 0xffu] = rr.w; }
       }
-      __syncthreads();
-      if (p == 1 && weights) {                                          // [R2] x_i = sqrt(w_i) a_i
+      if (wts) {                                                          // [R2] x_i = sqrt(w_i) a_i
         for (uint32_t k = hw; k < nent; k += 16) {
-          const uint32_t w = weights[ks + k];
+          const uint32_t w = mt->w[k];
           if (w != 1u) {
             const double sw = sqrt((double)w);
             V* r = reinterpret_cast<V*>(s_rows + (size_t)k * C);
             for (int c = l16; c < cv; c += 16) r[c] = vscale(r[c], sw);
           }
         }
-        __syncthreads();
       }
+      __syncthreads();
       uint32_t sj = 0;
-      for (int l = 1; l <= levels; ++l) {
-        const uint32_t ej = s_hdr.lev_end[l - 1];
-        if (ej > sj) {
-          for (uint32_t j = sj + hw; j < ej; j += 16) {
-            const uint4 rr = s_rec[j];
-            const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
-            const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
-            V* r0 = reinterpret_cast<V*>(s_rows + (size_t)li * C);
-            V* r1 = reinterpret_cast<V*>(s_rows + (size_t)k * C);
-            for (int c = l16; c < cv; c += 16) {
-              const V y0 = r0[c], y1 = r1[c];
-              r0[c] = bf_lo(a, b, y0, y1);                               // low-pass stays at the left index
-              r1[c] = bf_hi(a, b, y0, y1);                               // high-pass at the right index
-            }
+      for (uint32_t s = 0; s < nseg; ++s) {                               // non-empty levels, bottom-up
+        const uint32_t ej = mt->hdr.lev_end[s];
+        for (uint32_t j = sj + hw; j < ej; j += 16) {
+          const uint4 rr = mt->rec[j];
+          const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
+          const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
+          V* r0 = reinterpret_cast<V*>(s_rows + (size_t)li * C);
+          V* r1 = reinterpret_cast<V*>(s_rows + (size_t)k * C);
+          for (int c = l16; c < cv; c += 16) {
+            const V y0 = r0[c], y1 = r1[c];
+            r0[c] = bf_lo(a, b, y0, y1);                                   // low-pass stays at the left index
+            r1[c] = bf_hi(a, b, y0, y1);                                   // high-pass at the right index
           }
-          __syncthreads();
         }
+        __syncthreads();
         sj = ej;
       }
-      // finished high-pass coefficients -> canonical rows of the output
-      for (uint32_t j = hw; j < nmerge; j += 16) {
-        const uint4 rr = s_rec[j];
-        const uint32_t k = rr.x & 0xffu;
-        for (int c = l16; c < cv; c += 16)
-          store_coeff<VEC>(s_rows + (size_t)k * C, c, C, (size_t)rr.w, s_qinv, dz, out_q, out_f);
-      }
-      // pending low-pass nodes -> next phase's row pool (or, when one node is left, the DC at row 0)
-      const uint32_t pend_off = s_hdr.pend_off;
-      for (uint32_t j = hw; j < npend; j += 16) {
-        const uint32_t k = s_plist[j];
-        if (Mnext == 1u) {
-          for (int c = l16; c < cv; c += 16)
-            store_coeff<VEC>(s_rows + (size_t)k * C, c, C, (size_t)0, s_qinv, dz, out_q, out_f);
+      // rows out, in natural order: finished high-pass -> canonical output row (quantised); pending
+      // low-pass -> next phase's row pool, or -- when a single node is left -- the DC at output row 0
+      for (uint32_t k = hw; k < nent; k += 16) {
+        const uint32_t d = s_dst[k];
+        const float* rs = s_rows + (size_t)k * C;
+        if ((d & 0x80000000u) && Mnext != 1u) {
+          const V* r = reinterpret_cast<const V*>(rs);
+          V* g = reinterpret_cast<V*>(dstp + (size_t)(d & 0x7fffffffu) * C);
+          for (int c = l16; c < cv; c += 16) g[c] = r[c];
         } else {
-          const V* r = reinterpret_cast<const V*>(s_rows + (size_t)k * C);
-          V* d = reinterpret_cast<V*>(dstp + (size_t)(pend_off + j) * C);
-          for (int c = l16; c < cv; c += 16) d[c] = r[c];
+          const size_t orow = (d & 0x80000000u) ? (size_t)0 : (size_t)d;
+          for (int c = l16; c < cv; c += 16) store_coeff<VEC>(rs, c, C, orow, s_qinv, dz, out_q, out_f);
         }
       }
       __syncthreads();
+      cur ^= 1;
     }
+    cp_async_wait_all();
     if (p < nph) grid.sync();
+    if (blockIdx.x == 0 && tid == 0) plan->t_xform[p] = globaltimer_ns();
   }
 }
 
 template <int VEC>
-__device__ __forceinline__ void load_coeff(float* row_s, int c, int C, size_t irow, const double* s_step, double bias,
-                                           const int32_t* in_q, const float* in_f) {
+__device__ __forceinline__ void dequant_row_inplace(float* row_s, int c, const double* s_step, double bias) {
   if constexpr (VEC == 4) {
-    float4 y;
-    if (in_q) {
-      const int4 q = reinterpret_cast<const int4*>(in_q + irow * C)[c];
-      y = make_float4(dequant1(q.x, s_step[4 * c + 0], bias), dequant1(q.y, s_step[4 * c + 1], bias),
-                      dequant1(q.z, s_step[4 * c + 2], bias), dequant1(q.w, s_step[4 * c + 3], bias));
-    } else {
-      y = reinterpret_cast<const float4*>(in_f + irow * C)[c];
-    }
-    reinterpret_cast<float4*>(row_s)[c] = y;
+    const int4 q = reinterpret_cast<const int4*>(row_s)[c];
+    reinterpret_cast<float4*>(row_s)[c] =
+        make_float4(dequant1(q.x, s_step[4 * c + 0], bias), dequant1(q.y, s_step[4 * c + 1], bias),
+                    dequant1(q.z, s_step[4 * c + 2], bias), dequant1(q.w, s_step[4 * c + 3], bias));
   } else {
-    row_s[c] = in_q ? dequant1(in_q[irow * C + c], s_step[c], bias) : in_f[irow * C + c];
+    row_s[c] = dequant1(reinterpret_cast<const int*>(row_s)[c], s_step[c], bias);
+  }
+}
+
+template <int VEC>
+__device__ __forceinline__ void stage_row(float* row_s, const void* src_row, int C, int l16) {
+  if constexpr (VEC == 4) {
+    for (int c = l16; c < C / 4; c += 16)
+      cp_async16(reinterpret_cast<float4*>(row_s) + c, reinterpret_cast<const float4*>(src_row) + c);
+  } else {
+    for (int c = l16; c < C; c += 16) cp_async4(row_s + c, reinterpret_cast<const float*>(src_row) + c);
   }
 }
 
@@ -384,83 +556,97 @@ template <int VEC>
 __global__ void __launch_bounds__(256) raht_inverse_kernel(
     const int32_t* __restrict__ in_q, const float* __restrict__ in_f, const uint32_t* __restrict__ weights,
     float* __restrict__ pool, const uint4* __restrict__ rec, const RahtTileHdr* __restrict__ hdr,
-    const RahtPlan* __restrict__ plan, int C, int levels, QStepParams qs, double bias, float* __restrict__ attr_out) {
+    RahtPlan* __restrict__ plan, int C, QStepParams qs, double bias, float* __restrict__ attr_out) {
   using V = typename RowVec<VEC>::type;
   cg::grid_group grid = cg::this_grid();
   extern __shared__ __align__(16) unsigned char s_dyn[];
   float* s_rows = reinterpret_cast<float*>(s_dyn);
-  double* s_step = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C);
-  __shared__ uint4 s_rec[T];
-  __shared__ RahtTileHdr s_hdr;
-  __shared__ uint16_t s_plist[T];
+  TileMeta* s_meta = reinterpret_cast<TileMeta*>(s_dyn + sizeof(float) * T * C);
+  double* s_step = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C + 2 * sizeof(TileMeta));
+  __shared__ uint32_t s_srcrow[T];  // source row: coefficient row (finished) or pool row | 0x80000000 (pending)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int hw = tid >> 4, l16 = tid & 15;
   const int cv = C / VEC;
   for (int c = tid; c < C; c += 256) s_step[c] = in_q ? (double)qs.step[c] : 0.0;
+  const void* coef = in_q ? (const void*)in_q : (const void*)in_f;       // both are 4-byte rows of C entries
   const uint32_t nph = plan->nphases;
   if (plan->overflow) return;
+  if (blockIdx.x == 0 && tid == 0) plan->t_xform[nph + 1] = globaltimer_ns();
   for (uint32_t p = nph; p >= 1; --p) {
     const uint32_t M = plan->M[p], Mnext = plan->M[p + 1];
     const uint32_t ntiles = (M + T - 1) / T, toff = plan->toff[p];
     const float* srcp = pool + (size_t)plan->poff[p + 1] * C;            // low-pass values from phase p+1
     float* dst = (p == 1) ? attr_out : pool + (size_t)plan->poff[p] * C;
+    const uint32_t* wts = (p == 1) ? weights : nullptr;
+    int cur = 0;
+    if (blockIdx.x < ntiles) {
+      const uint32_t ks = blockIdx.x * T;
+      prefetch_meta(&s_meta[0], rec, hdr, wts, (size_t)toff + blockIdx.x, ks, min((uint32_t)T, M - ks));
+    }
+    cp_async_commit();
+    cp_async_wait_all();
+    __syncthreads();
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const uint32_t ks = tile * T;
-      if (tid < (int)(sizeof(RahtTileHdr) / 4))
-        reinterpret_cast<uint32_t*>(&s_hdr)[tid] = reinterpret_cast<const uint32_t*>(hdr + toff + tile)[tid];
-      __syncthreads();
-      const uint32_t nent = s_hdr.nent, nmerge = s_hdr.nmerge, npend = s_hdr.npend;
-      if ((uint32_t)tid < nmerge) s_rec[tid] = rec[(size_t)(toff + tile) * T + tid];
+      const uint32_t nent = min((uint32_t)T, M - ks);
+      TileMeta* mt = &s_meta[cur];
+      const uint32_t nmerge = mt->hdr.nmerge, nseg = mt->hdr.nent >> 16;
       {
-        const uint32_t pm = s_hdr.pendmask[warp];
+        const uint32_t pm = mt->hdr.pendmask[warp];
         uint32_t before = 0;
 #pragma unroll
-        for (int w = 0; w < 8; ++w) if (w < warp) before += __popc(s_hdr.pendmask[w]);
-        if ((pm >> lane) & 1u) s_plist[before + __popc(pm & lanemask_lt())] = (uint16_t)tid;
+        for (int w = 0; w < 8; ++w) if (w < warp) before += __popc(mt->hdr.pendmask[w]);
+        if ((pm >> lane) & 1u) s_srcrow[tid] = 0x80000000u | (mt->hdr.pend_off + before + __popc(pm & lanemask_lt()));
+        if ((uint32_t)tid < nmerge) { const uint4 rr = mt->rec[tid]; s_srcrow[rr.x & 0xffu] = rr.w; }
       }
       __syncthreads();
-      for (uint32_t j = hw; j < nmerge; j += 16) {                       // high-pass coefficients of this phase
-        const uint4 rr = s_rec[j];
-        const uint32_t k = rr.x & 0xffu;
-        for (int c = l16; c < cv; c += 16)
-          load_coeff<VEC>(s_rows + (size_t)k * C, c, C, (size_t)rr.w, s_step, bias, in_q, in_f);
+      // stage every row of the tile: high-pass coefficients of this phase from the coefficient array,
+      // low-pass inputs from phase p+1's rows (or, when a single node is left, the DC = coefficient row 0)
+      for (uint32_t k = hw; k < nent; k += 16) {
+        const uint32_t s = s_srcrow[k];
+        const void* g = ((s & 0x80000000u) && Mnext != 1u)
+                            ? (const void*)(srcp + (size_t)(s & 0x7fffffffu) * C)
+                            : (const void*)((const float*)coef + (size_t)((s & 0x80000000u) ? 0u : s) * C);
+        stage_row<VEC>(s_rows + (size_t)k * C, g, C, l16);
       }
-      const uint32_t pend_off = s_hdr.pend_off;
-      for (uint32_t j = hw; j < npend; j += 16) {                        // low-pass inputs
-        const uint32_t k = s_plist[j];
-        if (Mnext == 1u) {
-          for (int c = l16; c < cv; c += 16)
-            load_coeff<VEC>(s_rows + (size_t)k * C, c, C, (size_t)0, s_step, bias, in_q, in_f);
-        } else {
-          const V* g = reinterpret_cast<const V*>(srcp + (size_t)(pend_off + j) * C);
-          V* r = reinterpret_cast<V*>(s_rows + (size_t)k * C);
-          for (int c = l16; c < cv; c += 16) r[c] = g[c];
-        }
+      cp_async_commit();
+      const uint32_t tnext = tile + gridDim.x;
+      if (tnext < ntiles) {
+        const uint32_t ksn = tnext * T;
+        prefetch_meta(&s_meta[cur ^ 1], rec, hdr, wts, (size_t)toff + tnext, ksn, min((uint32_t)T, M - ksn));
       }
+      cp_async_commit();
+      asm volatile("cp.async.wait_group 1;" ::: "memory");
       __syncthreads();
-      for (int l = levels; l >= 1; --l) {
-        const uint32_t ej = s_hdr.lev_end[l - 1];
-        const uint32_t sj = l >= 2 ? s_hdr.lev_end[l - 2] : 0u;
-        if (ej > sj) {
-          for (uint32_t j = sj + hw; j < ej; j += 16) {
-            const uint4 rr = s_rec[j];
-            const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
-            const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
-            V* r0 = reinterpret_cast<V*>(s_rows + (size_t)li * C);
-            V* r1 = reinterpret_cast<V*>(s_rows + (size_t)k * C);
-            for (int c = l16; c < cv; c += 16) {
-              const V y0 = r0[c], y1 = r1[c];
-              r0[c] = bf_hi(a, b, y1, y0);          // a*y0 - b*y1  (A.6 l.37)
-              r1[c] = bf_lo(b, a, y0, y1);          // b*y0 + a*y1  (A.6 l.38)
-            }
-          }
-          __syncthreads();
-        }
-      }
-      if (p == 1 && weights) {                                           // [R2] a_i = x_i / sqrt(w_i)
+      if (in_q) {                                                          // de-quantise in place
         for (uint32_t k = hw; k < nent; k += 16) {
-          const uint32_t w = weights[ks + k];
+          const uint32_t s = s_srcrow[k];
+          if (!((s & 0x80000000u) && Mnext != 1u))
+            for (int c = l16; c < cv; c += 16) dequant_row_inplace<VEC>(s_rows + (size_t)k * C, c, s_step, bias);
+        }
+        __syncthreads();
+      }
+      for (int s = (int)nseg - 1; s >= 0; --s) {                           // non-empty levels, top-down
+        const uint32_t ej = mt->hdr.lev_end[s];
+        const uint32_t sj = s > 0 ? mt->hdr.lev_end[s - 1] : 0u;
+        for (uint32_t j = sj + hw; j < ej; j += 16) {
+          const uint4 rr = mt->rec[j];
+          const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
+          const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
+          V* r0 = reinterpret_cast<V*>(s_rows + (size_t)li * C);
+          V* r1 = reinterpret_cast<V*>(s_rows + (size_t)k * C);
+          for (int c = l16; c < cv; c += 16) {
+            const V y0 = r0[c], y1 = r1[c];
+            r0[c] = bf_hi(a, b, y1, y0);          // a*y0 - b*y1  (A.6 l.37)
+            r1[c] = bf_lo(b, a, y0, y1);          // b*y0 + a*y1  (A.6 l.38)
+          }
+        }
+        __syncthreads();
+      }
+      if (wts) {                                                           // [R2] a_i = x_i / sqrt(w_i)
+        for (uint32_t k = hw; k < nent; k += 16) {
+          const uint32_t w = mt->w[k];
           if (w != 1u) {
             const double sw = 1.0 / sqrt((double)w);
             V* r = reinterpret_cast<V*>(s_rows + (size_t)k * C);
@@ -475,14 +661,17 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
         const uint32_t tot = nent * cv;
         for (uint32_t i = tid; i < tot; i += 256) g[i] = s[i];
       }
+      cp_async_wait_all();                                                  // meta(next) before it is read
       __syncthreads();
+      cur ^= 1;
     }
     if (p > 1) grid.sync();
+    if (blockIdx.x == 0 && tid == 0) plan->t_xform[p] = globaltimer_ns();
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-static size_t raht_smem_bytes(int C) { return sizeof(float) * (size_t)T * C + sizeof(double) * C; }
+static size_t raht_smem_bytes(int C) { return sizeof(float) * (size_t)T * C + 2 * sizeof(TileMeta) + sizeof(double) * C; }
 
 int raht_setup(gsnfs_ctx* ctx) {
   const size_t smem = raht_smem_bytes(ctx->max_channels);
@@ -506,23 +695,20 @@ static int coop_grid(gsnfs_ctx* ctx, K kernel, size_t smem, uint32_t want, int* 
 int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_keys, const uint32_t* d_weights,
              uint32_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_in_f, const int32_t* d_in_q,
              int channels, const float* qstep, const gsnfs_quant* quant, int32_t* d_out_q, float* d_out_f) {
+  (void)depth;
   if (n_voxels == 0) return GSNFS_OK;
   const uint32_t* n_dev = d_counts ? &d_counts->n_voxels : nullptr;
-  const uint32_t* P = nullptr;
-  if (d_weights) {
-    int rc = run_scan_u32(ctx, st, d_weights, ctx->wprefix, n_voxels, n_dev);
-    if (rc != GSNFS_OK) return rc;
-    P = ctx->wprefix;
-  }
   const uint32_t want = (n_voxels + T - 1) / T;
-  uint32_t pool_rows = (uint32_t)ctx->raht_pool_rows, hdr_cap = (uint32_t)ctx->raht_hdr_cap;
+  SchedPools sp;
+  sp.rec = ctx->raht_rec; sp.hdr = ctx->raht_hdr; sp.pend_vidx = ctx->raht_idx; sp.pend_w = ctx->raht_pw;
+  sp.tile_pend = ctx->raht_tile_pend; sp.bsum = ctx->raht_bsum;
+  sp.hdr_cap = (uint32_t)ctx->raht_hdr_cap; sp.bsum_cap = ctx->raht_bsum_cap; sp.pool_rows = (uint32_t)ctx->raht_pool_rows;
+  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
   {
     int grid = 0;
     int rc = coop_grid(ctx, raht_schedule_kernel, 0, want, &grid);
     if (rc != GSNFS_OK) return rc;
-    void* args[] = {(void*)&d_keys, (void*)&P, (void*)&n_voxels, (void*)&n_dev, (void*)&ctx->raht_idx,
-                    (void*)&ctx->raht_rec, (void*)&ctx->raht_hdr, (void*)&ctx->raht_tile_pend, (void*)&ctx->raht_plan,
-                    (void*)&pool_rows, (void*)&hdr_cap};
+    void* args[] = {(void*)&d_keys, (void*)&d_weights, (void*)&n_voxels, (void*)&n_dev, (void*)&sp, (void*)&ctx->raht_plan};
     GSNFS_KERNEL(ctx, st, "raht_schedule");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)raht_schedule_kernel, dim3(grid), dim3(256), args, 0, st));
     GSNFS_LAUNCH_CHECK(ctx, st);
@@ -532,13 +718,12 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   const double dz = quant ? (double)quant->dz_round : (double)(1.0f / 3.0f);
   const double bias = quant ? (double)quant->recon_bias : 0.0;
   const size_t smem = raht_smem_bytes(channels);
-  const int levels = 3 * depth;
   const bool vec4 = (channels % 4) == 0;
   int grid = 0;
   if (!inverse) {
     int has_q = (qstep != nullptr && d_out_q != nullptr) ? 1 : 0;
     void* args[] = {(void*)&d_in_f, (void*)&d_weights, (void*)&ctx->raht_rows, (void*)&ctx->raht_rec, (void*)&ctx->raht_hdr,
-                    (void*)&ctx->raht_plan, (void*)&channels, (void*)&levels, (void*)&qs, (void*)&has_q, (void*)&dz,
+                    (void*)&ctx->raht_plan, (void*)&channels, (void*)&qs, (void*)&has_q, (void*)&dz,
                     (void*)&d_out_q, (void*)&d_out_f};
     void* fn = vec4 ? (void*)raht_forward_kernel<4> : (void*)raht_forward_kernel<1>;
     int rc = vec4 ? coop_grid(ctx, raht_forward_kernel<4>, smem, want, &grid) : coop_grid(ctx, raht_forward_kernel<1>, smem, want, &grid);
@@ -548,7 +733,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
     GSNFS_LAUNCH_CHECK(ctx, st);
   } else {
     void* args[] = {(void*)&d_in_q, (void*)&d_in_f, (void*)&d_weights, (void*)&ctx->raht_rows, (void*)&ctx->raht_rec,
-                    (void*)&ctx->raht_hdr, (void*)&ctx->raht_plan, (void*)&channels, (void*)&levels, (void*)&qs, (void*)&bias,
+                    (void*)&ctx->raht_hdr, (void*)&ctx->raht_plan, (void*)&channels, (void*)&qs, (void*)&bias,
                     (void*)&d_out_f};
     void* fn = vec4 ? (void*)raht_inverse_kernel<4> : (void*)raht_inverse_kernel<1>;
     int rc = vec4 ? coop_grid(ctx, raht_inverse_kernel<4>, smem, want, &grid) : coop_grid(ctx, raht_inverse_kernel<1>, smem, want, &grid);
