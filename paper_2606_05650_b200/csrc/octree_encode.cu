@@ -109,15 +109,22 @@ __global__ void __launch_bounds__(kSortThreads) onesweep_kernel(
   // global digit base for this pass (exclusive scan of the pass histogram)
   uint32_t gbase = block_excl_scan_256(ghist[tid], s_scan, nullptr);
 
+  // all match rounds first (independent, so their latencies overlap), then the ordered counter updates
+  unsigned peers[kSortItems];
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
     const bool valid = (wbase + j * 32) < n;
     const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
-    const unsigned peers = __match_any_sync(0xffffffffu, d);
-    const unsigned lt = peers & lanemask_lt();
+    peers[j] = __match_any_sync(0xffffffffu, d);
+  }
+#pragma unroll
+  for (int j = 0; j < kSortItems; ++j) {
+    const bool valid = (wbase + j * 32) < n;
+    const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
+    const unsigned lt = peers[j] & lanemask_lt();
     const uint32_t prev = s_whist[warp][d];
     __syncwarp();
-    if (lt == 0) s_whist[warp][d] = prev + __popc(peers);
+    if (lt == 0) s_whist[warp][d] = prev + __popc(peers[j]);
     __syncwarp();
     rank[j] = prev + __popc(lt);
   }
@@ -141,14 +148,25 @@ __global__ void __launch_bounds__(kSortThreads) onesweep_kernel(
   const uint32_t dstart = block_excl_scan_256(count, s_scan, nullptr);
   uint32_t excl = 0;
   if (tile > 0) {
+    // decoupled look-back, kLookBatch predecessors per round trip (their loads are independent)
+    constexpr int kLookBatch = 8;
     int t = (int)tile - 1;
-    while (true) {
-      const uint32_t* ps = status + (size_t)t * 256 + tid;
-      uint32_t s;
-      do { s = ld_volatile_u32(ps); } while ((s & ~kValMask) == 0u);
-      excl += s & kValMask;
-      if (s & kFlagInc) break;
-      --t;
+    bool done = false;
+    while (!done) {
+      uint32_t sv[kLookBatch];
+#pragma unroll
+      for (int b = 0; b < kLookBatch; ++b)
+        sv[b] = (t - b >= 0) ? ld_volatile_u32(status + (size_t)(t - b) * 256 + tid) : (kFlagInc | 0u);
+#pragma unroll
+      for (int b = 0; b < kLookBatch; ++b) {
+        if (!done) {
+          uint32_t s = sv[b];
+          while ((s & ~kValMask) == 0u) s = ld_volatile_u32(status + (size_t)(t - b) * 256 + tid);
+          excl += s & kValMask;
+          if (s & kFlagInc) done = true;
+        }
+      }
+      t -= kLookBatch;
     }
     st_volatile_u32(my_status, kFlagInc | (excl + count));
   }

@@ -362,36 +362,78 @@ __device__ __forceinline__ float4 vscale(float4 v, double s) {
 }
 __device__ __forceinline__ float vscale(float v, double s) { return (float)((double)v * s); }
 
-__device__ __forceinline__ int quant1(float y, double inv, double f) {
+// Dead-zone quantiser q = sign(y) floor(|y| / step + f), defined in fp64 on the fp32 coefficient [R10].
+// quant_exact is that definition (|y| * (1/step) in fp64; saturates to int32).  quant_fast evaluates
+// t = |y| * inv32 + f in fp32 and takes floor(t) only when t is provably on the same side of every integer
+// as the fp64 value: |t32 - t64| <= 2.4e-7 t + 1e-7, so a guard band of 4e-7 t + 2e-7 around the integers
+// (and t < 2^22) is enough; otherwise it signals a fallback to quant_exact.  floor uses the 1.5*2^23
+// magic-number trick (no F2I / F2F conversions, which run at 1/8 rate).
+__device__ __forceinline__ int quant_exact(float y, double inv, double f) {
   double m = floor(fma(fabs((double)y), inv, f));
   m = fmin(m, 2147483647.0);
   const int q = (int)m;
   return y < 0.f ? -q : q;
+}
+__device__ __forceinline__ bool quant_fast(float y, float inv32, float f32, int* q) {
+  const float t = fmaf(fabsf(y), inv32, f32);
+  const float u = t + 12582912.0f;                       // 1.5 * 2^23: integer part lands in the mantissa
+  const float rn = u - 12582912.0f;                      // round-to-nearest(t)
+  const float fl = rn > t ? rn - 1.0f : rn;              // floor(t)
+  const float frac = t - fl;
+  const float guard = fmaf(t, 4e-7f, 2e-7f);
+  const int qi = (__float_as_int(u) - 0x4B400000) - (rn > t ? 1 : 0);
+  *q = y < 0.f ? -qi : qi;
+  return (frac > guard) && (frac < 1.0f - guard) && (t < 4194304.0f);
 }
 __device__ __forceinline__ float dequant1(int q, double step, double bias) {
   if (q == 0) return 0.f;
   const double m = fabs((double)q) + bias;
   return (float)(q < 0 ? -m * step : m * step);
 }
+// bias == 0 and |q| < 2^24: (float)q * step32 is the single rounding of the exact product = the fp64 result
+__device__ __forceinline__ float dequant_fast(int q, float step32) { return (float)q * step32; }
+
+struct QuantTab {          // per-channel constants in shared memory
+  double* inv64;           // 1 / step            (forward)   |  step   (inverse)
+  float* inv32;            // (float)(1 / step)   (forward)   |  step32 (inverse)
+};
+
+__device__ __forceinline__ int4 quant4(float4 y, int c4, const QuantTab& qt, double dz, float dz32) {
+  int4 q;
+  const float4 iv = reinterpret_cast<const float4*>(qt.inv32)[c4];
+  bool ok = quant_fast(y.x, iv.x, dz32, &q.x);
+  ok &= quant_fast(y.y, iv.y, dz32, &q.y);
+  ok &= quant_fast(y.z, iv.z, dz32, &q.z);
+  ok &= quant_fast(y.w, iv.w, dz32, &q.w);
+  if (!ok) {
+    q.x = quant_exact(y.x, qt.inv64[4 * c4 + 0], dz); q.y = quant_exact(y.y, qt.inv64[4 * c4 + 1], dz);
+    q.z = quant_exact(y.z, qt.inv64[4 * c4 + 2], dz); q.w = quant_exact(y.w, qt.inv64[4 * c4 + 3], dz);
+  }
+  return q;
+}
+__device__ __forceinline__ int quant1s(float y, int c, const QuantTab& qt, double dz, float dz32) {
+  int q;
+  if (!quant_fast(y, qt.inv32[c], dz32, &q)) q = quant_exact(y, qt.inv64[c], dz);
+  return q;
+}
 
 template <int VEC>
-__device__ __forceinline__ void store_coeff(const float* row_s, int c, int C, size_t orow, const double* s_qinv,
-                                            double dz, int32_t* out_q, float* out_f) {
+__device__ __forceinline__ void store_coeff(const float* row_s, int c, int C, size_t orow, const QuantTab& qt, double dz,
+                                            float dz32, int32_t* out_q, float* out_f) {
   if constexpr (VEC == 4) {
     const float4 y = reinterpret_cast<const float4*>(row_s)[c];
     if (out_f) reinterpret_cast<float4*>(out_f + orow * C)[c] = y;
-    if (out_q) {
-      int4 q;
-      q.x = quant1(y.x, s_qinv[4 * c + 0], dz); q.y = quant1(y.y, s_qinv[4 * c + 1], dz);
-      q.z = quant1(y.z, s_qinv[4 * c + 2], dz); q.w = quant1(y.w, s_qinv[4 * c + 3], dz);
-      reinterpret_cast<int4*>(out_q + orow * C)[c] = q;
-    }
+    if (out_q) reinterpret_cast<int4*>(out_q + orow * C)[c] = quant4(y, c, qt, dz, dz32);
   } else {
     const float y = row_s[c];
     if (out_f) out_f[orow * C + c] = y;
-    if (out_q) out_q[orow * C + c] = quant1(y, s_qinv[c], dz);
+    if (out_q) out_q[orow * C + c] = quant1s(y, c, qt, dz, dz32);
   }
 }
+
+// i / d for i < 2^16 and d >= 1: umulhi(i, ceil(2^32 / d)), with d == 1 handled apart (the magic would be 2^32)
+__device__ __forceinline__ uint32_t make_div_magic(uint32_t d) { return d > 1 ? (uint32_t)((0x100000000ull + d - 1) / d) : 0u; }
+__device__ __forceinline__ uint32_t div_cv(uint32_t i, uint32_t magic, uint32_t d) { return d > 1 ? __umulhi(i, magic) : i; }
 
 // Per-tile metadata staged in shared memory (double buffered: the next tile's is prefetched).
 struct __align__(16) TileMeta {
@@ -432,13 +474,21 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
   extern __shared__ __align__(16) unsigned char s_dyn[];
   float* s_rows = reinterpret_cast<float*>(s_dyn);                                // T x C
   TileMeta* s_meta = reinterpret_cast<TileMeta*>(s_dyn + sizeof(float) * T * C);  // x 2
-  double* s_qinv = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C + 2 * sizeof(TileMeta));
+  QuantTab qt;
+  qt.inv64 = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C + 2 * sizeof(TileMeta));
+  qt.inv32 = reinterpret_cast<float*>(qt.inv64 + ((C + 3) & ~3));
   __shared__ uint32_t s_dst[T];     // destination row: out row (finished) or pool row | 0x80000000 (pending)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int hw = tid >> 4, l16 = tid & 15;
   const int cv = C / VEC;
-  for (int c = tid; c < C; c += 256) s_qinv[c] = has_q ? 1.0 / (double)qs.step[c] : 0.0;
+  for (int c = tid; c < C; c += 256) {
+    const double iv = has_q ? 1.0 / (double)qs.step[c] : 0.0;
+    qt.inv64[c] = iv;
+    qt.inv32[c] = (float)iv;
+  }
+  const float dz32 = (float)dz;
+  const uint32_t cv_magic = make_div_magic((uint32_t)(C / VEC));
   if (!has_q) out_q = nullptr;
   const uint32_t nph = plan->nphases;
   if (plan->overflow) return;                                           // uniform: no grid.sync mismatch
@@ -509,16 +559,19 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
       }
       // rows out, in natural order: finished high-pass -> canonical output row (quantised); pending
       // low-pass -> next phase's row pool, or -- when a single node is left -- the DC at output row 0
-      for (uint32_t k = hw; k < nent; k += 16) {
-        const uint32_t d = s_dst[k];
-        const float* rs = s_rows + (size_t)k * C;
-        if ((d & 0x80000000u) && Mnext != 1u) {
-          const V* r = reinterpret_cast<const V*>(rs);
-          V* g = reinterpret_cast<V*>(dstp + (size_t)(d & 0x7fffffffu) * C);
-          for (int c = l16; c < cv; c += 16) g[c] = r[c];
-        } else {
-          const size_t orow = (d & 0x80000000u) ? (size_t)0 : (size_t)d;
-          for (int c = l16; c < cv; c += 16) store_coeff<VEC>(rs, c, C, orow, s_qinv, dz, out_q, out_f);
+      {
+        const uint32_t tot = nent * (uint32_t)cv;
+        for (uint32_t i = tid; i < tot; i += 256) {
+          const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
+          const int c = (int)(i - k * (uint32_t)cv);
+          const uint32_t d = s_dst[k];
+          const float* rs = s_rows + (size_t)k * C;
+          if ((d & 0x80000000u) && Mnext != 1u) {
+            reinterpret_cast<V*>(dstp + (size_t)(d & 0x7fffffffu) * C)[c] = reinterpret_cast<const V*>(rs)[c];
+          } else {
+            const size_t orow = (d & 0x80000000u) ? (size_t)0 : (size_t)d;
+            store_coeff<VEC>(rs, c, C, orow, qt, dz, dz32, out_q, out_f);
+          }
         }
       }
       __syncthreads();
@@ -531,14 +584,22 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
 }
 
 template <int VEC>
-__device__ __forceinline__ void dequant_row_inplace(float* row_s, int c, const double* s_step, double bias) {
+__device__ __forceinline__ void dequant_row_inplace(float* row_s, int c, const QuantTab& qt, double bias) {
   if constexpr (VEC == 4) {
     const int4 q = reinterpret_cast<const int4*>(row_s)[c];
-    reinterpret_cast<float4*>(row_s)[c] =
-        make_float4(dequant1(q.x, s_step[4 * c + 0], bias), dequant1(q.y, s_step[4 * c + 1], bias),
-                    dequant1(q.z, s_step[4 * c + 2], bias), dequant1(q.w, s_step[4 * c + 3], bias));
+    const int amax = max(max(abs(q.x), abs(q.y)), max(abs(q.z), abs(q.w)));
+    float4 y;
+    if (bias == 0.0 && amax < (1 << 24)) {
+      const float4 st = reinterpret_cast<const float4*>(qt.inv32)[c];
+      y = make_float4(dequant_fast(q.x, st.x), dequant_fast(q.y, st.y), dequant_fast(q.z, st.z), dequant_fast(q.w, st.w));
+    } else {
+      y = make_float4(dequant1(q.x, qt.inv64[4 * c + 0], bias), dequant1(q.y, qt.inv64[4 * c + 1], bias),
+                      dequant1(q.z, qt.inv64[4 * c + 2], bias), dequant1(q.w, qt.inv64[4 * c + 3], bias));
+    }
+    reinterpret_cast<float4*>(row_s)[c] = y;
   } else {
-    row_s[c] = dequant1(reinterpret_cast<const int*>(row_s)[c], s_step[c], bias);
+    const int q = reinterpret_cast<const int*>(row_s)[c];
+    row_s[c] = (bias == 0.0 && abs(q) < (1 << 24)) ? dequant_fast(q, qt.inv32[c]) : dequant1(q, qt.inv64[c], bias);
   }
 }
 
@@ -562,13 +623,16 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
   extern __shared__ __align__(16) unsigned char s_dyn[];
   float* s_rows = reinterpret_cast<float*>(s_dyn);
   TileMeta* s_meta = reinterpret_cast<TileMeta*>(s_dyn + sizeof(float) * T * C);
-  double* s_step = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C + 2 * sizeof(TileMeta));
+  QuantTab qt;
+  qt.inv64 = reinterpret_cast<double*>(s_dyn + sizeof(float) * T * C + 2 * sizeof(TileMeta));
+  qt.inv32 = reinterpret_cast<float*>(qt.inv64 + ((C + 3) & ~3));
   __shared__ uint32_t s_srcrow[T];  // source row: coefficient row (finished) or pool row | 0x80000000 (pending)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int hw = tid >> 4, l16 = tid & 15;
   const int cv = C / VEC;
-  for (int c = tid; c < C; c += 256) s_step[c] = in_q ? (double)qs.step[c] : 0.0;
+  for (int c = tid; c < C; c += 256) { qt.inv64[c] = in_q ? (double)qs.step[c] : 0.0; qt.inv32[c] = in_q ? qs.step[c] : 0.f; }
+  const uint32_t cv_magic = make_div_magic((uint32_t)(C / VEC));
   const void* coef = in_q ? (const void*)in_q : (const void*)in_f;       // both are 4-byte rows of C entries
   const uint32_t nph = plan->nphases;
   if (plan->overflow) return;
@@ -603,12 +667,18 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
       __syncthreads();
       // stage every row of the tile: high-pass coefficients of this phase from the coefficient array,
       // low-pass inputs from phase p+1's rows (or, when a single node is left, the DC = coefficient row 0)
-      for (uint32_t k = hw; k < nent; k += 16) {
-        const uint32_t s = s_srcrow[k];
-        const void* g = ((s & 0x80000000u) && Mnext != 1u)
-                            ? (const void*)(srcp + (size_t)(s & 0x7fffffffu) * C)
-                            : (const void*)((const float*)coef + (size_t)((s & 0x80000000u) ? 0u : s) * C);
-        stage_row<VEC>(s_rows + (size_t)k * C, g, C, l16);
+      {
+        const uint32_t tot = nent * (uint32_t)cv;
+        for (uint32_t i = tid; i < tot; i += 256) {
+          const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
+          const uint32_t c = i - k * (uint32_t)cv;
+          const uint32_t s = s_srcrow[k];
+          const float* g = ((s & 0x80000000u) && Mnext != 1u)
+                               ? srcp + (size_t)(s & 0x7fffffffu) * C
+                               : (const float*)coef + (size_t)((s & 0x80000000u) ? 0u : s) * C;
+          if constexpr (VEC == 4) cp_async16(s_rows + (size_t)k * C + 4 * c, g + 4 * c);
+          else cp_async4(s_rows + (size_t)k * C + c, g + c);
+        }
       }
       cp_async_commit();
       const uint32_t tnext = tile + gridDim.x;
@@ -620,10 +690,12 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
       asm volatile("cp.async.wait_group 1;" ::: "memory");
       __syncthreads();
       if (in_q) {                                                          // de-quantise in place
-        for (uint32_t k = hw; k < nent; k += 16) {
+        const uint32_t tot = nent * (uint32_t)cv;
+        for (uint32_t i = tid; i < tot; i += 256) {
+          const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
           const uint32_t s = s_srcrow[k];
           if (!((s & 0x80000000u) && Mnext != 1u))
-            for (int c = l16; c < cv; c += 16) dequant_row_inplace<VEC>(s_rows + (size_t)k * C, c, s_step, bias);
+            dequant_row_inplace<VEC>(s_rows + (size_t)k * C, (int)(i - k * (uint32_t)cv), qt, bias);
         }
         __syncthreads();
       }
@@ -671,7 +743,9 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
 }
 
 // ------------------------------------------------------------------------------------------------
-static size_t raht_smem_bytes(int C) { return sizeof(float) * (size_t)T * C + 2 * sizeof(TileMeta) + sizeof(double) * C; }
+static size_t raht_smem_bytes(int C) {
+  return sizeof(float) * (size_t)T * C + 2 * sizeof(TileMeta) + (sizeof(double) + sizeof(float)) * ((C + 3) & ~3);
+}
 
 int raht_setup(gsnfs_ctx* ctx) {
   const size_t smem = raht_smem_bytes(ctx->max_channels);
