@@ -101,8 +101,8 @@ def algorithmic_bytes(n, nv, s_occ, channels, depth):
         "octree_count": k * n,
         "octree_emit": k * n + 12 * nv + s_occ,
         "merge": 4 * n + 8 * nv + c4 * n + c4 * nv + 4 * nv,
-        "raht_schedule": 12 * nv + 16 * nv,
-        "raht_forward": c4 * nv + c4 * nv + 16 * nv,
+        "raht_schedule": 12 * nv + 16 * nv + 8 * nv,
+        "raht_forward": c4 * nv + c4 * nv + 16 * nv + 8 * nv,   # fused merge: gathers the N input rows itself
         "raht_inverse": c4 * nv + c4 * nv + 16 * nv,
         "scan_reduce": None, "scan_sums": None, "scan_down": None,   # used twice with different inputs
         "expand_children": (s_occ + 4 * s_occ + 8 * (s_occ + nv) + 12 * nv) / max(depth, 1),

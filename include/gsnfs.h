@@ -147,6 +147,18 @@ int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
                        const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
                        int32_t* d_qcoeff, float* d_coeff);
 
+/* Fused gsnfs_voxel_merge + gsnfs_raht_forward(weights = counts): the same coefficients, bit for bit, as
+ * the two calls in sequence, but phase-1 rows are gathered through d_perm straight into shared memory and
+ * the merged N_v x channels tensor is never written (saves a 2 x 4*channels bytes/voxel round trip).
+ * d_attr is the UNSORTED n x channels input; d_weights_out (capacity n) receives the run lengths;
+ * d_counts (required) supplies N_v on the device; n is the row capacity as in gsnfs_raht_forward. */
+int gsnfs_merge_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
+                             const uint64_t* d_voxel_keys, const uint32_t* d_perm, const uint32_t* d_voxel_start,
+                             uint64_t n, const gsnfs_counts* d_counts, int depth,
+                             const float* d_attr /* n x channels, input order */, int channels,
+                             const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
+                             uint32_t* d_weights_out, int32_t* d_qcoeff, float* d_coeff);
+
 /* Inverse transform (A.6 l.24-43): de-quantise (if d_qcoeff != NULL, else take d_coeff), run the same
  * schedule top-down with low' = a*y0 - b*y1, high' = b*y0 + a*y1, then divide row i by sqrt(w_i) [R2]. */
 int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream,

@@ -58,6 +58,8 @@ _SIGNATURES = {
                                     c_void_p, c_void_p]),
     "gsnfs_raht_forward": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p,
                                    c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p, c_void_p]),
+    "gsnfs_merge_raht_forward": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p,
+                                         c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p, c_void_p, c_void_p]),
     "gsnfs_raht_inverse": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p,
                                    c_void_p, c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p]),
     "gsnfs_frame_encode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_int, POINTER(c_float),
@@ -253,6 +255,17 @@ def gsnfs_raht_forward(ctx: Context, d_voxel_keys, d_weights, n_voxels, d_counts
     ctx._check(rc, "gsnfs_raht_forward")
 
 
+def gsnfs_merge_raht_forward(ctx: Context, d_voxel_keys, d_perm, d_voxel_start, n, d_counts, depth, d_attr, channels, qstep,
+                             quant, d_weights_out, d_qcoeff, d_coeff, stream=None):
+    rc = lib().gsnfs_merge_raht_forward(
+        ctx.handle, _stream(stream), _dptr(d_voxel_keys, torch.int64, "d_voxel_keys"), _dptr(d_perm, torch.int32, "d_perm"),
+        _dptr(d_voxel_start, torch.int32, "d_voxel_start"), int(n), _dptr(d_counts, torch.int32, "d_counts"), int(depth),
+        _dptr(d_attr, torch.float32, "d_attr"), int(channels), _farr(qstep, channels), _quant(quant),
+        _dptr(d_weights_out, torch.int32, "d_weights_out"), _dptr(d_qcoeff, torch.int32, "d_qcoeff"),
+        _dptr(d_coeff, torch.float32, "d_coeff"))
+    ctx._check(rc, "gsnfs_merge_raht_forward")
+
+
 def gsnfs_raht_inverse(ctx: Context, d_voxel_keys, d_weights, n_voxels, d_counts, depth, d_qcoeff, d_coeff, channels,
                        qstep, quant, d_attr_out, stream=None):
     rc = lib().gsnfs_raht_inverse(
@@ -311,10 +324,16 @@ class FrameBuffers:
         self.dec_attr = torch.empty((n1, channels), dtype=torch.float32, device=dev)
 
 
-def encode_frame(ctx: Context, buf: FrameBuffers, d_xyz, d_attr, bbox_min, bbox_max, qstep, quant=None, stream=None):
-    """The encoder's three ABI calls chained on one stream with no host synchronisation."""
+def encode_frame(ctx: Context, buf: FrameBuffers, d_xyz, d_attr, bbox_min, bbox_max, qstep, quant=None, stream=None,
+                 fused=True):
+    """The encoder's ABI calls chained on one stream with no host synchronisation.  fused=True uses
+    gsnfs_merge_raht_forward (merge folded into the transform); fused=False the separate calls."""
     gsnfs_octree_encode(ctx, d_xyz, buf.n, bbox_min, bbox_max, buf.depth, buf.occ, buf.level_sizes, buf.perm,
                         buf.voxel_keys, buf.voxel_start, buf.counts, stream)
+    if fused:
+        gsnfs_merge_raht_forward(ctx, buf.voxel_keys, buf.perm, buf.voxel_start, buf.n, buf.counts, buf.depth, d_attr,
+                                 buf.channels, qstep, quant, buf.weights, buf.qcoeff, None, stream)
+        return
     gsnfs_voxel_merge(ctx, d_attr, buf.channels, buf.n, buf.perm, buf.voxel_start, buf.counts, buf.merged,
                       buf.weights, stream)
     gsnfs_raht_forward(ctx, buf.voxel_keys, buf.weights, buf.n, buf.counts, buf.depth, buf.merged, buf.channels,

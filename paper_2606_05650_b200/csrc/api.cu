@@ -82,6 +82,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->raht_bsum_cap = (uint32_t)(c->raht_hdr_cap / 256 + 2 * kRahtMaxPhases + 8);
   const size_t o_ridx = b.take(c->raht_rec_cap * 4), o_rpw = b.take(c->raht_rec_cap * 4);
   const size_t o_rbs = b.take((size_t)c->raht_bsum_cap * 4);
+  const size_t o_rgs = b.take(N * 4);
   const size_t o_rrec = b.take(c->raht_rec_cap * sizeof(uint4));
   const size_t o_rhdr = b.take(c->raht_hdr_cap * sizeof(RahtTileHdr));
   const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
@@ -100,7 +101,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->oct_hist = (uint32_t*)(p + o_ohist); c->oct_base = (uint32_t*)(p + o_obase); c->oct_meta = (uint32_t*)(p + o_ometa);
   c->scan_sums = (uint32_t*)(p + o_ssums);
   c->raht_idx = (uint32_t*)(p + o_ridx); c->raht_pw = (uint32_t*)(p + o_rpw); c->raht_bsum = (uint32_t*)(p + o_rbs);
-  c->raht_rec = (uint4*)(p + o_rrec);
+  c->raht_rec = (uint4*)(p + o_rrec); c->raht_gsrc = (uint32_t*)(p + o_rgs);
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
   c->dec_scan = (uint32_t*)(p + o_dscan); c->dec_keys_a = (uint64_t*)(p + o_dka); c->dec_keys_b = (uint64_t*)(p + o_dkb);
@@ -266,6 +267,22 @@ int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_vo
                   nullptr, channels, qstep, quant, d_qcoeff, d_coeff);
 }
 
+int gsnfs_merge_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_perm,
+                             const uint32_t* d_voxel_start, uint64_t n, const gsnfs_counts* d_counts, int depth,
+                             const float* d_attr, int channels, const float* qstep, const gsnfs_quant* quant,
+                             uint32_t* d_weights_out, int32_t* d_qcoeff, float* d_coeff) {
+  int rc = raht_check(ctx, d_voxel_keys, n, depth, channels);
+  if (rc != GSNFS_OK) return rc;
+  if (!d_counts || (n && (!d_perm || !d_voxel_start || !d_attr || !d_weights_out || (!d_qcoeff && !d_coeff) || (d_qcoeff && !qstep))))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (qstep)
+    for (int c = 0; c < channels; ++c)
+      if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return run_raht(ctx, (cudaStream_t)stream, false, d_voxel_keys, nullptr, (uint32_t)n, d_counts, depth, d_attr, nullptr,
+                  channels, qstep, quant, d_qcoeff, d_coeff, d_perm, d_voxel_start, d_weights_out);
+}
+
 int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_weights,
                        uint64_t n_voxels, const gsnfs_counts* d_counts, int depth, const int32_t* d_qcoeff,
                        const float* d_coeff, int channels, const float* qstep, const gsnfs_quant* quant,
@@ -321,11 +338,8 @@ int gsnfs_frame_encode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_
   rc = gsnfs_octree_encode(ctx, stream, ctx->f_xyz, n, bbox_min, bbox_max, depth, ctx->f_occ, cap, ctx->f_levels,
                            ctx->f_perm, ctx->f_vkeys, ctx->f_vstart, ctx->f_counts);
   if (rc != GSNFS_OK) return rc;
-  rc = gsnfs_voxel_merge(ctx, stream, ctx->f_attr, channels, n, ctx->f_perm, ctx->f_vstart, ctx->f_counts, ctx->f_merged,
-                         ctx->f_weights);
-  if (rc != GSNFS_OK) return rc;
-  rc = gsnfs_raht_forward(ctx, stream, ctx->f_vkeys, ctx->f_weights, n, ctx->f_counts, depth, ctx->f_merged, channels,
-                          qstep, quant, ctx->f_q, nullptr);
+  rc = gsnfs_merge_raht_forward(ctx, stream, ctx->f_vkeys, ctx->f_perm, ctx->f_vstart, n, ctx->f_counts, depth, ctx->f_attr,
+                                channels, qstep, quant, ctx->f_weights, ctx->f_q, nullptr);
   if (rc != GSNFS_OK) return rc;
   // header first: the sizes of the remaining copies depend on it
   GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_counts, ctx->f_counts, sizeof(gsnfs_counts), cudaMemcpyDeviceToHost, st));

@@ -93,6 +93,7 @@ struct gsnfs_ctx {
   uint32_t* raht_idx;      // pending-entry first-voxel indices, tile strided (raht_hdr_cap x kRahtTile)
   uint32_t* raht_pw;       // pending-entry node weights, same indexing
   uint32_t* raht_bsum;     // pending counts summed per 256 tiles
+  uint32_t* raht_gsrc;     // fused merge: first Gaussian of every voxel
   uint32_t raht_bsum_cap;
   uint4* raht_rec;         // merge records
   gsnfs::RahtTileHdr* raht_hdr;
@@ -227,7 +228,8 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
 int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_keys, const uint32_t* d_weights,
              uint32_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_in_f,
              const int32_t* d_in_q, int channels, const float* qstep, const gsnfs_quant* quant,
-             int32_t* d_out_q, float* d_out_f);
+             int32_t* d_out_q, float* d_out_f, const uint32_t* d_perm = nullptr, const uint32_t* d_vstart = nullptr,
+             uint32_t* d_weights_out = nullptr);
 int raht_setup(gsnfs_ctx* ctx);   // occupancy queries + attributes, called from gsnfs_create
 
 // generic exclusive scan of uint32 (weights) with the element count read on the device

@@ -96,6 +96,11 @@ struct SchedPools {
   uint32_t hdr_cap;
   uint32_t bsum_cap;
   uint32_t pool_rows;    // capacity of the pending-row pool used by the transform kernels
+  // fused merge (gsnfs_merge_raht_forward): leaf weight = run length in the sorted permutation
+  const uint32_t* perm;      // NULL unless fused
+  const uint32_t* vstart;
+  uint32_t* gsrc;            // out: index of the first Gaussian of every voxel
+  uint32_t* weights_out;     // out: run lengths
 };
 
 __global__ void __launch_bounds__(256) raht_schedule_kernel(
@@ -159,7 +164,18 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
       uint32_t vidx = 0xffffffffu, went = 0;
       uint64_t mk = ~0ull;
       if (p == 1) {
-        if (valid) { vidx = ks + tid; mk = keys[vidx]; went = weights ? weights[vidx] : 1u; }
+        if (valid) {
+          vidx = ks + tid;
+          mk = keys[vidx];
+          if (sp.perm) {
+            const uint32_t s0 = sp.vstart[vidx], s1 = sp.vstart[vidx + 1];
+            went = s1 - s0;
+            sp.gsrc[vidx] = sp.perm[s0];
+            sp.weights_out[vidx] = went;
+          } else {
+            went = weights ? weights[vidx] : 1u;
+          }
+        }
         if (tid == 0) {
           s_edge[0] = has_prev ? keys[ks - 1] : 0ull;
           s_edge[1] = has_next ? keys[ks + cnt] : 0ull;
@@ -440,15 +456,18 @@ struct __align__(16) TileMeta {
   uint4 rec[T];
   RahtTileHdr hdr;
   uint32_t w[T];          // leaf weights of the tile's rows (phase 1 with weights only)
+  uint32_t g[T];          // fused merge: first Gaussian of each voxel (phase 1 only)
 };
 
 __device__ __forceinline__ void prefetch_meta(TileMeta* m, const uint4* rec, const RahtTileHdr* hdr,
-                                              const uint32_t* weights, size_t tglob, uint32_t ks, uint32_t cnt) {
+                                              const uint32_t* weights, const uint32_t* gsrc, size_t tglob, uint32_t ks,
+                                              uint32_t cnt) {
   const int tid = threadIdx.x;
   cp_async16(&m->rec[tid], rec + tglob * T + tid);
   if (tid < (int)(sizeof(RahtTileHdr) / 16))
     cp_async16(reinterpret_cast<uint4*>(&m->hdr) + tid, reinterpret_cast<const uint4*>(hdr + tglob) + tid);
   if (weights && (uint32_t)tid < cnt) cp_async4(&m->w[tid], weights + ks + tid);
+  if (gsrc && (uint32_t)tid < cnt) cp_async4(&m->g[tid], gsrc + ks + tid);
 }
 
 template <int VEC>
@@ -464,9 +483,15 @@ __device__ __forceinline__ void stage_rows_contig(float* s_rows, const float* sr
   }
 }
 
+struct GatherArgs {          // fused merge: rows of phase 1 are gathered through the sorted permutation
+  const uint32_t* gsrc;      // NULL => rows are contiguous
+  const uint32_t* perm;
+  const uint32_t* vstart;
+};
+
 template <int VEC>
 __global__ void __launch_bounds__(256) raht_forward_kernel(
-    const float* __restrict__ attr_in, const uint32_t* __restrict__ weights, float* __restrict__ pool,
+    const float* __restrict__ attr_in, const uint32_t* __restrict__ weights, GatherArgs ga, float* __restrict__ pool,
     const uint4* __restrict__ rec, const RahtTileHdr* __restrict__ hdr, RahtPlan* __restrict__ plan, int C,
     QStepParams qs, int has_q, double dz, int32_t* __restrict__ out_q, float* __restrict__ out_f) {
   using V = typename RowVec<VEC>::type;
@@ -499,22 +524,36 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
     const float* src = (p == 1) ? attr_in : pool + (size_t)plan->poff[p] * C;
     float* dstp = pool + (size_t)plan->poff[p + 1] * C;
     const uint32_t* wts = (p == 1) ? weights : nullptr;
+    const uint32_t* gsrc = (p == 1) ? ga.gsrc : nullptr;
     int cur = 0;
     if (blockIdx.x < ntiles) {
       const uint32_t ks = blockIdx.x * T;
-      prefetch_meta(&s_meta[0], rec, hdr, wts, (size_t)toff + blockIdx.x, ks, min((uint32_t)T, M - ks));
+      prefetch_meta(&s_meta[0], rec, hdr, wts, gsrc, (size_t)toff + blockIdx.x, ks, min((uint32_t)T, M - ks));
     }
     cp_async_commit();
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const uint32_t ks = tile * T;
       const uint32_t nent = min((uint32_t)T, M - ks);
       TileMeta* mt = &s_meta[cur];
-      stage_rows_contig<VEC>(s_rows, src + (size_t)ks * C, nent, C);
+      if (gsrc) {
+        cp_async_wait_all();                       // meta(cur) was prefetched one tile ago
+        __syncthreads();
+        const uint32_t tot = nent * (uint32_t)cv;
+        for (uint32_t i = tid; i < tot; i += 256) {
+          const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
+          const uint32_t c = i - k * (uint32_t)cv;
+          const float* g = src + (size_t)mt->g[k] * C;
+          if constexpr (VEC == 4) cp_async16(s_rows + (size_t)k * C + 4 * c, g + 4 * c);
+          else cp_async4(s_rows + (size_t)k * C + c, g + c);
+        }
+      } else {
+        stage_rows_contig<VEC>(s_rows, src + (size_t)ks * C, nent, C);
+      }
       cp_async_commit();
       const uint32_t tnext = tile + gridDim.x;
       if (tnext < ntiles) {
         const uint32_t ksn = tnext * T;
-        prefetch_meta(&s_meta[cur ^ 1], rec, hdr, wts, (size_t)toff + tnext, ksn, min((uint32_t)T, M - ksn));
+        prefetch_meta(&s_meta[cur ^ 1], rec, hdr, wts, gsrc, (size_t)toff + tnext, ksn, min((uint32_t)T, M - ksn));
       }
       cp_async_commit();
       asm volatile("cp.async.wait_group 1;" ::: "memory");      // meta(cur) + rows(cur) landed; meta(next) may be in flight
@@ -532,8 +571,27 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
         for (uint32_t k = hw; k < nent; k += 16) {
           const uint32_t w = mt->w[k];
           if (w != 1u) {
-            const double sw = sqrt((double)w);
             V* r = reinterpret_cast<V*>(s_rows + (size_t)k * C);
+            if (gsrc) {      // duplicate voxel: mean of its Gaussians, fp64 accumulation in sorted order [O9]
+              const uint32_t s0 = ga.vstart[ks + k];
+              for (int c = l16; c < cv; c += 16) {
+                if constexpr (VEC == 4) {
+                  const float4 x = r[c];
+                  double a0 = x.x, a1 = x.y, a2 = x.z, a3 = x.w;
+                  for (uint32_t q = 1; q < w; ++q) {
+                    const float4 y = reinterpret_cast<const float4*>(src + (size_t)ga.perm[s0 + q] * C)[c];
+                    a0 += y.x; a1 += y.y; a2 += y.z; a3 += y.w;
+                  }
+                  const double dw = (double)w;
+                  r[c] = make_float4((float)(a0 / dw), (float)(a1 / dw), (float)(a2 / dw), (float)(a3 / dw));
+                } else {
+                  double a0 = r[c];
+                  for (uint32_t q = 1; q < w; ++q) a0 += src[(size_t)ga.perm[s0 + q] * C + c];
+                  r[c] = (float)(a0 / (double)w);
+                }
+              }
+            }
+            const double sw = sqrt((double)w);
             for (int c = l16; c < cv; c += 16) r[c] = vscale(r[c], sw);
           }
         }
@@ -646,7 +704,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
     int cur = 0;
     if (blockIdx.x < ntiles) {
       const uint32_t ks = blockIdx.x * T;
-      prefetch_meta(&s_meta[0], rec, hdr, wts, (size_t)toff + blockIdx.x, ks, min((uint32_t)T, M - ks));
+      prefetch_meta(&s_meta[0], rec, hdr, wts, nullptr, (size_t)toff + blockIdx.x, ks, min((uint32_t)T, M - ks));
     }
     cp_async_commit();
     cp_async_wait_all();
@@ -684,7 +742,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
       const uint32_t tnext = tile + gridDim.x;
       if (tnext < ntiles) {
         const uint32_t ksn = tnext * T;
-        prefetch_meta(&s_meta[cur ^ 1], rec, hdr, wts, (size_t)toff + tnext, ksn, min((uint32_t)T, M - ksn));
+        prefetch_meta(&s_meta[cur ^ 1], rec, hdr, wts, nullptr, (size_t)toff + tnext, ksn, min((uint32_t)T, M - ksn));
       }
       cp_async_commit();
       asm volatile("cp.async.wait_group 1;" ::: "memory");
@@ -768,7 +826,8 @@ static int coop_grid(gsnfs_ctx* ctx, K kernel, size_t smem, uint32_t want, int* 
 
 int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_keys, const uint32_t* d_weights,
              uint32_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_in_f, const int32_t* d_in_q,
-             int channels, const float* qstep, const gsnfs_quant* quant, int32_t* d_out_q, float* d_out_f) {
+             int channels, const float* qstep, const gsnfs_quant* quant, int32_t* d_out_q, float* d_out_f,
+             const uint32_t* d_perm, const uint32_t* d_vstart, uint32_t* d_weights_out) {
   (void)depth;
   if (n_voxels == 0) return GSNFS_OK;
   const uint32_t* n_dev = d_counts ? &d_counts->n_voxels : nullptr;
@@ -777,6 +836,11 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   sp.rec = ctx->raht_rec; sp.hdr = ctx->raht_hdr; sp.pend_vidx = ctx->raht_idx; sp.pend_w = ctx->raht_pw;
   sp.tile_pend = ctx->raht_tile_pend; sp.bsum = ctx->raht_bsum;
   sp.hdr_cap = (uint32_t)ctx->raht_hdr_cap; sp.bsum_cap = ctx->raht_bsum_cap; sp.pool_rows = (uint32_t)ctx->raht_pool_rows;
+  const bool fused = d_perm != nullptr;
+  sp.perm = d_perm; sp.vstart = d_vstart; sp.gsrc = ctx->raht_gsrc; sp.weights_out = d_weights_out;
+  if (fused) d_weights = d_weights_out;        // the transform kernels read the run lengths the schedule writes
+  GatherArgs ga;
+  ga.gsrc = fused ? ctx->raht_gsrc : nullptr; ga.perm = d_perm; ga.vstart = d_vstart;
   GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
   {
     int grid = 0;
@@ -796,7 +860,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   int grid = 0;
   if (!inverse) {
     int has_q = (qstep != nullptr && d_out_q != nullptr) ? 1 : 0;
-    void* args[] = {(void*)&d_in_f, (void*)&d_weights, (void*)&ctx->raht_rows, (void*)&ctx->raht_rec, (void*)&ctx->raht_hdr,
+    void* args[] = {(void*)&d_in_f, (void*)&d_weights, (void*)&ga, (void*)&ctx->raht_rows, (void*)&ctx->raht_rec, (void*)&ctx->raht_hdr,
                     (void*)&ctx->raht_plan, (void*)&channels, (void*)&qs, (void*)&has_q, (void*)&dz,
                     (void*)&d_out_q, (void*)&d_out_f};
     void* fn = vec4 ? (void*)raht_forward_kernel<4> : (void*)raht_forward_kernel<1>;

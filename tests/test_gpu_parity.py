@@ -231,6 +231,33 @@ def test_unit_weights_paper_mode(B, ctx_small):
     assert np.all(np.abs(back.cpu().numpy() - ref["merged"]) <= 1e-4 * rng_c)     # perfect reconstruction
 
 
+@pytest.mark.parametrize("maker", ["config1", "dense56", "dense7", "dense12"])
+def test_fused_merge_forward_equals_separate_calls(B, ctx_small, maker):
+    fr = {"config1": lambda: synth.make_frame(1),
+          "dense56": lambda: synth.make_dense_frame(n=20_000, depth=5, channels=56, seed=3),
+          "dense7": lambda: synth.make_dense_frame(n=3_000, depth=4, channels=7, seed=4),
+          "dense12": lambda: synth.make_dense_frame(n=30_000, depth=6, channels=12, seed=5)}[maker]()
+    buf, got = gpu_position_encode(B, ctx_small, fr)
+    nv = got["n_voxels"]
+    d_attr = _t(fr.attr)
+    B.gsnfs_voxel_merge(ctx_small, d_attr, fr.channels, fr.n, buf.perm, buf.voxel_start, buf.counts, buf.merged, buf.weights)
+    c1 = torch.zeros((fr.n, fr.channels), dtype=torch.float32, device=DEV)
+    q1 = torch.zeros((fr.n, fr.channels), dtype=torch.int32, device=DEV)
+    B.gsnfs_raht_forward(ctx_small, buf.voxel_keys, buf.weights, fr.n, buf.counts, fr.depth, buf.merged, fr.channels,
+                         fr.qstep, None, q1, c1)
+    w2 = torch.zeros(fr.n, dtype=torch.int32, device=DEV)
+    c2 = torch.zeros_like(c1)
+    q2 = torch.zeros_like(q1)
+    B.gsnfs_merge_raht_forward(ctx_small, buf.voxel_keys, buf.perm, buf.voxel_start, fr.n, buf.counts, fr.depth, d_attr,
+                               fr.channels, fr.qstep, None, w2, q2, c2)
+    torch.cuda.synchronize()
+    assert torch.equal(w2[:nv], buf.weights[:nv])
+    assert torch.equal(c1[:nv], c2[:nv])            # bit for bit
+    assert torch.equal(q1[:nv], q2[:nv])
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    check_quantised(q2[:nv].cpu().numpy(), ref["qcoeff"])
+
+
 def test_corrupt_stream_is_flagged(B, ctx_small):
     fr = synth.make_frame(1, n_override=3000)
     ref = orc.position_encode(fr.xyz, fr.bbox_min, fr.bbox_max, fr.depth)
