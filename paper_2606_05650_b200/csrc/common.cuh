@@ -44,6 +44,7 @@ struct RahtPlan {
   uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
   unsigned long long t_sched[kRahtMaxPhases + 2];  // globaltimer (ns) at the end of each phase, CTA 0 (diagnostics)
   unsigned long long t_xform[kRahtMaxPhases + 2];
+  unsigned long long t_dec[kRahtMaxPhases + 2];    // octree decode: after scan reduce, after down-sweep, after each level step
 };
 
 struct ProfRec {
@@ -231,11 +232,5 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
              int32_t* d_out_q, float* d_out_f, const uint32_t* d_perm = nullptr, const uint32_t* d_vstart = nullptr,
              uint32_t* d_weights_out = nullptr);
 int raht_setup(gsnfs_ctx* ctx);   // occupancy queries + attributes, called from gsnfs_create
-
-// generic exclusive scan of uint32 (weights) with the element count read on the device
-int run_scan_u32(gsnfs_ctx* ctx, cudaStream_t st, const uint32_t* d_in, uint32_t* d_out /* n+1 */,
-                 uint32_t n_cap, const uint32_t* d_n /* may be NULL => n_cap */);
-// exclusive scan of popcount(byte)
-int run_scan_popc8(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_in, uint32_t* d_out /* n+1 */, uint32_t n);
 
 }  // namespace gsnfs
