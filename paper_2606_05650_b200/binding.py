@@ -185,13 +185,13 @@ class Context:
 
     def read_raht_plan(self):
         """Diagnostics: phase sizes and per-phase timestamps of the last RAHT call (synchronises)."""
-        raw = np.zeros(2 + 3 * 32 + 3 * 2 * 32, dtype=np.uint32)
+        raw = np.zeros(2 + 3 * 32 + 4 * 2 * 32, dtype=np.uint32)
         self._check(lib().gsnfs_debug_read_plan(self.handle, raw.ctypes.data_as(c_void_p), raw.nbytes), "read_plan")
         nph = int(raw[0])
         t = raw[2 + 96:].view(np.uint64)
         return {"nphases": nph, "overflow": int(raw[1]), "M": raw[2:34][:nph + 2].tolist(),
                 "t_sched_ns": t[:32][:nph + 1].tolist(), "t_xform_ns": t[32:64][:nph + 2].tolist(),
-                "t_dec_ns": t[64:96].tolist()}
+                "t_dec_ns": t[64:96].tolist(), "t_sort_ns": t[96:128].tolist()}
 
     def profile_start(self, max_records: int = 4096):
         self._check(lib().gsnfs_profile_start(self.handle, int(max_records)), "gsnfs_profile_start")

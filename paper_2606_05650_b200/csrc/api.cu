@@ -73,9 +73,10 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_keys_a = b.take(N * 8), o_keys_b = b.take(N * 8);
   const size_t o_pay_a = b.take(N * 4), o_pay_b = b.take(N * 4);
   const size_t o_hist = b.take((size_t)kSortMaxPasses * 256 * 4);
-  const size_t o_status = b.take((size_t)kSortMaxPasses * stiles * 256 * 4);
-  const size_t o_ticket = b.take((size_t)kSortMaxPasses * 4);
+  c->sort_groups_cap = (uint32_t)(stiles / 32 + 2);
+  const size_t o_sgrp = b.take((size_t)2 * c->sort_groups_cap * 256 * 4);
   const size_t o_zero_end = b.off;
+  const size_t o_sth = b.take((size_t)stiles * 256 * 4);
   const size_t o_ohist = b.take((size_t)kOctLevels * otiles * 4), o_obase = b.take((size_t)kOctLevels * otiles * 4);
   const size_t o_ometa = b.take((size_t)2 * kOctLevels * 4);
   const size_t o_ssums = b.take((size_t)c->scan_tiles_cap * 4);
@@ -95,8 +96,7 @@ static int create_impl(gsnfs_ctx* c) {
   char* p = c->pool;
   c->keys_a = p + o_keys_a; c->keys_b = p + o_keys_b;
   c->pay_a = (uint32_t*)(p + o_pay_a); c->pay_b = (uint32_t*)(p + o_pay_b);
-  c->hist = (uint32_t*)(p + o_hist); c->sort_status = (uint32_t*)(p + o_status);
-  c->sort_ticket = (uint32_t*)(p + o_ticket);
+  c->hist = (uint32_t*)(p + o_hist); c->sort_group_hist = (uint32_t*)(p + o_sgrp); c->sort_tile_hist = (uint32_t*)(p + o_sth);
   c->sort_zero_bytes = o_zero_end - o_hist;
   c->oct_hist = (uint32_t*)(p + o_ohist); c->oct_base = (uint32_t*)(p + o_obase); c->oct_meta = (uint32_t*)(p + o_ometa);
   c->scan_sums = (uint32_t*)(p + o_ssums);

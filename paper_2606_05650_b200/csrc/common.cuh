@@ -44,7 +44,8 @@ struct RahtPlan {
   uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
   unsigned long long t_sched[kRahtMaxPhases + 2];  // globaltimer (ns) at the end of each phase, CTA 0 (diagnostics)
   unsigned long long t_xform[kRahtMaxPhases + 2];
-  unsigned long long t_dec[kRahtMaxPhases + 2];    // octree decode: after scan reduce, after down-sweep, after each level step
+  unsigned long long t_dec[kRahtMaxPhases + 2];
+  unsigned long long t_sort[kRahtMaxPhases + 2];   // radix sort: start, then after phase A / barrier / phase B of each pass    // octree decode: after scan reduce, after down-sweep, after each level step
 };
 
 struct ProfRec {
@@ -78,9 +79,10 @@ struct gsnfs_ctx {
   uint32_t* pay_a;
   uint32_t* pay_b;
   uint32_t* hist;          // kSortMaxPasses x 256
-  uint32_t* sort_status;   // kSortMaxPasses x tiles x 256
-  uint32_t* sort_ticket;   // kSortMaxPasses
-  size_t sort_zero_bytes;  // hist..ticket are contiguous; cleared by one memset
+  uint32_t* sort_group_hist;  // 2 x sort_groups_cap x 256 (digit counts summed per 32 tiles, double buffered by pass parity)
+  uint32_t sort_groups_cap;
+  uint32_t* sort_tile_hist;   // tiles x 256
+  size_t sort_zero_bytes;     // hist + sort_group_hist are contiguous; cleared by one memset
   uint32_t* oct_hist;      // kOctLevels x oct_tiles (level-major)
   uint32_t* oct_base;      // kOctLevels x oct_tiles
   uint32_t* oct_meta;      // level sizes [kOctLevels] + level offsets [kOctLevels]

@@ -7,7 +7,11 @@
 // entry i starts a new node at every depth d >= J - floor(h_i / 3) (and at no depth if it is a duplicate),
 // so |L_d|, the index of every node inside its level and each parent's occupancy bits all follow from
 // per-level prefix counts of those flags.  The bytes produced are exactly Alg. A.1's.
+#include <cooperative_groups.h>
+
 #include "common.cuh"
+
+namespace cg = cooperative_groups;
 
 namespace gsnfs {
 
@@ -66,132 +70,172 @@ __global__ void __launch_bounds__(256) voxelize_kernel(const float* __restrict__
 }
 
 // ------------------------------------------------------------------------------------------------
-// K3: one onesweep pass (stable LSD radix sort, 8-bit digits): warp-level match_any ranking into
-// shared-memory warp histograms, per-digit decoupled look-back across tiles for the global offsets,
-// shared-memory staged scatter so that global writes are coalesced per digit run.
+// K3: stable LSD radix sort of (code, original index), 8-bit digits, ALL passes in one persistent
+// cooperative kernel.  Per pass and tile (4096 keys): warp-level match_any ranking into shared-memory warp
+// histograms (onesweep-style), the tile's digit counts are published and added into a per-32-tiles group
+// sum, one grid barrier, then every tile gets its global digit offsets from <= 32 + ngroups independent
+// loads (no serial look-back chain: at ~1M keys all tiles are co-resident and would all wait on each other),
+// shared-memory staged scatter so that global writes are coalesced per digit run, grid barrier, next pass.
+// When every CTA owns a single tile the keys, payloads and ranks stay in registers across the barrier.
 // ------------------------------------------------------------------------------------------------
-constexpr uint32_t kFlagAgg = 1u << 30, kFlagInc = 2u << 30, kValMask = (1u << 30) - 1u;
+constexpr int kSortGroup = 32;     // tiles per histogram group
 
 template <typename KeyT>
-__global__ void __launch_bounds__(kSortThreads) onesweep_kernel(
-    const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ pay_in, KeyT* __restrict__ keys_out,
-    uint32_t* __restrict__ pay_out, uint32_t n, int shift, int bits, const uint32_t* __restrict__ ghist,
-    uint32_t* status, uint32_t* ticket) {
-  constexpr int WARPS = kSortThreads / 32;
-  extern __shared__ __align__(16) unsigned char s_dyn[];
-  KeyT* s_keys = reinterpret_cast<KeyT*>(s_dyn);
-  uint32_t* s_pay = reinterpret_cast<uint32_t*>(s_dyn + sizeof(KeyT) * kSortTile);
-  __shared__ uint32_t s_whist[WARPS][257];
-  __shared__ uint32_t s_dstart[256];
-  __shared__ uint32_t s_goff[256];
-  __shared__ uint32_t s_scan[9];
-  __shared__ uint32_t s_tile;
-
+__device__ __forceinline__ void sort_load_rank(const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ pay_in,
+                                               uint32_t n, uint32_t base, int shift, uint32_t mask, bool want_pay,
+                                               KeyT (&key)[kSortItems], uint32_t (&pay)[kSortItems],
+                                               uint32_t (&rank)[kSortItems], uint32_t (*s_whist)[257]) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  if (tid == 0) s_tile = atomicAdd(ticket, 1u);
-  for (int i = tid; i < WARPS * 257; i += kSortThreads) (&s_whist[0][0])[i] = 0;
-  __syncthreads();
-  const uint32_t tile = s_tile;
-  const uint32_t base = tile * (uint32_t)kSortTile;
-  const uint32_t mask = (1u << bits) - 1u;
-
-  KeyT key[kSortItems];
-  uint32_t pay[kSortItems];
-  uint32_t rank[kSortItems];
+  for (int i = tid; i < 8 * 257; i += kSortThreads) (&s_whist[0][0])[i] = 0;
   const uint32_t wbase = base + warp * (kSortItems * 32) + lane;
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
     const uint32_t idx = wbase + j * 32;
     const bool valid = idx < n;
-    key[j] = valid ? keys_in[idx] : (KeyT)~(KeyT)0;
-    pay[j] = valid ? (pay_in ? pay_in[idx] : idx) : 0xffffffffu;
+    key[j] = valid ? __ldcg(keys_in + idx) : (KeyT) ~(KeyT)0;
+    if (want_pay) pay[j] = valid ? (pay_in ? __ldcg(pay_in + idx) : idx) : 0xffffffffu;
   }
-  // global digit base for this pass (exclusive scan of the pass histogram)
-  uint32_t gbase = block_excl_scan_256(ghist[tid], s_scan, nullptr);
-
-  // all match rounds first (independent, so their latencies overlap), then the ordered counter updates
+  __syncthreads();
+  // lanes holding the same digit, found with one ballot per digit bit (9 bits: bit 8 marks tail padding):
+  // a fixed ~27 instructions per key, where the hardware match.any serialises over the distinct values
   unsigned peers[kSortItems];
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
     const bool valid = (wbase + j * 32) < n;
     const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
-    peers[j] = __match_any_sync(0xffffffffu, d);
+    unsigned m = 0xffffffffu;
+#pragma unroll
+    for (int b = 0; b < 9; ++b) {
+      const bool bit = (d >> b) & 1u;
+      const unsigned v = __ballot_sync(0xffffffffu, bit);
+      m &= bit ? v : ~v;
+    }
+    peers[j] = m;
   }
+  // per-warp digit counters: the leader of every peer group adds the group size (shared-memory atomics of
+  // one warp execute in program order, so earlier items get the lower ranks) and broadcasts the old value
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
     const bool valid = (wbase + j * 32) < n;
     const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
     const unsigned lt = peers[j] & lanemask_lt();
-    const uint32_t prev = s_whist[warp][d];
-    __syncwarp();
-    if (lt == 0) s_whist[warp][d] = prev + __popc(peers[j]);
-    __syncwarp();
+    uint32_t prev = 0;
+    if (lt == 0) prev = atomicAdd(&s_whist[warp][d], (uint32_t)__popc(peers[j]));
+    prev = __shfl_sync(0xffffffffu, prev, __ffs(peers[j]) - 1);
     rank[j] = prev + __popc(lt);
   }
   __syncthreads();
+}
 
-  // thread d: exclusive prefix over warps of digit d, tile count of digit d
-  uint32_t count = 0;
+template <typename KeyT>
+__global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT* kb, uint32_t* pa, uint32_t* pb,
+                                                                 uint32_t* perm_out, uint32_t n, SortPlan plan,
+                                                                 const uint32_t* __restrict__ ghist, uint32_t* tile_hist,
+                                                                 uint32_t* group_hist, uint32_t ngroups_cap,
+                                                                 unsigned long long* __restrict__ tstamp) {
+  cg::grid_group grid = cg::this_grid();
+  int ts = 0;
+#define GSNFS_SSTAMP() do { if (blockIdx.x == 0 && threadIdx.x == 0 && ts < kRahtMaxPhases + 2) tstamp[ts] = globaltimer_ns(); ++ts; } while (0)
+  GSNFS_SSTAMP();
+  extern __shared__ __align__(16) unsigned char s_dyn[];
+  KeyT* s_keys = reinterpret_cast<KeyT*>(s_dyn);
+  uint32_t* s_pay = reinterpret_cast<uint32_t*>(s_dyn + sizeof(KeyT) * kSortTile);
+  __shared__ uint32_t s_whist[8][257];
+  __shared__ uint32_t s_dstart[256];
+  __shared__ uint32_t s_goff[256];
+  __shared__ uint32_t s_scan[9];
+  __shared__ uint32_t s_gbase[kSortMaxPasses][256];   // exclusive scan of every pass's global digit histogram
+
+  const int tid = threadIdx.x, warp = tid >> 5;
+  const uint32_t ntiles = (n + kSortTile - 1) / kSortTile;
+  const uint32_t ngroups = (ntiles + kSortGroup - 1) / kSortGroup;
+  const bool single = ntiles <= gridDim.x;          // one tile per CTA: registers survive the barrier
+  KeyT key[kSortItems];
+  uint32_t pay[kSortItems];
+  uint32_t rank[kSortItems];
+
+  {
+    uint32_t h[kSortMaxPasses];
 #pragma unroll
-  for (int w = 0; w < WARPS; ++w) {
-    const uint32_t c = s_whist[w][tid];
-    s_whist[w][tid] = count;
-    count += c;
+    for (int p = 0; p < kSortMaxPasses; ++p) h[p] = p < plan.passes ? ghist[p * 256 + tid] : 0u;
+#pragma unroll
+    for (int p = 0; p < kSortMaxPasses; ++p)
+      if (p < plan.passes) s_gbase[p][tid] = block_excl_scan_256(h[p], s_scan, nullptr);
   }
-  // publish the aggregate early, then resolve the exclusive prefix by look-back
-  uint32_t* my_status = status + (size_t)tile * 256 + tid;
-  if (tile == 0) {
-    st_volatile_u32(my_status, kFlagInc | count);
-  } else {
-    st_volatile_u32(my_status, kFlagAgg | count);
-  }
-  const uint32_t dstart = block_excl_scan_256(count, s_scan, nullptr);
-  uint32_t excl = 0;
-  if (tile > 0) {
-    // decoupled look-back, kLookBatch predecessors per round trip (their loads are independent)
-    constexpr int kLookBatch = 8;
-    int t = (int)tile - 1;
-    bool done = false;
-    while (!done) {
-      uint32_t sv[kLookBatch];
+  for (int p = 0; p < plan.passes; ++p) {
+    const KeyT* kin = (p & 1) ? kb : ka;
+    KeyT* kout = (p & 1) ? ka : kb;
+    const uint32_t* pin = (p == 0) ? nullptr : ((p & 1) ? pb : pa);
+    uint32_t* pout = (p == plan.passes - 1) ? perm_out : ((p & 1) ? pa : pb);
+    const int shift = plan.shift[p];
+    const uint32_t mask = (1u << plan.bits[p]) - 1u;
+    uint32_t* gh = group_hist + (size_t)(p & 1) * ngroups_cap * 256;
+    uint32_t* gh_next = group_hist + (size_t)((p + 1) & 1) * ngroups_cap * 256;
+
+    // ---- phase A: digit counts of every tile -> tile_hist, group sums
+    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      sort_load_rank<KeyT>(kin, pin, n, tile * (uint32_t)kSortTile, shift, mask, single, key, pay, rank, s_whist);
+      uint32_t count = 0;
 #pragma unroll
-      for (int b = 0; b < kLookBatch; ++b)
-        sv[b] = (t - b >= 0) ? ld_volatile_u32(status + (size_t)(t - b) * 256 + tid) : (kFlagInc | 0u);
+      for (int w = 0; w < 8; ++w) count += s_whist[w][tid];
+      tile_hist[(size_t)tile * 256 + tid] = count;
+      if (count) atomicAdd(&gh[(size_t)(tile / kSortGroup) * 256 + tid], count);
+      __syncthreads();
+    }
+    GSNFS_SSTAMP();
+    grid.sync();
+    GSNFS_SSTAMP();
+    // the other parity's group sums are free now: clear them for the next pass
+    for (uint32_t i = blockIdx.x * kSortThreads + tid; i < ngroups * 256; i += gridDim.x * kSortThreads) gh_next[i] = 0;
+
+    // ---- phase B: global offsets, scatter
+    const uint32_t gbase = s_gbase[p][tid];
+    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
+      const uint32_t base = tile * (uint32_t)kSortTile;
+      if (!single) sort_load_rank<KeyT>(kin, pin, n, base, shift, mask, true, key, pay, rank, s_whist);
+      // thread d: exclusive prefix over warps of digit d; tile count of digit d
+      uint32_t count = 0;
 #pragma unroll
-      for (int b = 0; b < kLookBatch; ++b) {
-        if (!done) {
-          uint32_t s = sv[b];
-          while ((s & ~kValMask) == 0u) s = ld_volatile_u32(status + (size_t)(t - b) * 256 + tid);
-          excl += s & kValMask;
-          if (s & kFlagInc) done = true;
+      for (int w = 0; w < 8; ++w) {
+        const uint32_t c = s_whist[w][tid];
+        s_whist[w][tid] = count;
+        count += c;
+      }
+      // digit-d keys in earlier tiles: whole groups from the group sums, the rest of this group tile by tile
+      uint32_t excl = 0;
+      const uint32_t g = tile / kSortGroup;
+#pragma unroll 8
+      for (uint32_t gg = 0; gg < g; ++gg) excl += __ldcg(gh + (size_t)gg * 256 + tid);
+#pragma unroll 8
+      for (uint32_t t = g * kSortGroup; t < tile; ++t) excl += __ldcg(tile_hist + (size_t)t * 256 + tid);
+      const uint32_t dstart = block_excl_scan_256(count, s_scan, nullptr);
+      s_dstart[tid] = dstart;
+      s_goff[tid] = gbase + excl - dstart;      // global position = s_goff[d] + tile-local sorted position
+      __syncthreads();
+      const uint32_t wbase = base + warp * (kSortItems * 32) + (tid & 31);
+#pragma unroll
+      for (int j = 0; j < kSortItems; ++j) {
+        if (wbase + j * 32 < n) {
+          const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
+          const uint32_t pos = s_dstart[d] + s_whist[warp][d] + rank[j];
+          s_keys[pos] = key[j];
+          s_pay[pos] = pay[j];
         }
       }
-      t -= kLookBatch;
+      __syncthreads();
+      const uint32_t cnt = min((uint32_t)kSortTile, n - base);
+      for (uint32_t i = tid; i < cnt; i += kSortThreads) {
+        const KeyT k = s_keys[i];
+        const uint32_t d = (uint32_t)(k >> shift) & mask;
+        const uint32_t o = s_goff[d] + i;
+        kout[o] = k;
+        pout[o] = s_pay[i];
+      }
+      __syncthreads();
     }
-    st_volatile_u32(my_status, kFlagInc | (excl + count));
-  }
-  s_dstart[tid] = dstart;
-  s_goff[tid] = gbase + excl - dstart;      // global position = s_goff[d] + tile-local sorted position
-  __syncthreads();
-
-#pragma unroll
-  for (int j = 0; j < kSortItems; ++j) {
-    const bool valid = (wbase + j * 32) < n;
-    if (valid) {
-      const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
-      const uint32_t pos = s_dstart[d] + s_whist[warp][d] + rank[j];
-      s_keys[pos] = key[j];
-      s_pay[pos] = pay[j];
-    }
-  }
-  __syncthreads();
-  const uint32_t cnt = min((uint32_t)kSortTile, n - base);
-  for (uint32_t i = tid; i < cnt; i += kSortThreads) {
-    const KeyT k = s_keys[i];
-    const uint32_t d = (uint32_t)(k >> shift) & mask;
-    const uint32_t o = s_goff[d] + i;
-    keys_out[o] = k;
-    pay_out[o] = s_pay[i];
+    GSNFS_SSTAMP();
+    if (p + 1 < plan.passes) grid.sync();
+    GSNFS_SSTAMP();
   }
 }
 
@@ -420,23 +464,30 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
     voxelize_kernel<KeyT><<<vgrid, 256, 0, st>>>(d_xyz, n, vp, plan, ka, ctx->hist);
     GSNFS_LAUNCH_CHECK(ctx, st);
     const size_t smem = (sizeof(KeyT) + 4) * (size_t)kSortTile;
-    const uint32_t status_stride = (uint32_t)((ctx->max_points + kSortTile - 1) / kSortTile) * 256;
-    const KeyT* kin = ka;
-    KeyT* kout = kb;
-    const uint32_t* pin = nullptr;
-    for (int p = 0; p < plan.passes; ++p) {
-      uint32_t* pout = (p == plan.passes - 1) ? d_perm : ((p & 1) ? ctx->pay_b : ctx->pay_a);
-      GSNFS_KERNEL(ctx, st, "onesweep_pass");
-      onesweep_kernel<KeyT><<<stiles, kSortThreads, smem, st>>>(
-          kin, pin, kout, pout, n, plan.shift[p], plan.bits[p], ctx->hist + p * 256,
-          ctx->sort_status + (size_t)p * status_stride, ctx->sort_ticket + p);
+    {
+      int per_sm = 0;
+      GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sort_coop_kernel<KeyT>, kSortThreads, smem));
+      if (per_sm < 1) { snprintf(ctx->err, sizeof(ctx->err), "sort kernel does not fit on an SM"); return GSNFS_E_CUDA; }
+      uint32_t grid = (uint32_t)per_sm * (uint32_t)ctx->num_sms;
+      if (grid > stiles) grid = stiles;
+      KeyT* kbuf_a = ka;
+      KeyT* kbuf_b = kb;
+      uint32_t* pbuf_a = ctx->pay_a;
+      uint32_t* pbuf_b = ctx->pay_b;
+      uint32_t nn = n;
+      SortPlan pl = plan;
+      const uint32_t* gh = ctx->hist;
+      uint32_t* th = ctx->sort_tile_hist;
+      uint32_t* grp = ctx->sort_group_hist;
+      uint32_t gcap = ctx->sort_groups_cap;
+      unsigned long long* tstamp = ctx->raht_plan->t_sort;
+      void* args[] = {(void*)&kbuf_a, (void*)&kbuf_b, (void*)&pbuf_a, (void*)&pbuf_b, (void*)&d_perm, (void*)&nn, (void*)&pl,
+                      (void*)&gh, (void*)&th, (void*)&grp, (void*)&gcap, (void*)&tstamp};
+      GSNFS_KERNEL(ctx, st, "radix_sort");
+      GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)sort_coop_kernel<KeyT>, dim3(grid), dim3(kSortThreads), args, smem, st));
       GSNFS_LAUNCH_CHECK(ctx, st);
-      pin = pout;
-      const KeyT* t = kin;
-      kin = kout;
-      kout = const_cast<KeyT*>(t);
     }
-    const KeyT* sorted = kin;
+    const KeyT* sorted = (plan.passes & 1) ? kb : ka;
     const uint32_t otiles = (n + kOctTile - 1) / kOctTile;
     GSNFS_KERNEL(ctx, st, "octree_count");
     octree_count_kernel<KeyT><<<otiles, 256, 0, st>>>(sorted, n, depth, otiles, ctx->oct_hist);
@@ -459,9 +510,9 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
 }
 
 int octree_encode_setup(gsnfs_ctx* ctx) {
-  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(onesweep_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(sort_coop_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)((8 + 4) * kSortTile)));
-  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(onesweep_kernel<uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(sort_coop_kernel<uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)((4 + 4) * kSortTile)));
   const int esmem = GSNFS_MAX_DEPTH * (kOctTile + 4);
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(octree_emit_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, esmem));

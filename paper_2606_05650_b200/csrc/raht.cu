@@ -38,6 +38,13 @@ __device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) 
   const unsigned s = (unsigned)__cvta_generic_to_shared(smem_dst);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(s), "l"(gmem_src) : "memory");
 }
+__device__ __forceinline__ void prefetch_l2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+// pull one C-float row (not necessarily line aligned) into L2
+__device__ __forceinline__ void prefetch_row_l2(const float* row, int C) {
+  const char* b = reinterpret_cast<const char*>(row);
+  const char* e = b + (size_t)C * 4 - 1;
+  for (const char* q = (const char*)((uintptr_t)b & ~(uintptr_t)127); q <= e; q += 128) prefetch_l2(q);
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
@@ -614,6 +621,17 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
         }
         __syncthreads();
         sj = ej;
+      }
+      if (tnext < ntiles) {          // next tile's input rows -> L2 while this tile is written out
+        const uint32_t ksn = tnext * T;
+        if ((uint32_t)tid < min((uint32_t)T, M - ksn)) {
+          if (gsrc) {
+            cp_async_wait_all();       // this thread's own piece of meta(next) (its g entry) has landed
+            prefetch_row_l2(src + (size_t)s_meta[cur ^ 1].g[tid] * C, C);
+          } else {
+            prefetch_row_l2(src + (size_t)(ksn + tid) * C, C);
+          }
+        }
       }
       // rows out, in natural order: finished high-pass -> canonical output row (quantised); pending
       // low-pass -> next phase's row pool, or -- when a single node is left -- the DC at output row 0
