@@ -113,7 +113,7 @@ def algorithmic_bytes(n, nv, s_occ, channels, depth):
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
-    from paper_2606_05650_b200 import binding as B, synth
+    from paper_2606_05650_b200 import binding as B, dist as gdist, synth
 
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
@@ -158,10 +158,7 @@ def run_ours(args, rank, world, local_rank):
     ms_total = e0.elapsed_time(e1)
     launches = ctx.launch_count() - l0
     clocks = sampler.stop()
-    if world > 1:
-        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    ms_total = gdist.max_over_ranks(ms_total, dev)          # replicas: the job is as slow as its slowest rank
     ms_step = ms_total / args.steps
     value = world * n / (ms_step * 1e-3) / 1e6
 
@@ -231,11 +228,7 @@ def run_ours(args, rank, world, local_rank):
         e1.record(stream)
         barrier()
         ms_e = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms_e], dtype=torch.float64, device=dev)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e = float(t.item())
-        ms_e /= ks
+        ms_e = gdist.max_over_ranks(ms_e, dev) / ks
         nv_e = int(h_cnt[0])
         h2d = n * 12 + n * C * 4 + int(h_cnt[1]) + nv_e * 4 + nv_e * C * 4
         d2h = 16 + 4 * (J + 1) + int(h_cnt[1]) + nv_e * 4 + nv_e * C * 4 + 16 + nv_e * 12 + nv_e * C * 4
@@ -317,7 +310,7 @@ def run_reference(args, rank, world):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); 3 = headline 1M frame")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
