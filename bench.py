@@ -126,12 +126,19 @@ def run_ours(args, rank, world, local_rank):
     h_hdr = torch.empty(J + 1 + 4, dtype=torch.int32).pin_memory()
     stream = torch.cuda.current_stream()
 
+    hdr_ready = torch.cuda.Event()
+
     def step():
-        B.encode_frame(ctx, buf, d_xyz, d_attr, fr.bbox_min, fr.bbox_max, fr.qstep)
-        # the decoder needs the stream header (level sizes) on the host: read it back like a receiver would
+        B.gsnfs_octree_encode(ctx, d_xyz, n, fr.bbox_min, fr.bbox_max, J, buf.occ, buf.level_sizes, buf.perm,
+                              buf.voxel_keys, buf.voxel_start, buf.counts)
+        # the decoder needs the stream header (level sizes) on the host, like a receiver would: copy it out as soon
+        # as the position coder is done, so the host can enqueue the decode while the GPU runs the attribute coder
         h_hdr[:J + 1].copy_(buf.level_sizes, non_blocking=True)
         h_hdr[J + 1:].copy_(buf.counts, non_blocking=True)
-        stream.synchronize()
+        hdr_ready.record(stream)
+        B.gsnfs_merge_raht_forward(ctx, buf.voxel_keys, buf.perm, buf.voxel_start, n, buf.counts, J, d_attr, C,
+                                   fr.qstep, None, buf.weights, buf.qcoeff, None)
+        hdr_ready.synchronize()
         levels = h_hdr[:J + 1].numpy()
         B.decode_frame(ctx, buf, levels, int(h_hdr[J + 2]), fr.qstep)
 

@@ -107,7 +107,8 @@ struct gsnfs_ctx {
   uint64_t raht_rec_cap;
   uint64_t raht_hdr_cap;
   float* qparams;          // 2 x max_channels doubles (inv step / step) stored as double
-  int raht_grid_sched, raht_grid_fwd, raht_grid_inv;
+  int occ_cache[16];       // cached cudaOccupancyMaxActiveBlocksPerMultiprocessor results (0 = not yet queried)
+  size_t occ_cache_smem[16];
 
   // decode
   uint32_t* dec_scan;      // exclusive popcount scan over the stream (one per byte)

@@ -284,8 +284,11 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
   }
   const uint32_t S = (uint32_t)occ_bytes;
   if (S / kScanTile + 2 > ctx->scan_tiles_cap) return GSNFS_E_CAPACITY;
-  int per_sm = 0;
-  GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, octree_decode_kernel, 256, 0));
+  int per_sm = ctx->occ_cache[7];
+  if (per_sm == 0) {
+    GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, octree_decode_kernel, 256, 0));
+    ctx->occ_cache[7] = per_sm;
+  }
   if (per_sm < 1) return GSNFS_E_CUDA;
   if (per_sm > 8) per_sm = 8;
   const uint32_t want = (nv + 255) / 256;

@@ -270,7 +270,8 @@ __global__ void __launch_bounds__(256) octree_count_kernel(const KeyT* __restric
   for (int it = 0; it < 8; ++it) {
     uint64_t k;
     const int t = start_levels(keys, base + it * 32 + lane, n, J, &k);
-    for (int d = 0; d <= J; ++d) {
+    const int tmax = __reduce_max_sync(0xffffffffu, t);          // no lane starts a node above depth J + 1 - tmax
+    for (int d = max(0, J + 1 - tmax); d <= J; ++d) {
       const unsigned b = __ballot_sync(0xffffffffu, t >= J - d + 1);
       if (lane == d) mine += __popc(b);
     }
@@ -363,7 +364,8 @@ __global__ void __launch_bounds__(256) octree_emit_kernel(const KeyT* __restrict
 #pragma unroll
   for (int it = 0; it < 8; ++it) {
     tt[it] = start_levels(keys, base + it * 32 + lane, n, J, &kk[it]);
-    for (int d = 0; d <= J; ++d) {
+    const int tmax = __reduce_max_sync(0xffffffffu, tt[it]);
+    for (int d = max(0, J + 1 - tmax); d <= J; ++d) {
       const unsigned b = __ballot_sync(0xffffffffu, tt[it] >= J - d + 1);
       if (lane == d) mine += __popc(b);
     }
@@ -383,8 +385,10 @@ __global__ void __launch_bounds__(256) octree_emit_kernel(const KeyT* __restrict
     const uint32_t i = base + it * 32 + lane;
     const int t = tt[it];
     const uint64_t k = kk[it];
-    uint32_t prev_incl = 0;            // tile-local inclusive rank at depth d-1
-    for (int d = 0; d <= J; ++d) {
+    const int tmax = __reduce_max_sync(0xffffffffu, t);
+    const int dmin = max(0, J + 1 - tmax);                       // shallower depths: no lane starts a node
+    uint32_t prev_incl = dmin > 0 ? __shfl_sync(0xffffffffu, run, dmin - 1) : 0u;   // tile-local inclusive rank at depth d-1
+    for (int d = dmin; d <= J; ++d) {
       const bool f = t >= J - d + 1;
       const unsigned b = __ballot_sync(0xffffffffu, f);
       const uint32_t run_d = __shfl_sync(0xffffffffu, run, d);
@@ -465,8 +469,12 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
     GSNFS_LAUNCH_CHECK(ctx, st);
     const size_t smem = (sizeof(KeyT) + 4) * (size_t)kSortTile;
     {
-      int per_sm = 0;
-      GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sort_coop_kernel<KeyT>, kSortThreads, smem));
+      const int slot = sizeof(KeyT) == 8 ? 5 : 6;
+      int per_sm = ctx->occ_cache[slot];
+      if (per_sm == 0) {
+        GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, sort_coop_kernel<KeyT>, kSortThreads, smem));
+        ctx->occ_cache[slot] = per_sm;
+      }
       if (per_sm < 1) { snprintf(ctx->err, sizeof(ctx->err), "sort kernel does not fit on an SM"); return GSNFS_E_CUDA; }
       uint32_t grid = (uint32_t)per_sm * (uint32_t)ctx->num_sms;
       if (grid > stiles) grid = stiles;

@@ -833,9 +833,13 @@ int raht_setup(gsnfs_ctx* ctx) {
 }
 
 template <typename K>
-static int coop_grid(gsnfs_ctx* ctx, K kernel, size_t smem, uint32_t want, int* out) {
-  int per_sm = 0;
-  GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, 256, smem));
+static int coop_grid(gsnfs_ctx* ctx, int slot, K kernel, size_t smem, uint32_t want, int* out) {
+  int per_sm = ctx->occ_cache[slot];
+  if (per_sm == 0 || ctx->occ_cache_smem[slot] != smem) {
+    GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, 256, smem));
+    ctx->occ_cache[slot] = per_sm;
+    ctx->occ_cache_smem[slot] = smem;
+  }
   if (per_sm < 1) { snprintf(ctx->err, sizeof(ctx->err), "raht kernel does not fit on an SM"); return GSNFS_E_CUDA; }
   const uint32_t cap = (uint32_t)per_sm * (uint32_t)ctx->num_sms;
   *out = (int)max(1u, min(cap, want));
@@ -862,7 +866,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
   {
     int grid = 0;
-    int rc = coop_grid(ctx, raht_schedule_kernel, 0, want, &grid);
+    int rc = coop_grid(ctx, 0, raht_schedule_kernel, 0, want, &grid);
     if (rc != GSNFS_OK) return rc;
     void* args[] = {(void*)&d_keys, (void*)&d_weights, (void*)&n_voxels, (void*)&n_dev, (void*)&sp, (void*)&ctx->raht_plan};
     GSNFS_KERNEL(ctx, st, "raht_schedule");
@@ -882,7 +886,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
                     (void*)&ctx->raht_plan, (void*)&channels, (void*)&qs, (void*)&has_q, (void*)&dz,
                     (void*)&d_out_q, (void*)&d_out_f};
     void* fn = vec4 ? (void*)raht_forward_kernel<4> : (void*)raht_forward_kernel<1>;
-    int rc = vec4 ? coop_grid(ctx, raht_forward_kernel<4>, smem, want, &grid) : coop_grid(ctx, raht_forward_kernel<1>, smem, want, &grid);
+    int rc = vec4 ? coop_grid(ctx, 1, raht_forward_kernel<4>, smem, want, &grid) : coop_grid(ctx, 2, raht_forward_kernel<1>, smem, want, &grid);
     if (rc != GSNFS_OK) return rc;
     GSNFS_KERNEL(ctx, st, "raht_forward");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, st));
@@ -892,7 +896,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
                     (void*)&ctx->raht_hdr, (void*)&ctx->raht_plan, (void*)&channels, (void*)&qs, (void*)&bias,
                     (void*)&d_out_f};
     void* fn = vec4 ? (void*)raht_inverse_kernel<4> : (void*)raht_inverse_kernel<1>;
-    int rc = vec4 ? coop_grid(ctx, raht_inverse_kernel<4>, smem, want, &grid) : coop_grid(ctx, raht_inverse_kernel<1>, smem, want, &grid);
+    int rc = vec4 ? coop_grid(ctx, 3, raht_inverse_kernel<4>, smem, want, &grid) : coop_grid(ctx, 4, raht_inverse_kernel<1>, smem, want, &grid);
     if (rc != GSNFS_OK) return rc;
     GSNFS_KERNEL(ctx, st, "raht_inverse");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, st));
