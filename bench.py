@@ -106,6 +106,7 @@ def algorithmic_bytes(n, nv, s_occ, channels, depth):
         "raht_inverse": c4 * nv + c4 * nv + 16 * nv,
         "scan_reduce": None, "scan_sums": None, "scan_down": None,   # used twice with different inputs
         "expand_children": (s_occ + 4 * s_occ + 8 * (s_occ + nv) + 12 * nv) / max(depth, 1),
+        "radix_sort": k * n + passes * 2 * (k + 4) * n,         # histogram read + P passes of (key, index) in and out
         "_sort_total": k * n + passes * 2 * (k + 4) * n, "_passes": passes,
     }
 
@@ -206,7 +207,7 @@ def run_ours(args, rank, world, local_rank):
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["alg_GBps"], "peak": peak, "unit": "GB/s",
                 "frac": round(kernels[dom]["alg_GBps"] / peak, 4), "traffic": traffic, "peak_source": peak_src,
                 "alg_bytes_per_launch": ab[dom]}
-    sort_ms = kernels.get("onesweep_pass", {}).get("ms_per_step", 0.0)
+    sort_ms = kernels.get("radix_sort", {}).get("ms_per_step", 0.0)
     sort_frac = (ab["_sort_total"] / (sort_ms * 1e-3) / 1e9 / peak) if sort_ms else None
 
     # ---- end to end through the host-buffer ABI calls (pinned host memory, copies inside the timed region)

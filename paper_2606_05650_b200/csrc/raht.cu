@@ -372,11 +372,42 @@ template <int VEC> struct RowVec;
 template <> struct RowVec<4> { using type = float4; };
 template <> struct RowVec<1> { using type = float; };
 
-__device__ __forceinline__ float4 bf_lo(float a, float b, float4 y0, float4 y1) {
-  return make_float4(fmaf(a, y0.x, b * y1.x), fmaf(a, y0.y, b * y1.y), fmaf(a, y0.z, b * y1.z), fmaf(a, y0.w, b * y1.w));
+// packed fp32x2 arithmetic (FFMA2 / FMUL2 / FADD2 on sm_100: one issue slot for two lanes of a float4); every
+// product is rounded once and the sum is an FMA, exactly as the scalar fmaf(a, y0, b * y1) form
+__device__ __forceinline__ uint64_t pk2(float lo, float hi) {
+  uint64_t r;
+  asm("mov.b64 %0, {%1, %2};" : "=l"(r) : "f"(lo), "f"(hi));
+  return r;
 }
-__device__ __forceinline__ float4 bf_hi(float a, float b, float4 y0, float4 y1) {
-  return make_float4(fmaf(a, y1.x, -b * y0.x), fmaf(a, y1.y, -b * y0.y), fmaf(a, y1.z, -b * y0.z), fmaf(a, y1.w, -b * y0.w));
+__device__ __forceinline__ void upk2(uint64_t v, float& lo, float& hi) { asm("mov.b64 {%0, %1}, %2;" : "=f"(lo), "=f"(hi) : "l"(v)); }
+__device__ __forceinline__ uint64_t fma2(uint64_t a, uint64_t b, uint64_t c) {
+  uint64_t r;
+  asm("fma.rn.f32x2 %0, %1, %2, %3;" : "=l"(r) : "l"(a), "l"(b), "l"(c));
+  return r;
+}
+__device__ __forceinline__ uint64_t mul2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("mul.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ uint64_t add2(uint64_t a, uint64_t b) {
+  uint64_t r;
+  asm("add.rn.f32x2 %0, %1, %2;" : "=l"(r) : "l"(a), "l"(b));
+  return r;
+}
+__device__ __forceinline__ float4 bf_lo(float a, float b, float4 y0, float4 y1) {      // a y0 + b y1
+  const uint64_t aa = pk2(a, a), bb = pk2(b, b);
+  float4 r;
+  upk2(fma2(aa, pk2(y0.x, y0.y), mul2(bb, pk2(y1.x, y1.y))), r.x, r.y);
+  upk2(fma2(aa, pk2(y0.z, y0.w), mul2(bb, pk2(y1.z, y1.w))), r.z, r.w);
+  return r;
+}
+__device__ __forceinline__ float4 bf_hi(float a, float b, float4 y0, float4 y1) {      // a y1 - b y0
+  const uint64_t aa = pk2(a, a), nb = pk2(-b, -b);
+  float4 r;
+  upk2(fma2(aa, pk2(y1.x, y1.y), mul2(nb, pk2(y0.x, y0.y))), r.x, r.y);
+  upk2(fma2(aa, pk2(y1.z, y1.w), mul2(nb, pk2(y0.z, y0.w))), r.z, r.w);
+  return r;
 }
 __device__ __forceinline__ float bf_lo(float a, float b, float y0, float y1) { return fmaf(a, y0, b * y1); }
 __device__ __forceinline__ float bf_hi(float a, float b, float y0, float y1) { return fmaf(a, y1, -b * y0); }
@@ -385,28 +416,33 @@ __device__ __forceinline__ float4 vscale(float4 v, double s) {
 }
 __device__ __forceinline__ float vscale(float v, double s) { return (float)((double)v * s); }
 
-// Dead-zone quantiser q = sign(y) floor(|y| / step + f), defined in fp64 on the fp32 coefficient [R10].
-// quant_exact is that definition (|y| * (1/step) in fp64; saturates to int32).  quant_fast evaluates
-// t = |y| * inv32 + f in fp32 and takes floor(t) only when t is provably on the same side of every integer
-// as the fp64 value: |t32 - t64| <= 2.4e-7 t + 1e-7, so a guard band of 4e-7 t + 2e-7 around the integers
-// (and t < 2^22) is enough; otherwise it signals a fallback to quant_exact.  floor uses the 1.5*2^23
-// magic-number trick (no F2I / F2F conversions, which run at 1/8 rate).
+// Dead-zone quantiser [R10].  Definition (both sides of the parity test): q = sign(y) floor(|y| * (1/step) + f),
+// evaluated in fp64 on the fp32 coefficient, saturating to int32 (quant_exact).  quant_fast2 evaluates the
+// signed, half-shifted value t' = y * inv32 + sign(y)(f - 1/2) in fp32 and rounds it to nearest with the
+// 1.5*2^23 magic constant, so that RN(t') = sign(y) floor(|y| inv + f) whenever t' is not within `guard` of a
+// half-integer.  |t'_32 - t'_exact| <= 1.2e-7 |t| + 2e-8 (inv32 rounding, (f - 1/2) rounding, the FMA rounding);
+// the guard 4e-7 |t'| + 4e-7 covers it with margin and |t'| >= 2^20 fails the test by itself.  Outside the guard
+// the caller falls back to quant_exact, so the result always equals the fp64 definition.  Two values per call:
+// the arithmetic is packed fp32x2.
 __device__ __forceinline__ int quant_exact(float y, double inv, double f) {
   double m = floor(fma(fabs((double)y), inv, f));
   m = fmin(m, 2147483647.0);
   const int q = (int)m;
   return y < 0.f ? -q : q;
 }
-__device__ __forceinline__ bool quant_fast(float y, float inv32, float f32, int* q) {
-  const float t = fmaf(fabsf(y), inv32, f32);
-  const float u = t + 12582912.0f;                       // 1.5 * 2^23: integer part lands in the mantissa
-  const float rn = u - 12582912.0f;                      // round-to-nearest(t)
-  const float fl = rn > t ? rn - 1.0f : rn;              // floor(t)
-  const float frac = t - fl;
-  const float guard = fmaf(t, 4e-7f, 2e-7f);
-  const int qi = (__float_as_int(u) - 0x4B400000) - (rn > t ? 1 : 0);
-  *q = y < 0.f ? -qi : qi;
-  return (frac > guard) && (frac < 1.0f - guard) && (t < 4194304.0f);
+__device__ __forceinline__ bool quant_fast2(float y0, float y1, float i0, float i1, float fm, int& q0, int& q1) {
+  const float s0 = __uint_as_float(__float_as_uint(fm) ^ (__float_as_uint(y0) & 0x80000000u));
+  const float s1 = __uint_as_float(__float_as_uint(fm) ^ (__float_as_uint(y1) & 0x80000000u));
+  const uint64_t t = fma2(pk2(y0, y1), pk2(i0, i1), pk2(s0, s1));
+  const uint64_t u = add2(t, pk2(12582912.0f, 12582912.0f));
+  const uint64_t rn = add2(u, pk2(-12582912.0f, -12582912.0f));
+  const uint64_t d = add2(t, rn ^ 0x8000000080000000ull);
+  float t0, t1, u0, u1, d0, d1;
+  upk2(t, t0, t1); upk2(u, u0, u1); upk2(d, d0, d1);
+  q0 = __float_as_int(u0) - 0x4B400000;
+  q1 = __float_as_int(u1) - 0x4B400000;
+  const float lim0 = fmaf(fabsf(t0), -4e-7f, 0.4999996f), lim1 = fmaf(fabsf(t1), -4e-7f, 0.4999996f);
+  return (fabsf(d0) < lim0) && (fabsf(d1) < lim1);
 }
 __device__ __forceinline__ float dequant1(int q, double step, double bias) {
   if (q == 0) return 0.f;
@@ -421,23 +457,21 @@ struct QuantTab {          // per-channel constants in shared memory
   float* inv32;            // (float)(1 / step)   (forward)   |  step32 (inverse)
 };
 
-__device__ __forceinline__ int4 quant4(float4 y, int c4, const QuantTab& qt, double dz, float dz32) {
+__device__ __forceinline__ int4 quant4(float4 y, int c4, const QuantTab& qt, double dz, float fm) {
   int4 q;
   const float4 iv = reinterpret_cast<const float4*>(qt.inv32)[c4];
-  bool ok = quant_fast(y.x, iv.x, dz32, &q.x);
-  ok &= quant_fast(y.y, iv.y, dz32, &q.y);
-  ok &= quant_fast(y.z, iv.z, dz32, &q.z);
-  ok &= quant_fast(y.w, iv.w, dz32, &q.w);
+  bool ok = quant_fast2(y.x, y.y, iv.x, iv.y, fm, q.x, q.y);
+  ok &= quant_fast2(y.z, y.w, iv.z, iv.w, fm, q.z, q.w);
   if (!ok) {
     q.x = quant_exact(y.x, qt.inv64[4 * c4 + 0], dz); q.y = quant_exact(y.y, qt.inv64[4 * c4 + 1], dz);
     q.z = quant_exact(y.z, qt.inv64[4 * c4 + 2], dz); q.w = quant_exact(y.w, qt.inv64[4 * c4 + 3], dz);
   }
   return q;
 }
-__device__ __forceinline__ int quant1s(float y, int c, const QuantTab& qt, double dz, float dz32) {
-  int q;
-  if (!quant_fast(y, qt.inv32[c], dz32, &q)) q = quant_exact(y, qt.inv64[c], dz);
-  return q;
+__device__ __forceinline__ int quant1s(float y, int c, const QuantTab& qt, double dz, float fm) {
+  int q0, q1;
+  if (!quant_fast2(y, 0.f, qt.inv32[c], 0.f, fm, q0, q1)) q0 = quant_exact(y, qt.inv64[c], dz);
+  return q0;
 }
 
 template <int VEC>
@@ -519,7 +553,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
     qt.inv64[c] = iv;
     qt.inv32[c] = (float)iv;
   }
-  const float dz32 = (float)dz;
+  const float dz32 = (float)(dz - 0.5);                                  // the quantiser's half-shifted rounding offset
   const uint32_t cv_magic = make_div_magic((uint32_t)(C / VEC));
   if (!has_q) out_q = nullptr;
   const uint32_t nph = plan->nphases;
@@ -574,7 +608,9 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
         if ((pm >> lane) & 1u) s_dst[tid] = 0x80000000u | (mt->hdr.pend_off + before + __popc(pm & lanemask_lt()));
         if ((uint32_t)tid < nmerge) { const uint4 rr = mt->rec[tid]; s_dst[rr.x & 0xffu] = rr.w; }
       }
-      if (wts) {                                                          // [R2] x_i = sqrt(w_i) a_i
+      // [R2] x_i = sqrt(w_i) a_i: only rows with w != 1 need work (block-uniform test first)
+      bool staged = false;             // a barrier has passed since the rows and s_dst were written
+      if (wts && !(staged = !__syncthreads_or((uint32_t)tid < nent && mt->w[tid] != 1u))) {
         for (uint32_t k = hw; k < nent; k += 16) {
           const uint32_t w = mt->w[k];
           if (w != 1u) {
@@ -603,7 +639,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
           }
         }
       }
-      __syncthreads();
+      if (!staged) __syncthreads();
       uint32_t sj = 0;
       for (uint32_t s = 0; s < nseg; ++s) {                               // non-empty levels, bottom-up
         const uint32_t ej = mt->hdr.lev_end[s];
@@ -792,7 +828,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
         }
         __syncthreads();
       }
-      if (wts) {                                                           // [R2] a_i = x_i / sqrt(w_i)
+      if (wts && __syncthreads_or((uint32_t)tid < nent && mt->w[tid] != 1u)) {   // [R2] a_i = x_i / sqrt(w_i)
         for (uint32_t k = hw; k < nent; k += 16) {
           const uint32_t w = mt->w[k];
           if (w != 1u) {
