@@ -60,7 +60,7 @@ static int create_impl(gsnfs_ctx* c) {
   }
   const uint64_t N = c->max_points;
   const int C = c->max_channels;
-  const uint64_t stiles = (N + kSortTile - 1) / kSortTile + 1;
+  const uint64_t stiles = N / 1024 + 2048;      // sort tiles hold 1024..kSortTile keys (balanced tiling)
   const uint64_t otiles = (N + kOctTile - 1) / kOctTile + 1;
   c->oct_tiles_cap = (uint32_t)otiles;
   c->occ_cap = gsnfs_occ_capacity(N, c->max_depth) + 16;

@@ -80,18 +80,23 @@ __global__ void __launch_bounds__(256) voxelize_kernel(const float* __restrict__
 // ------------------------------------------------------------------------------------------------
 constexpr int kSortGroup = 32;     // tiles per histogram group
 
+// Tile = `cnt` consecutive keys starting at `base`; thread (warp, lane) holds items j < ipt at tile-local
+// position warp * ipt * 32 + j * 32 + lane (ipt * 256 >= tile stride), so positions grow with (warp, j, lane).
 template <typename KeyT>
-__device__ __forceinline__ void sort_load_rank(const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ pay_in,
-                                               uint32_t n, uint32_t base, int shift, uint32_t mask, bool want_pay,
-                                               KeyT (&key)[kSortItems], uint32_t (&pay)[kSortItems],
-                                               uint32_t (&rank)[kSortItems], uint32_t (*s_whist)[257]) {
+__device__ __forceinline__ uint32_t sort_load_rank(const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ pay_in,
+                                                   uint32_t base, uint32_t cnt, int ipt, int shift, uint32_t mask, bool want_pay,
+                                                   KeyT (&key)[kSortItems], uint32_t (&pay)[kSortItems],
+                                                   uint32_t (&rank)[kSortItems], uint32_t (*s_whist)[257]) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int i = tid; i < 8 * 257; i += kSortThreads) (&s_whist[0][0])[i] = 0;
-  const uint32_t wbase = base + warp * (kSortItems * 32) + lane;
+  const uint32_t lbase = (uint32_t)(warp * ipt * 32 + lane);
+  uint32_t vmask = 0;
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
-    const uint32_t idx = wbase + j * 32;
-    const bool valid = idx < n;
+    const uint32_t li = lbase + j * 32;
+    const bool valid = j < ipt && li < cnt;
+    vmask |= (uint32_t)valid << j;
+    const uint32_t idx = base + li;
     key[j] = valid ? __ldcg(keys_in + idx) : (KeyT) ~(KeyT)0;
     if (want_pay) pay[j] = valid ? (pay_in ? __ldcg(pay_in + idx) : idx) : 0xffffffffu;
   }
@@ -101,35 +106,43 @@ __device__ __forceinline__ void sort_load_rank(const KeyT* __restrict__ keys_in,
   unsigned peers[kSortItems];
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
-    const bool valid = (wbase + j * 32) < n;
-    const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
-    unsigned m = 0xffffffffu;
+    if (j < ipt) {                                           // warp-uniform
+      const bool valid = (vmask >> j) & 1u;
+      const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
+      unsigned m = 0xffffffffu;
 #pragma unroll
-    for (int b = 0; b < 9; ++b) {
-      const bool bit = (d >> b) & 1u;
-      const unsigned v = __ballot_sync(0xffffffffu, bit);
-      m &= bit ? v : ~v;
+      for (int b = 0; b < 9; ++b) {
+        const bool bit = (d >> b) & 1u;
+        const unsigned v = __ballot_sync(0xffffffffu, bit);
+        m &= bit ? v : ~v;
+      }
+      peers[j] = m;
+    } else {
+      peers[j] = 0xffffffffu;
     }
-    peers[j] = m;
   }
   // per-warp digit counters: the leader of every peer group adds the group size (shared-memory atomics of
   // one warp execute in program order, so earlier items get the lower ranks) and broadcasts the old value
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
-    const bool valid = (wbase + j * 32) < n;
-    const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
-    const unsigned lt = peers[j] & lanemask_lt();
-    uint32_t prev = 0;
-    if (lt == 0) prev = atomicAdd(&s_whist[warp][d], (uint32_t)__popc(peers[j]));
-    prev = __shfl_sync(0xffffffffu, prev, __ffs(peers[j]) - 1);
-    rank[j] = prev + __popc(lt);
+    if (j < ipt) {
+      const bool valid = (vmask >> j) & 1u;
+      const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
+      const unsigned lt = peers[j] & lanemask_lt();
+      uint32_t prev = 0;
+      if (lt == 0) prev = atomicAdd(&s_whist[warp][d], (uint32_t)__popc(peers[j]));
+      prev = __shfl_sync(0xffffffffu, prev, __ffs(peers[j]) - 1);
+      rank[j] = prev + __popc(lt);
+    }
   }
   __syncthreads();
+  return vmask;
 }
 
 template <typename KeyT>
 __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT* kb, uint32_t* pa, uint32_t* pb,
-                                                                 uint32_t* perm_out, uint32_t n, SortPlan plan,
+                                                                 uint32_t* perm_out, uint32_t n, uint32_t ntiles,
+                                                                 uint32_t tstride, int ipt, SortPlan plan,
                                                                  const uint32_t* __restrict__ ghist, uint32_t* tile_hist,
                                                                  uint32_t* group_hist, uint32_t ngroups_cap,
                                                                  unsigned long long* __restrict__ tstamp) {
@@ -147,12 +160,12 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
   __shared__ uint32_t s_gbase[kSortMaxPasses][256];   // exclusive scan of every pass's global digit histogram
 
   const int tid = threadIdx.x, warp = tid >> 5;
-  const uint32_t ntiles = (n + kSortTile - 1) / kSortTile;
   const uint32_t ngroups = (ntiles + kSortGroup - 1) / kSortGroup;
   const bool single = ntiles <= gridDim.x;          // one tile per CTA: registers survive the barrier
   KeyT key[kSortItems];
   uint32_t pay[kSortItems];
   uint32_t rank[kSortItems];
+  uint32_t vmask = 0;
 
   {
     uint32_t h[kSortMaxPasses];
@@ -174,7 +187,8 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
 
     // ---- phase A: digit counts of every tile -> tile_hist, group sums
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      sort_load_rank<KeyT>(kin, pin, n, tile * (uint32_t)kSortTile, shift, mask, single, key, pay, rank, s_whist);
+      vmask = sort_load_rank<KeyT>(kin, pin, tile * tstride, min(tstride, n - tile * tstride), ipt, shift, mask, single,
+                                   key, pay, rank, s_whist);
       uint32_t count = 0;
 #pragma unroll
       for (int w = 0; w < 8; ++w) count += s_whist[w][tid];
@@ -191,8 +205,9 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
     // ---- phase B: global offsets, scatter
     const uint32_t gbase = s_gbase[p][tid];
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      const uint32_t base = tile * (uint32_t)kSortTile;
-      if (!single) sort_load_rank<KeyT>(kin, pin, n, base, shift, mask, true, key, pay, rank, s_whist);
+      const uint32_t base = tile * tstride;
+      const uint32_t cnt = min(tstride, n - base);
+      if (!single) vmask = sort_load_rank<KeyT>(kin, pin, base, cnt, ipt, shift, mask, true, key, pay, rank, s_whist);
       // thread d: exclusive prefix over warps of digit d; tile count of digit d
       uint32_t count = 0;
 #pragma unroll
@@ -204,18 +219,27 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
       // digit-d keys in earlier tiles: whole groups from the group sums, the rest of this group tile by tile
       uint32_t excl = 0;
       const uint32_t g = tile / kSortGroup;
-#pragma unroll 8
-      for (uint32_t gg = 0; gg < g; ++gg) excl += __ldcg(gh + (size_t)gg * 256 + tid);
-#pragma unroll 8
-      for (uint32_t t = g * kSortGroup; t < tile; ++t) excl += __ldcg(tile_hist + (size_t)t * 256 + tid);
+      {   // all loads of a batch of 16 are issued before the first use (they are independent L2 hits)
+        const uint32_t ntl = tile - g * kSortGroup, tot = g + ntl;
+        for (uint32_t i0 = 0; i0 < tot; i0 += 16) {
+          uint32_t v[16];
+#pragma unroll
+          for (int u = 0; u < 16; ++u) {
+            const uint32_t i = i0 + u;
+            const uint32_t* src = i < g ? gh + (size_t)i * 256 + tid : tile_hist + (size_t)(g * kSortGroup + (i - g)) * 256 + tid;
+            v[u] = i < tot ? __ldcg(src) : 0u;
+          }
+#pragma unroll
+          for (int u = 0; u < 16; ++u) excl += v[u];
+        }
+      }
       const uint32_t dstart = block_excl_scan_256(count, s_scan, nullptr);
       s_dstart[tid] = dstart;
       s_goff[tid] = gbase + excl - dstart;      // global position = s_goff[d] + tile-local sorted position
       __syncthreads();
-      const uint32_t wbase = base + warp * (kSortItems * 32) + (tid & 31);
 #pragma unroll
       for (int j = 0; j < kSortItems; ++j) {
-        if (wbase + j * 32 < n) {
+        if ((vmask >> j) & 1u) {
           const uint32_t d = (uint32_t)(key[j] >> shift) & mask;
           const uint32_t pos = s_dstart[d] + s_whist[warp][d] + rank[j];
           s_keys[pos] = key[j];
@@ -223,7 +247,6 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
         }
       }
       __syncthreads();
-      const uint32_t cnt = min((uint32_t)kSortTile, n - base);
       for (uint32_t i = tid; i < cnt; i += kSortThreads) {
         const KeyT k = s_keys[i];
         const uint32_t d = (uint32_t)(k >> shift) & mask;
@@ -455,7 +478,6 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
                        int depth, uint8_t* d_occ, uint64_t occ_capacity, uint32_t* d_level_sizes, uint32_t* d_perm,
                        uint64_t* d_voxel_keys, uint32_t* d_voxel_start, gsnfs_counts* d_counts) {
   const SortPlan plan = make_sort_plan(depth);
-  const uint32_t stiles = (n + kSortTile - 1) / kSortTile;
   KeyT* ka = reinterpret_cast<KeyT*>(ctx->keys_a);
   KeyT* kb = reinterpret_cast<KeyT*>(ctx->keys_b);
 
@@ -476,8 +498,15 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
         ctx->occ_cache[slot] = per_sm;
       }
       if (per_sm < 1) { snprintf(ctx->err, sizeof(ctx->err), "sort kernel does not fit on an SM"); return GSNFS_E_CUDA; }
-      uint32_t grid = (uint32_t)per_sm * (uint32_t)ctx->num_sms;
-      if (grid > stiles) grid = stiles;
+      // balanced tiling: the tile count is (close to) a multiple of the co-resident grid, so that every SM
+      // ranks and scatters the same number of keys in every pass; tile stride <= kSortTile, a multiple of 32
+      const uint32_t cap = (uint32_t)per_sm * (uint32_t)ctx->num_sms;
+      const uint32_t rounds = (n + cap * (uint32_t)kSortTile - 1u) / (cap * (uint32_t)kSortTile);
+      uint32_t tstride = ((n + cap * rounds - 1u) / (cap * rounds) + 31u) & ~31u;
+      if (tstride < 1024u) tstride = 1024u;
+      const uint32_t stiles = (n + tstride - 1u) / tstride;
+      int ipt = (int)((tstride + kSortThreads - 1u) / kSortThreads);
+      uint32_t grid = cap < stiles ? cap : stiles;
       KeyT* kbuf_a = ka;
       KeyT* kbuf_b = kb;
       uint32_t* pbuf_a = ctx->pay_a;
@@ -489,7 +518,9 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
       uint32_t* grp = ctx->sort_group_hist;
       uint32_t gcap = ctx->sort_groups_cap;
       unsigned long long* tstamp = ctx->raht_plan->t_sort;
-      void* args[] = {(void*)&kbuf_a, (void*)&kbuf_b, (void*)&pbuf_a, (void*)&pbuf_b, (void*)&d_perm, (void*)&nn, (void*)&pl,
+      uint32_t ntl = stiles;
+      void* args[] = {(void*)&kbuf_a, (void*)&kbuf_b, (void*)&pbuf_a, (void*)&pbuf_b, (void*)&d_perm, (void*)&nn, (void*)&ntl,
+                      (void*)&tstride, (void*)&ipt, (void*)&pl,
                       (void*)&gh, (void*)&th, (void*)&grp, (void*)&gcap, (void*)&tstamp};
       GSNFS_KERNEL(ctx, st, "radix_sort");
       GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)sort_coop_kernel<KeyT>, dim3(grid), dim3(kSortThreads), args, smem, st));
