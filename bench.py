@@ -111,6 +111,75 @@ def algorithmic_bytes(n, nv, s_occ, channels, depth):
     }
 
 
+def run_ladder(B, synth, torch, ctx, buf, dev, n_frames):
+    """BASELINE.json configs[4]: the dynamic sequence, every frame encoded + decoded at the 4 qstep rungs back to
+    back on one stream through the public calls.  Frames are generated on the device outside the timed region;
+    per frame the 4 rungs are bracketed by CUDA events.  Two variants: "independent" = 4 full encode+decode passes;
+    "shared" = one sort/octree/transform + 4 gsnfs_quantize, one octree decode + 4 inverse transforms."""
+    seq = synth.DynamicSequenceDevice(dev)
+    n, C, J = seq.n, seq.channels, seq.depth
+    lo, hi = np.zeros(3, np.float32), np.ones(3, np.float32)
+    stream = torch.cuda.current_stream()
+    h_hdr = torch.empty(J + 1 + 4, dtype=torch.int32).pin_memory()
+    coeff = torch.empty((n, C), dtype=torch.float32, device=dev)
+    qrung = [torch.empty((n, C), dtype=torch.int32, device=dev) for _ in synth.LADDER_QDIVS]
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+
+    def header():
+        h_hdr[:J + 1].copy_(buf.level_sizes, non_blocking=True)
+        h_hdr[J + 1:].copy_(buf.counts, non_blocking=True)
+        stream.synchronize()
+        return h_hdr[:J + 1].numpy(), int(h_hdr[J + 2])
+
+    def independent(xyz, attr):
+        for d in synth.LADDER_QDIVS:
+            B.encode_frame(ctx, buf, xyz, attr, lo, hi, seq.qsteps[d])
+            levels, occ_bytes = header()
+            B.decode_frame(ctx, buf, levels, occ_bytes, seq.qsteps[d])
+
+    def shared(xyz, attr):
+        B.gsnfs_octree_encode(ctx, xyz, n, lo, hi, J, buf.occ, buf.level_sizes, buf.perm, buf.voxel_keys,
+                              buf.voxel_start, buf.counts)
+        B.gsnfs_merge_raht_forward(ctx, buf.voxel_keys, buf.perm, buf.voxel_start, n, buf.counts, J, attr, C, None, None,
+                                   buf.weights, None, coeff)
+        for i, d in enumerate(synth.LADDER_QDIVS):
+            B.gsnfs_quantize(ctx, coeff, n, buf.counts, C, seq.qsteps[d], None, qrung[i])
+        levels, occ_bytes = header()
+        nv = int(levels[J])
+        B.gsnfs_octree_decode(ctx, buf.occ, occ_bytes, levels, J, buf.dec_xyz, buf.dec_keys, buf.dec_counts)
+        for i, d in enumerate(synth.LADDER_QDIVS):
+            B.gsnfs_raht_inverse(ctx, buf.dec_keys, buf.weights, nv, None, J, qrung[i], None, C, seq.qsteps[d], None,
+                                 buf.dec_attr)
+
+    xyz, attr = seq.frame(0)
+    for _ in range(3):
+        independent(xyz, attr)
+        shared(xyz, attr)
+    torch.cuda.synchronize()
+    ms_ind = ms_sh = 0.0
+    for t in range(n_frames):
+        xyz, attr = seq.frame(t)
+        torch.cuda.synchronize()
+        e0.record(stream)
+        independent(xyz, attr)
+        e1.record(stream)
+        shared(xyz, attr)
+        e2.record(stream)
+        torch.cuda.synchronize()
+        ms_ind += e0.elapsed_time(e1)
+        ms_sh += e1.elapsed_time(e2)
+    r = len(synth.LADDER_QDIVS)
+    return {"workload": f"BASELINE.json configs[4]: {n_frames} frames x {r} rungs (qstep = range/{list(synth.LADDER_QDIVS)}), "
+                        f"N={n}, C={C}, depth {J}, frames generated on the device (synth.DynamicSequenceDevice)",
+            "frames": n_frames, "rungs": r, "target_fps": 30.0,
+            "independent": {"frames_per_s": round(n_frames / (ms_ind * 1e-3), 1),
+                            "frame_rungs_per_s": round(n_frames * r / (ms_ind * 1e-3), 1),
+                            "ms_per_frame": round(ms_ind / n_frames, 4)},
+            "shared_geometry_and_transform": {"frames_per_s": round(n_frames / (ms_sh * 1e-3), 1),
+                                              "frame_rungs_per_s": round(n_frames * r / (ms_sh * 1e-3), 1),
+                                              "ms_per_frame": round(ms_sh / n_frames, 4)}}
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -243,6 +312,9 @@ def run_ours(args, rank, world, local_rank):
         e2e = {"value": round(world * n / (ms_e * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_e, 4),
                "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ks}
 
+    ladder = None
+    if rank == 0 and world == 1 and args.ladder_frames > 0 and args.config == 3:
+        ladder = run_ladder(B, synth, torch, ctx, buf, dev, args.ladder_frames)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = oracle_time(fr, sample_n=None)
@@ -264,7 +336,7 @@ def run_ours(args, rank, world, local_rank):
         "roofline": roofline,
         "sort": {"alg_bytes": ab["_sort_total"], "ms_per_step": sort_ms, "passes": ab["_passes"],
                  "frac_of_peak": round(sort_frac, 4) if sort_frac else None},
-        "kernels": kernels, "cpu_baseline": cpu,
+        "kernels": kernels, "ladder": ladder, "cpu_baseline": cpu,
     }
     print(json.dumps(out))
 
@@ -323,6 +395,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); 3 = headline 1M frame")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--ladder-frames", type=int, default=300,
+                    help="frames of the config-5 dynamic sequence to run at 4 rungs each (0 = skip; N=1, config 3 only)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

@@ -147,6 +147,18 @@ int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
                        const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
                        int32_t* d_qcoeff, float* d_coeff);
 
+/* One more quantisation of an unquantised coefficient tensor (d_coeff of gsnfs_raht_forward, N_v x channels,
+ * canonical order): d_qcoeff[i][c] = sign(y) floor(|y|/qstep_c + dz_round), the same rule and arithmetic as the
+ * quantiser fused into gsnfs_raht_forward [R10], so a bitrate ladder (one step per
+ * attribute and rung) can share one sort/octree/transform and pay only this pass per rung.  qstep: host,
+ * `channels` entries, all > 0 and finite; quant may be NULL (dz_round = 1/3).  n_rows is the row count; if
+ * d_counts != NULL the actual N_v is read on the device and n_rows is an upper bound (rows beyond N_v are
+ * untouched).  Asynchronous on `stream`; d_coeff and d_qcoeff are caller-owned device memory and may not overlap. */
+int gsnfs_quantize(gsnfs_ctx* ctx, gsnfs_stream stream,
+                   const float* d_coeff /* N_v x channels */, uint64_t n_rows, const gsnfs_counts* d_counts,
+                   int channels, const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
+                   int32_t* d_qcoeff /* N_v x channels */);
+
 /* Fused gsnfs_voxel_merge + gsnfs_raht_forward(weights = counts): the same coefficients, bit for bit, as
  * the two calls in sequence, but phase-1 rows are gathered through d_perm straight into shared memory and
  * the merged N_v x channels tensor is never written (saves a 2 x 4*channels bytes/voxel round trip).

@@ -62,6 +62,8 @@ _SIGNATURES = {
                                          c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p, c_void_p, c_void_p]),
     "gsnfs_raht_inverse": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p,
                                    c_void_p, c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p]),
+    "gsnfs_quantize": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, POINTER(c_float),
+                               POINTER(GsnfsQuant), c_void_p]),
     "gsnfs_frame_encode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_int, POINTER(c_float),
                                         POINTER(c_float), c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p,
                                         c_uint64, c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -265,6 +267,14 @@ def gsnfs_merge_raht_forward(ctx: Context, d_voxel_keys, d_perm, d_voxel_start, 
         _dptr(d_weights_out, torch.int32, "d_weights_out"), _dptr(d_qcoeff, torch.int32, "d_qcoeff"),
         _dptr(d_coeff, torch.float32, "d_coeff"))
     ctx._check(rc, "gsnfs_merge_raht_forward")
+
+
+def gsnfs_quantize(ctx: Context, d_coeff, n_rows, d_counts, channels, qstep, quant, d_qcoeff, stream=None):
+    rc = lib().gsnfs_quantize(
+        ctx.handle, _stream(stream), _dptr(d_coeff, torch.float32, "d_coeff"), int(n_rows),
+        _dptr(d_counts, torch.int32, "d_counts"), int(channels), _farr(qstep, channels), _quant(quant),
+        _dptr(d_qcoeff, torch.int32, "d_qcoeff"))
+    ctx._check(rc, "gsnfs_quantize")
 
 
 def gsnfs_raht_inverse(ctx: Context, d_voxel_keys, d_weights, n_voxels, d_counts, depth, d_qcoeff, d_coeff, channels,

@@ -283,6 +283,17 @@ int gsnfs_merge_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t
                   channels, qstep, quant, d_qcoeff, d_coeff, d_perm, d_voxel_start, d_weights_out);
 }
 
+int gsnfs_quantize(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_coeff, uint64_t n_rows,
+                   const gsnfs_counts* d_counts, int channels, const float* qstep, const gsnfs_quant* quant,
+                   int32_t* d_qcoeff) {
+  if (!ctx || !qstep || (n_rows && (!d_coeff || !d_qcoeff))) return GSNFS_E_INVALID_ARGUMENT;
+  if (channels < 1 || channels > GSNFS_MAX_CHANNELS || n_rows >= (1ull << 30)) return GSNFS_E_INVALID_ARGUMENT;
+  for (int c = 0; c < channels; ++c)
+    if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  return run_quantize(ctx, (cudaStream_t)stream, d_coeff, (uint32_t)n_rows, d_counts, channels, qstep, quant, d_qcoeff);
+}
+
 int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_weights,
                        uint64_t n_voxels, const gsnfs_counts* d_counts, int depth, const int32_t* d_qcoeff,
                        const float* d_coeff, int channels, const float* qstep, const gsnfs_quant* quant,

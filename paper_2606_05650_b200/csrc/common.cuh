@@ -234,6 +234,8 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
              const int32_t* d_in_q, int channels, const float* qstep, const gsnfs_quant* quant,
              int32_t* d_out_q, float* d_out_f, const uint32_t* d_perm = nullptr, const uint32_t* d_vstart = nullptr,
              uint32_t* d_weights_out = nullptr);
+int run_quantize(gsnfs_ctx* ctx, cudaStream_t st, const float* d_coeff, uint32_t n, const gsnfs_counts* d_counts,
+                 int channels, const float* qstep, const gsnfs_quant* quant, int32_t* d_qcoeff);
 int raht_setup(gsnfs_ctx* ctx);   // occupancy queries + attributes, called from gsnfs_create
 
 }  // namespace gsnfs

@@ -855,6 +855,54 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
 }
 
 // ------------------------------------------------------------------------------------------------
+// Quantise an N_v x C fp32 coefficient tensor with one step per channel (one ladder rung from a shared
+// transform, section 3.4 L255 + L47-49 bitrate ladder).  Same quantiser as the fused one [R10].
+// ------------------------------------------------------------------------------------------------
+template <int VEC>
+__global__ void __launch_bounds__(256) quantize_kernel(const float* __restrict__ coeff, uint32_t n_host,
+                                                       const uint32_t* __restrict__ n_dev, int C, QStepParams qs, double dz,
+                                                       int32_t* __restrict__ out_q) {
+  __shared__ double s_inv64[(GSNFS_MAX_CHANNELS + 3) & ~3];
+  __shared__ __align__(16) float s_inv32[(GSNFS_MAX_CHANNELS + 3) & ~3];
+  for (int c = threadIdx.x; c < ((C + 3) & ~3); c += 256) {
+    const double iv = c < C ? 1.0 / (double)qs.step[c] : 0.0;
+    s_inv64[c] = iv;
+    s_inv32[c] = (float)iv;
+  }
+  __syncthreads();
+  QuantTab qt;
+  qt.inv64 = s_inv64;
+  qt.inv32 = s_inv32;
+  const float dz32 = (float)(dz - 0.5);
+  const uint32_t n = n_dev ? min(*n_dev, n_host) : n_host;
+  const uint32_t cv = (uint32_t)(C / VEC);
+  const uint64_t tot = (uint64_t)n * cv;
+  const uint64_t stride = (uint64_t)gridDim.x * 256u;
+  for (uint64_t i = (uint64_t)blockIdx.x * 256u + threadIdx.x; i < tot; i += stride) {
+    const int c = (int)(i % cv);
+    if constexpr (VEC == 4) reinterpret_cast<int4*>(out_q)[i] = quant4(reinterpret_cast<const float4*>(coeff)[i], c, qt, dz, dz32);
+    else out_q[i] = quant1s(coeff[i], c, qt, dz, dz32);
+  }
+}
+
+int run_quantize(gsnfs_ctx* ctx, cudaStream_t st, const float* d_coeff, uint32_t n, const gsnfs_counts* d_counts,
+                 int channels, const float* qstep, const gsnfs_quant* quant, int32_t* d_qcoeff) {
+  if (n == 0) return GSNFS_OK;
+  QStepParams qs;
+  for (int c = 0; c < GSNFS_MAX_CHANNELS; ++c) qs.step[c] = c < channels ? qstep[c] : 1.0f;
+  const double dz = quant ? (double)quant->dz_round : (double)(1.0f / 3.0f);
+  const uint32_t* n_dev = d_counts ? &d_counts->n_voxels : nullptr;
+  const bool vec4 = (channels % 4) == 0;
+  const uint64_t tot = (uint64_t)n * (uint64_t)(vec4 ? channels / 4 : channels);
+  const int grid = (int)min((uint64_t)ctx->num_sms * 8u, (tot + 255u) / 256u);     // 8 resident CTAs per SM, grid-stride
+  GSNFS_KERNEL(ctx, st, "quantize");
+  if (vec4) quantize_kernel<4><<<grid, 256, 0, st>>>(d_coeff, n, n_dev, channels, qs, dz, d_qcoeff);
+  else quantize_kernel<1><<<grid, 256, 0, st>>>(d_coeff, n, n_dev, channels, qs, dz, d_qcoeff);
+  GSNFS_LAUNCH_CHECK(ctx, st);
+  return GSNFS_OK;
+}
+
+// ------------------------------------------------------------------------------------------------
 static size_t raht_smem_bytes(int C) {
   return sizeof(float) * (size_t)T * C + 2 * sizeof(TileMeta) + (sizeof(double) + sizeof(float)) * ((C + 3) & ~3);
 }

@@ -233,3 +233,54 @@ class DynamicSequence:
         return Frame(name=f"config5_t{t}", xyz=xyz32, attr=attr32, qstep=self.qsteps[256],
                      depth=self.depth, qdiv=256,
                      bbox_min=np.zeros(3, np.float32), bbox_max=np.ones(3, np.float32))
+
+
+class DynamicSequenceDevice:
+    """Config 5 generated on the device (300 x 236 MB cannot be pre-stored, and 300 numpy steps of
+    56M normal draws would take minutes).  Frame 0 is ``DynamicSequence``'s (numpy, seed 4); frames t >= 1 use the
+    same formulas in fp64 with a seeded ``torch.Generator`` on the device: positions from frame 0 directly,
+    attributes by a random walk, one N(0, 0.01) step per frame on all channels.  ``frame(t)`` returns the fp32
+    device tensors; ``host_frame(t)`` copies them into a ``Frame`` so a CPU checker sees the very same arrays."""
+
+    def __init__(self, device="cuda:0", n_override: int | None = None):
+        import torch
+        self.torch = torch
+        base = DynamicSequence(n_override)
+        self.depth = base.depth
+        self.qsteps = base.qsteps                       # from frame 0's channel ranges, one per ladder rung
+        self.device = device
+        self.p0 = torch.from_numpy(base.p0).to(device)                   # fp64
+        self.k = torch.from_numpy(np.ascontiguousarray(base.k)).to(device)
+        self.attr = torch.from_numpy(base.attr).to(device)               # fp64 random-walk state
+        self.proj = (self.k * self.p0).sum(dim=1)
+        self.gen = torch.Generator(device=device)
+        self.gen.manual_seed(_CONFIGS[5][0])
+        self.t = 0
+        self.n, self.channels = int(self.p0.shape[0]), int(self.attr.shape[1])
+        self._xyz = self.p0.to(torch.float32).contiguous()
+        self._attr = self.attr.to(torch.float32).contiguous()
+
+    def _step(self):
+        torch = self.torch
+        self.t += 1
+        t = self.t
+        phase = 2.0 * np.pi * (0.5 * t / 30.0 + self.proj)
+        jit = torch.randn(self.p0.shape, generator=self.gen, device=self.device, dtype=torch.float64) * 1e-4
+        pos = (self.p0 + 0.01 * torch.sin(phase)[:, None] * self.k + jit).clamp_(0.0, 1.0)
+        self.attr += torch.randn(self.attr.shape, generator=self.gen, device=self.device, dtype=torch.float64) * 0.01
+        self._xyz = pos.to(torch.float32).contiguous()
+        self._attr = self.attr.to(torch.float32).contiguous()
+
+    def frame(self, t: int):
+        """Device tensors (xyz N x 3, attr N x C, fp32) of frame t; frames are visited in increasing order."""
+        if t < self.t:
+            raise ValueError("frames must be requested in increasing order")
+        while self.t < t:
+            self._step()
+        return self._xyz, self._attr
+
+    def host_frame(self, t: int, qdiv: int = 256) -> Frame:
+        xyz, attr = self.frame(t)
+        return Frame(name=f"config5_t{t}_D{qdiv}", xyz=xyz.cpu().numpy(), attr=attr.cpu().numpy(),
+                     qstep=self.qsteps[qdiv], depth=self.depth, qdiv=qdiv,
+                     bbox_min=np.zeros(3, np.float32), bbox_max=np.ones(3, np.float32))

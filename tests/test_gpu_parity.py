@@ -373,3 +373,66 @@ def test_host_frame_calls_roundtrip(B, ctx_small):
     # reconstruction error bounded by the quantiser: compare against the merged attributes loosely
     rng_c = (fr.qstep.astype(np.float64) * fr.qdiv)[None, :]
     assert np.max(np.abs(h_out[:nv].numpy() - ref["merged"]) / rng_c) < 0.05
+
+
+# ---------------------------------------------------------------------------------------------- ladder
+@pytest.mark.parametrize("maker", ["config2", "dense12", "dense7"])
+def test_quantize_call_matches_fused_quantiser_and_oracle(B, ctx_small, maker):
+    """gsnfs_quantize on the unquantised coefficients == the quantiser fused into gsnfs_raht_forward, bit for bit,
+    for every ladder rung, and == the oracle's rule applied to the same fp32 coefficients (the integer decision
+    is taken in fp64 on both sides)."""
+    fr = {"config2": lambda: synth.make_frame(2), "dense12": lambda: synth.make_dense_frame(30_000, 6, 12),
+          "dense7": lambda: synth.make_dense_frame(3_000, 4, 7)}[maker]()
+    buf, got = gpu_position_encode(B, ctx_small, fr)
+    nv = got["n_voxels"]
+    d_attr = _t(fr.attr)
+    coeff = torch.empty((fr.n, fr.channels), dtype=torch.float32, device=DEV)
+    w = torch.empty(fr.n, dtype=torch.int32, device=DEV)
+    B.gsnfs_merge_raht_forward(ctx_small, buf.voxel_keys, buf.perm, buf.voxel_start, fr.n, buf.counts, fr.depth, d_attr,
+                               fr.channels, None, None, w, None, coeff)
+    q_sep = torch.empty((fr.n, fr.channels), dtype=torch.int32, device=DEV)
+    ch_range = fr.qstep.astype(np.float64) * fr.qdiv
+    for qdiv in synth.LADDER_QDIVS:
+        for dz in (None, 0.5):
+            qstep = (ch_range / qdiv).astype(np.float32)
+            quant = None if dz is None else (dz, 0.0)
+            B.gsnfs_quantize(ctx_small, coeff, fr.n, buf.counts, fr.channels, qstep, quant, q_sep)
+            B.gsnfs_merge_raht_forward(ctx_small, buf.voxel_keys, buf.perm, buf.voxel_start, fr.n, buf.counts, fr.depth,
+                                       d_attr, fr.channels, qstep, quant, w, buf.qcoeff, None)
+            torch.cuda.synchronize()
+            assert torch.equal(q_sep[:nv], buf.qcoeff[:nv])
+            q_ref = orc.quantize(coeff[:nv].cpu().numpy().astype(np.float64), qstep,
+                                 dz_round=orc.DZ_ROUND_DEFAULT if dz is None else float(np.float32(dz)))
+            assert np.array_equal(q_sep[:nv].cpu().numpy().astype(np.int64), q_ref)
+    # argument errors
+    with pytest.raises(B.GsnfsError):
+        B.gsnfs_quantize(ctx_small, coeff, fr.n, buf.counts, fr.channels, np.zeros(fr.channels, np.float32), None, q_sep)
+
+
+@pytest.mark.parametrize("t", [0, 149, 299])
+def test_config5_dynamic_sequence_frames_all_rungs(B, ctx_big, t):
+    """BASELINE.json configs[4]: frames {0, 149, 299} of the 300-frame sequence at the 4 ladder rungs, position
+    coder bit-exact, quantised coefficients and decoded attributes within north_star's tolerances."""
+    seq = synth.DynamicSequenceDevice(DEV)
+    fr = seq.host_frame(t, 256)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    buf, got = gpu_position_encode(B, ctx_big, fr)
+    check_position(got, ref, fr.n)
+    nv = got["n_voxels"]
+    d_attr = _t(fr.attr)
+    dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], fr.depth)
+    assert ok
+    for qdiv in synth.LADDER_QDIVS:
+        qstep = seq.qsteps[qdiv]
+        q_ref = orc.quantize(ref["coeff"], qstep)
+        B.gsnfs_merge_raht_forward(ctx_big, buf.voxel_keys, buf.perm, buf.voxel_start, fr.n, buf.counts, fr.depth, d_attr,
+                                   fr.channels, qstep, None, buf.weights, buf.qcoeff, None)
+        torch.cuda.synchronize()
+        check_quantised(buf.qcoeff[:nv].cpu().numpy(), q_ref)
+        buf.qcoeff[:nv].copy_(_t(q_ref.astype(np.int32)))
+        B.decode_frame(ctx_big, buf, ref["level_sizes"], len(ref["occ"]), qstep)
+        torch.cuda.synchronize()
+        assert np.array_equal(buf.dec_xyz[:nv].cpu().numpy().astype(np.uint64), dc)
+        ref_attr = orc.raht_inverse(orc.dequantize(q_ref, qstep), dk, ref["weights"], fr.depth)
+        ch_range = (seq.qsteps[256].astype(np.float64) * 256)[None, :]
+        assert np.all(np.abs(buf.dec_attr[:nv].cpu().numpy().astype(np.float64) - ref_attr) <= 1e-4 * ch_range)
