@@ -122,7 +122,8 @@ int gsnfs_voxel_merge(gsnfs_ctx* ctx, gsnfs_stream stream,
  * level_sizes (host, depth+1 entries) is the stream header [O6]; N_v = level_sizes[depth] and
  * occ_bytes must equal sum_{d<depth} level_sizes[d].  d_voxel_xyz is N_v x 3 (x, y, z) uint32;
  * d_voxel_keys (N_v) may be NULL.  A zero occupancy byte or a level whose popcount sum differs from
- * the header sets d_counts->status bit 0 [O12]; no out-of-bounds access happens either way. */
+ * the header sets d_counts->status bit 0 [O12]; no out-of-bounds access happens either way.
+ * occ_bytes must be < 2^29 (GSNFS_E_CAPACITY otherwise). */
 int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream,
                         const uint8_t* d_occ, uint64_t occ_bytes,
                         const uint32_t* level_sizes /* host, depth+1 */, int depth,

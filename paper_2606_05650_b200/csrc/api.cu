@@ -89,8 +89,8 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
   const size_t o_rplan = b.take(sizeof(RahtPlan));
   const size_t o_rrows = b.take(c->raht_pool_rows * (size_t)C * 4);
-  const size_t o_dscan = b.take((c->occ_cap + 1) * 4);
-  const size_t o_dka = b.take((N + 1) * 8), o_dkb = b.take((N + 1) * 8);
+  const size_t o_dscan = b.take(256);
+  const size_t o_dpar = b.take((c->occ_cap + N + 2) * 4), o_dkm = b.take((N + 1) * 8);
   c->pool_bytes = b.off;
   GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->pool, c->pool_bytes));
   char* p = c->pool;
@@ -104,8 +104,9 @@ static int create_impl(gsnfs_ctx* c) {
   c->raht_rec = (uint4*)(p + o_rrec); c->raht_gsrc = (uint32_t*)(p + o_rgs);
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
-  c->dec_scan = (uint32_t*)(p + o_dscan); c->dec_keys_a = (uint64_t*)(p + o_dka); c->dec_keys_b = (uint64_t*)(p + o_dkb);
-  GSNFS_CUDA_OK(c, cudaMemset(c->pool, 0, o_rrows));     // everything but the big row pool
+  c->dec_scan = (uint32_t*)(p + o_dscan); c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);
+  GSNFS_CUDA_OK(c, cudaMemset(c->pool, 0, o_rrows));     // everything but the big row pool ...
+  GSNFS_CUDA_OK(c, cudaMemset(p + o_dscan, 0, c->pool_bytes - o_dscan));   // ... and the decoder's scan / parent arrays
   int rc = octree_encode_setup(c);
   if (rc != GSNFS_OK) return rc;
   return raht_setup(c);
