@@ -105,7 +105,8 @@ def algorithmic_bytes(n, nv, s_occ, channels, depth):
         "raht_forward": c4 * nv + c4 * nv + 16 * nv + 8 * nv,   # fused merge: gathers the N input rows itself
         "raht_inverse": c4 * nv + c4 * nv + 16 * nv,
         "scan_reduce": None, "scan_sums": None, "scan_down": None,   # used twice with different inputs
-        "expand_children": (s_occ + 4 * s_occ + 8 * (s_occ + nv) + 12 * nv) / max(depth, 1),
+        "octree_decode": s_occ + 20 * nv,                       # stream in, leaf codes + coordinates out
+        "quantize": 8 * channels * nv,
         "radix_sort": k * n + passes * 2 * (k + 4) * n,         # histogram read + P passes of (key, index) in and out
         "_sort_total": k * n + passes * 2 * (k + 4) * n, "_passes": passes,
     }

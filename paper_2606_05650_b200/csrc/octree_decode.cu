@@ -226,6 +226,9 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
     if (occ_bytes != 0) status = 1;
   } else if (sum != occ_bytes || level_sizes[0] != 1) {
     status = 1;                                               // header inconsistent with the stream [O12]
+  } else {
+    for (int d = 0; d < depth; ++d)
+      if (level_sizes[d] == 0 || level_sizes[d] > level_sizes[d + 1]) status = 1;    // every node has >= 1 child
   }
   for (int d = 0; d <= depth; ++d)
     if (level_sizes[d] > ctx->max_points) return GSNFS_E_CAPACITY;

@@ -274,6 +274,39 @@ def test_corrupt_stream_is_flagged(B, ctx_small):
     B.gsnfs_octree_decode(ctx_small, buf.occ, len(ref["occ"]), sizes, fr.depth, buf.dec_xyz, buf.dec_keys, buf.dec_counts)
     torch.cuda.synchronize()
     assert int(buf.dec_counts.cpu()[2]) & 1
+    # header whose level sizes do not match the stream although their sum does: one node moved between two levels
+    # (every level boundary after it is off by one), an empty level, a level larger than the next one
+    S = len(ref["occ"])
+    for mutate in ("shift", "empty", "order"):
+        sizes = ref["level_sizes"].copy()
+        d = fr.depth // 2
+        if mutate == "shift":
+            sizes[d] += 1; sizes[d + 1] -= 1
+        elif mutate == "empty":
+            sizes[d + 1] += sizes[d]; sizes[d] = 0
+        else:
+            sizes[d], sizes[d - 1] = sizes[d - 1] + sizes[d] - 1, 1
+        assert int(sizes[:fr.depth].sum()) == S
+        B.gsnfs_octree_decode(ctx_small, buf.occ, S, sizes, fr.depth, buf.dec_xyz, buf.dec_keys, buf.dec_counts)
+        torch.cuda.synchronize()
+        assert int(buf.dec_counts.cpu()[2]) & 1, mutate
+    # a bit flipped in the middle of the stream (no zero byte): the popcount total no longer matches the header
+    occ = ref["occ"].copy()
+    k = len(occ) // 3
+    occ[k] = occ[k] ^ 0x10 if occ[k] ^ 0x10 else occ[k] ^ 0x01
+    buf.occ[:len(occ)].copy_(_t(occ))
+    B.gsnfs_octree_decode(ctx_small, buf.occ, S, ref["level_sizes"], fr.depth, buf.dec_xyz, buf.dec_keys, buf.dec_counts)
+    torch.cuda.synchronize()
+    assert int(buf.dec_counts.cpu()[2]) & 1
+    # and the intact stream still decodes cleanly afterwards (stale scratch from the corrupt runs is harmless)
+    buf.occ[:S].copy_(_t(ref["occ"]))
+    B.gsnfs_octree_decode(ctx_small, buf.occ, S, ref["level_sizes"], fr.depth, buf.dec_xyz, buf.dec_keys, buf.dec_counts)
+    torch.cuda.synchronize()
+    assert int(buf.dec_counts.cpu()[2]) == 0
+    dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], fr.depth)
+    nv = int(ref["level_sizes"][fr.depth])
+    assert np.array_equal(buf.dec_keys[:nv].cpu().numpy().astype(np.uint64), dk)
+    assert np.array_equal(buf.dec_xyz[:nv].cpu().numpy().astype(np.uint64), dc)
 
 
 def test_argument_errors(B, ctx_small):
