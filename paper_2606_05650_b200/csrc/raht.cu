@@ -24,6 +24,10 @@ namespace cg = cooperative_groups;
 namespace gsnfs {
 
 constexpr int T = kRahtTile;
+#ifndef RAHT_XT
+#define RAHT_XT 256
+#endif
+constexpr int kXT = RAHT_XT;        // threads per CTA of the transform kernels
 
 struct QStepParams {
   float step[GSNFS_MAX_CHANNELS];
@@ -436,7 +440,7 @@ __device__ __forceinline__ bool quant_fast2(float y0, float y1, float i0, float 
   const uint64_t t = fma2(pk2(y0, y1), pk2(i0, i1), pk2(s0, s1));
   const uint64_t u = add2(t, pk2(12582912.0f, 12582912.0f));
   const uint64_t rn = add2(u, pk2(-12582912.0f, -12582912.0f));
-  const uint64_t d = add2(t, rn ^ 0x8000000080000000ull);
+  const uint64_t d = fma2(t, pk2(-1.0f, -1.0f), rn);      // rn - t (exact); only |d| is used
   float t0, t1, u0, u1, d0, d1;
   upk2(t, t0, t1); upk2(u, u0, u1); upk2(d, d0, d1);
   q0 = __float_as_int(u0) - 0x4B400000;
@@ -504,7 +508,7 @@ __device__ __forceinline__ void prefetch_meta(TileMeta* m, const uint4* rec, con
                                               const uint32_t* weights, const uint32_t* gsrc, size_t tglob, uint32_t ks,
                                               uint32_t cnt) {
   const int tid = threadIdx.x;
-  cp_async16(&m->rec[tid], rec + tglob * T + tid);
+  if (tid < T) cp_async16(&m->rec[tid], rec + tglob * T + tid);
   if (tid < (int)(sizeof(RahtTileHdr) / 16))
     cp_async16(reinterpret_cast<uint4*>(&m->hdr) + tid, reinterpret_cast<const uint4*>(hdr + tglob) + tid);
   if (weights && (uint32_t)tid < cnt) cp_async4(&m->w[tid], weights + ks + tid);
@@ -517,10 +521,10 @@ __device__ __forceinline__ void stage_rows_contig(float* s_rows, const float* sr
     const uint32_t tot = nrows * (uint32_t)(C / 4);
     const float4* g = reinterpret_cast<const float4*>(src);
     float4* s = reinterpret_cast<float4*>(s_rows);
-    for (uint32_t i = threadIdx.x; i < tot; i += 256) cp_async16(s + i, g + i);
+    for (uint32_t i = threadIdx.x; i < tot; i += kXT) cp_async16(s + i, g + i);
   } else {
     const uint32_t tot = nrows * (uint32_t)C;
-    for (uint32_t i = threadIdx.x; i < tot; i += 256) cp_async4(s_rows + i, src + i);
+    for (uint32_t i = threadIdx.x; i < tot; i += kXT) cp_async4(s_rows + i, src + i);
   }
 }
 
@@ -531,7 +535,7 @@ struct GatherArgs {          // fused merge: rows of phase 1 are gathered throug
 };
 
 template <int VEC>
-__global__ void __launch_bounds__(256) raht_forward_kernel(
+__global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
     const float* __restrict__ attr_in, const uint32_t* __restrict__ weights, GatherArgs ga, float* __restrict__ pool,
     const uint4* __restrict__ rec, const RahtTileHdr* __restrict__ hdr, RahtPlan* __restrict__ plan, int C,
     QStepParams qs, int has_q, double dz, int32_t* __restrict__ out_q, float* __restrict__ out_f) {
@@ -548,7 +552,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int hw = tid >> 4, l16 = tid & 15;
   const int cv = C / VEC;
-  for (int c = tid; c < C; c += 256) {
+  for (int c = tid; c < C; c += kXT) {
     const double iv = has_q ? 1.0 / (double)qs.step[c] : 0.0;
     qt.inv64[c] = iv;
     qt.inv32[c] = (float)iv;
@@ -580,7 +584,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
         cp_async_wait_all();                       // meta(cur) was prefetched one tile ago
         __syncthreads();
         const uint32_t tot = nent * (uint32_t)cv;
-        for (uint32_t i = tid; i < tot; i += 256) {
+        for (uint32_t i = tid; i < tot; i += kXT) {
           const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
           const uint32_t c = i - k * (uint32_t)cv;
           const float* g = src + (size_t)mt->g[k] * C;
@@ -601,7 +605,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
       __syncthreads();
       const uint32_t nmerge = mt->hdr.nmerge, nseg = mt->hdr.nent >> 16;
       {   // destination of every entry, in natural order
-        const uint32_t pm = mt->hdr.pendmask[warp];
+        const uint32_t pm = warp < 8 ? mt->hdr.pendmask[warp] : 0u;
         uint32_t before = 0;
 #pragma unroll
         for (int w = 0; w < 8; ++w) if (w < warp) before += __popc(mt->hdr.pendmask[w]);
@@ -611,7 +615,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
       // [R2] x_i = sqrt(w_i) a_i: only rows with w != 1 need work (block-uniform test first)
       bool staged = false;             // a barrier has passed since the rows and s_dst were written
       if (wts && !(staged = !__syncthreads_or((uint32_t)tid < nent && mt->w[tid] != 1u))) {
-        for (uint32_t k = hw; k < nent; k += 16) {
+        for (uint32_t k = hw; k < nent; k += kXT / 16) {
           const uint32_t w = mt->w[k];
           if (w != 1u) {
             V* r = reinterpret_cast<V*>(s_rows + (size_t)k * C);
@@ -643,7 +647,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
       uint32_t sj = 0;
       for (uint32_t s = 0; s < nseg; ++s) {                               // non-empty levels, bottom-up
         const uint32_t ej = mt->hdr.lev_end[s];
-        for (uint32_t j = sj + hw; j < ej; j += 16) {
+        for (uint32_t j = sj + hw; j < ej; j += kXT / 16) {
           const uint4 rr = mt->rec[j];
           const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
           const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
@@ -673,7 +677,7 @@ __global__ void __launch_bounds__(256) raht_forward_kernel(
       // low-pass -> next phase's row pool, or -- when a single node is left -- the DC at output row 0
       {
         const uint32_t tot = nent * (uint32_t)cv;
-        for (uint32_t i = tid; i < tot; i += 256) {
+        for (uint32_t i = tid; i < tot; i += kXT) {
           const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
           const int c = (int)(i - k * (uint32_t)cv);
           const uint32_t d = s_dst[k];
@@ -700,8 +704,9 @@ __device__ __forceinline__ void dequant_row_inplace(float* row_s, int c, const Q
   if constexpr (VEC == 4) {
     const int4 q = reinterpret_cast<const int4*>(row_s)[c];
     const int amax = max(max(abs(q.x), abs(q.y)), max(abs(q.z), abs(q.w)));
+    const bool fast = bias == 0.0 && amax < (1 << 24);
     float4 y;
-    if (bias == 0.0 && amax < (1 << 24)) {
+    if (fast) {
       const float4 st = reinterpret_cast<const float4*>(qt.inv32)[c];
       y = make_float4(dequant_fast(q.x, st.x), dequant_fast(q.y, st.y), dequant_fast(q.z, st.z), dequant_fast(q.w, st.w));
     } else {
@@ -726,7 +731,7 @@ __device__ __forceinline__ void stage_row(float* row_s, const void* src_row, int
 }
 
 template <int VEC>
-__global__ void __launch_bounds__(256) raht_inverse_kernel(
+__global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
     const int32_t* __restrict__ in_q, const float* __restrict__ in_f, const uint32_t* __restrict__ weights,
     float* __restrict__ pool, const uint4* __restrict__ rec, const RahtTileHdr* __restrict__ hdr,
     RahtPlan* __restrict__ plan, int C, QStepParams qs, double bias, float* __restrict__ attr_out) {
@@ -743,7 +748,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int hw = tid >> 4, l16 = tid & 15;
   const int cv = C / VEC;
-  for (int c = tid; c < C; c += 256) { qt.inv64[c] = in_q ? (double)qs.step[c] : 0.0; qt.inv32[c] = in_q ? qs.step[c] : 0.f; }
+  for (int c = tid; c < C; c += kXT) { qt.inv64[c] = in_q ? (double)qs.step[c] : 0.0; qt.inv32[c] = in_q ? qs.step[c] : 0.f; }
   const uint32_t cv_magic = make_div_magic((uint32_t)(C / VEC));
   const void* coef = in_q ? (const void*)in_q : (const void*)in_f;       // both are 4-byte rows of C entries
   const uint32_t nph = plan->nphases;
@@ -769,7 +774,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
       TileMeta* mt = &s_meta[cur];
       const uint32_t nmerge = mt->hdr.nmerge, nseg = mt->hdr.nent >> 16;
       {
-        const uint32_t pm = mt->hdr.pendmask[warp];
+        const uint32_t pm = warp < 8 ? mt->hdr.pendmask[warp] : 0u;
         uint32_t before = 0;
 #pragma unroll
         for (int w = 0; w < 8; ++w) if (w < warp) before += __popc(mt->hdr.pendmask[w]);
@@ -781,7 +786,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
       // low-pass inputs from phase p+1's rows (or, when a single node is left, the DC = coefficient row 0)
       {
         const uint32_t tot = nent * (uint32_t)cv;
-        for (uint32_t i = tid; i < tot; i += 256) {
+        for (uint32_t i = tid; i < tot; i += kXT) {
           const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
           const uint32_t c = i - k * (uint32_t)cv;
           const uint32_t s = s_srcrow[k];
@@ -803,7 +808,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
       __syncthreads();
       if (in_q) {                                                          // de-quantise in place
         const uint32_t tot = nent * (uint32_t)cv;
-        for (uint32_t i = tid; i < tot; i += 256) {
+        for (uint32_t i = tid; i < tot; i += kXT) {
           const uint32_t k = div_cv(i, cv_magic, (uint32_t)cv);
           const uint32_t s = s_srcrow[k];
           if (!((s & 0x80000000u) && Mnext != 1u))
@@ -814,7 +819,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
       for (int s = (int)nseg - 1; s >= 0; --s) {                           // non-empty levels, top-down
         const uint32_t ej = mt->hdr.lev_end[s];
         const uint32_t sj = s > 0 ? mt->hdr.lev_end[s - 1] : 0u;
-        for (uint32_t j = sj + hw; j < ej; j += 16) {
+        for (uint32_t j = sj + hw; j < ej; j += kXT / 16) {
           const uint4 rr = mt->rec[j];
           const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
           const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
@@ -829,7 +834,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
         __syncthreads();
       }
       if (wts && __syncthreads_or((uint32_t)tid < nent && mt->w[tid] != 1u)) {   // [R2] a_i = x_i / sqrt(w_i)
-        for (uint32_t k = hw; k < nent; k += 16) {
+        for (uint32_t k = hw; k < nent; k += kXT / 16) {
           const uint32_t w = mt->w[k];
           if (w != 1u) {
             const double sw = 1.0 / sqrt((double)w);
@@ -843,7 +848,7 @@ __global__ void __launch_bounds__(256) raht_inverse_kernel(
         V* g = reinterpret_cast<V*>(dst + (size_t)ks * C);
         const V* s = reinterpret_cast<const V*>(s_rows);
         const uint32_t tot = nent * cv;
-        for (uint32_t i = tid; i < tot; i += 256) g[i] = s[i];
+        for (uint32_t i = tid; i < tot; i += kXT) g[i] = s[i];
       }
       cp_async_wait_all();                                                  // meta(next) before it is read
       __syncthreads();
@@ -917,10 +922,10 @@ int raht_setup(gsnfs_ctx* ctx) {
 }
 
 template <typename K>
-static int coop_grid(gsnfs_ctx* ctx, int slot, K kernel, size_t smem, uint32_t want, int* out) {
+static int coop_grid(gsnfs_ctx* ctx, int slot, K kernel, size_t smem, uint32_t want, int* out, int threads = 256) {
   int per_sm = ctx->occ_cache[slot];
   if (per_sm == 0 || ctx->occ_cache_smem[slot] != smem) {
-    GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, 256, smem));
+    GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
     ctx->occ_cache[slot] = per_sm;
     ctx->occ_cache_smem[slot] = smem;
   }
@@ -970,20 +975,20 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
                     (void*)&ctx->raht_plan, (void*)&channels, (void*)&qs, (void*)&has_q, (void*)&dz,
                     (void*)&d_out_q, (void*)&d_out_f};
     void* fn = vec4 ? (void*)raht_forward_kernel<4> : (void*)raht_forward_kernel<1>;
-    int rc = vec4 ? coop_grid(ctx, 1, raht_forward_kernel<4>, smem, want, &grid) : coop_grid(ctx, 2, raht_forward_kernel<1>, smem, want, &grid);
+    int rc = vec4 ? coop_grid(ctx, 1, raht_forward_kernel<4>, smem, want, &grid, kXT) : coop_grid(ctx, 2, raht_forward_kernel<1>, smem, want, &grid, kXT);
     if (rc != GSNFS_OK) return rc;
     GSNFS_KERNEL(ctx, st, "raht_forward");
-    GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, st));
+    GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(kXT), args, smem, st));
     GSNFS_LAUNCH_CHECK(ctx, st);
   } else {
     void* args[] = {(void*)&d_in_q, (void*)&d_in_f, (void*)&d_weights, (void*)&ctx->raht_rows, (void*)&ctx->raht_rec,
                     (void*)&ctx->raht_hdr, (void*)&ctx->raht_plan, (void*)&channels, (void*)&qs, (void*)&bias,
                     (void*)&d_out_f};
     void* fn = vec4 ? (void*)raht_inverse_kernel<4> : (void*)raht_inverse_kernel<1>;
-    int rc = vec4 ? coop_grid(ctx, 3, raht_inverse_kernel<4>, smem, want, &grid) : coop_grid(ctx, 4, raht_inverse_kernel<1>, smem, want, &grid);
+    int rc = vec4 ? coop_grid(ctx, 3, raht_inverse_kernel<4>, smem, want, &grid, kXT) : coop_grid(ctx, 4, raht_inverse_kernel<1>, smem, want, &grid, kXT);
     if (rc != GSNFS_OK) return rc;
     GSNFS_KERNEL(ctx, st, "raht_inverse");
-    GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(256), args, smem, st));
+    GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel(fn, dim3(grid), dim3(kXT), args, smem, st));
     GSNFS_LAUNCH_CHECK(ctx, st);
   }
   return GSNFS_OK;
