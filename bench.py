@@ -9,7 +9,8 @@ gsnfs_raht_inverse (decode).  `value` is whole-job Mgaussians/s with inputs resi
 same metric through the *_host ABI calls with pinned host buffers (H2D/D2H inside the timed region).
 Multi-GPU: frames are independent (intra-only codec) => replicas only, one frame stream per
 rank, no collective on the data path ("scaling": "weak").  `--impl reference` times the fp64 oracle on the
-host cores (a deliberately slow baseline, not the target).
+host cores (a deliberately slow baseline, not the target).  At N = 1 the line also carries `ladder`: the 300-frame
+dynamic sequence of BASELINE.json configs[4] encoded + decoded at 4 qstep rungs per frame (`--ladder-frames 0` skips it).
 """
 from __future__ import annotations
 
