@@ -29,7 +29,7 @@ extern "C" {
 #endif
 
 #define GSNFS_MAX_DEPTH 21
-#define GSNFS_MAX_CHANNELS 216
+#define GSNFS_MAX_CHANNELS 208   /* a 256-row tile of fp32 channels + its metadata must fit the 227 KB of shared memory per CTA */
 
 typedef enum gsnfs_status {
   GSNFS_OK = 0,

@@ -22,7 +22,7 @@ GSNFS_E_CAPACITY = -2
 GSNFS_E_CUDA = -3
 GSNFS_E_CORRUPT_STREAM = -4
 GSNFS_MAX_DEPTH = 21
-GSNFS_MAX_CHANNELS = 216
+GSNFS_MAX_CHANNELS = 208
 
 
 class GsnfsQuant(ctypes.Structure):

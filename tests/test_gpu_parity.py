@@ -469,3 +469,17 @@ def test_config5_dynamic_sequence_frames_all_rungs(B, ctx_big, t):
         ref_attr = orc.raht_inverse(orc.dequantize(q_ref, qstep), dk, ref["weights"], fr.depth)
         ch_range = (seq.qsteps[256].astype(np.float64) * 256)[None, :]
         assert np.all(np.abs(buf.dec_attr[:nv].cpu().numpy().astype(np.float64) - ref_attr) <= 1e-4 * ch_range)
+
+
+@pytest.mark.parametrize("channels", [208, 130, 60])
+def test_wide_rows_up_to_max_channels(B, channels):
+    """Channel counts beyond one float4 column per lane (C > 64) up to GSNFS_MAX_CHANNELS: one 256-row tile per SM."""
+    assert B.GSNFS_MAX_CHANNELS == 208
+    fr = synth.make_uniform_frame(3000, 6, channels, seed=5)
+    ctx = B.Context(max_points=fr.n, max_channels=channels, max_depth=fr.depth)
+    try:
+        full_pipeline_check(B, ctx, fr)
+    finally:
+        ctx.close()
+    with pytest.raises(B.GsnfsError):
+        B.Context(max_points=100, max_channels=B.GSNFS_MAX_CHANNELS + 1, max_depth=5)
