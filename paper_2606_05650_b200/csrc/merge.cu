@@ -45,7 +45,18 @@ __global__ void __launch_bounds__(256) merge_kernel(const float* __restrict__ at
         if (cnt > 1) {                           // rare: fp64 accumulation in sorted order, then mean
           if constexpr (VEC == 4) {
             double a0 = x[k].x, a1 = x[k].y, a2 = x[k].z, a3 = x[k].w;
-            for (uint32_t q = s[k] + 1; q < e[k]; ++q) {
+            uint32_t q = s[k] + 1;
+            for (; q + 4 <= e[k]; q += 4) {          // four rows in flight; the sums stay in sorted order
+              uint32_t g4[4];
+              float4 y4[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) g4[u] = perm[q + u];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) y4[u] = reinterpret_cast<const float4*>(attr + (size_t)g4[u] * C)[c];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { a0 += y4[u].x; a1 += y4[u].y; a2 += y4[u].z; a3 += y4[u].w; }
+            }
+            for (; q < e[k]; ++q) {
               const float4 y = reinterpret_cast<const float4*>(attr + (size_t)perm[q] * C)[c];
               a0 += y.x; a1 += y.y; a2 += y.z; a3 += y.w;
             }

@@ -625,7 +625,18 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
                 if constexpr (VEC == 4) {
                   const float4 x = r[c];
                   double a0 = x.x, a1 = x.y, a2 = x.z, a3 = x.w;
-                  for (uint32_t q = 1; q < w; ++q) {
+                  uint32_t q = 1;
+                  for (; q + 4 <= w; q += 4) {       // four rows in flight; the sums stay in sorted order
+                    uint32_t g4[4];
+                    float4 y4[4];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) g4[u] = ga.perm[s0 + q + u];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) y4[u] = reinterpret_cast<const float4*>(src + (size_t)g4[u] * C)[c];
+#pragma unroll
+                    for (int u = 0; u < 4; ++u) { a0 += y4[u].x; a1 += y4[u].y; a2 += y4[u].z; a3 += y4[u].w; }
+                  }
+                  for (; q < w; ++q) {
                     const float4 y = reinterpret_cast<const float4*>(src + (size_t)ga.perm[s0 + q] * C)[c];
                     a0 += y.x; a1 += y.y; a2 += y.z; a3 += y.w;
                   }
