@@ -550,8 +550,13 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
   __shared__ uint32_t s_dst[T];     // destination row: out row (finished) or pool row | 0x80000000 (pending)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int hw = tid >> 4, l16 = tid & 15;
   const int cv = C / VEC;
+  // lanes per row: the smallest power of two >= cv, at most 16 (C = 56: a half-warp per row; C = 3: four lanes per row,
+  // eight butterflies per warp step)
+  int lsh = 4;
+  while (lsh > 0 && (1 << (lsh - 1)) >= cv) --lsh;
+  const int lpr = 1 << lsh, nhw = kXT >> lsh;
+  const int hw = tid >> lsh, l16 = tid & (lpr - 1);
   for (int c = tid; c < C; c += kXT) {
     const double iv = has_q ? 1.0 / (double)qs.step[c] : 0.0;
     qt.inv64[c] = iv;
@@ -615,13 +620,13 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
       // [R2] x_i = sqrt(w_i) a_i: only rows with w != 1 need work (block-uniform test first)
       bool staged = false;             // a barrier has passed since the rows and s_dst were written
       if (wts && !(staged = !__syncthreads_or((uint32_t)tid < nent && mt->w[tid] != 1u))) {
-        for (uint32_t k = hw; k < nent; k += kXT / 16) {
+        for (uint32_t k = hw; k < nent; k += nhw) {
           const uint32_t w = mt->w[k];
           if (w != 1u) {
             V* r = reinterpret_cast<V*>(s_rows + (size_t)k * C);
             if (gsrc) {      // duplicate voxel: mean of its Gaussians, fp64 accumulation in sorted order [O9]
               const uint32_t s0 = ga.vstart[ks + k];
-              for (int c = l16; c < cv; c += 16) {
+              for (int c = l16; c < cv; c += lpr) {
                 if constexpr (VEC == 4) {
                   const float4 x = r[c];
                   double a0 = x.x, a1 = x.y, a2 = x.z, a3 = x.w;
@@ -650,7 +655,7 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
               }
             }
             const double sw = sqrt((double)w);
-            for (int c = l16; c < cv; c += 16) r[c] = vscale(r[c], sw);
+            for (int c = l16; c < cv; c += lpr) r[c] = vscale(r[c], sw);
           }
         }
       }
@@ -658,13 +663,13 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
       uint32_t sj = 0;
       for (uint32_t s = 0; s < nseg; ++s) {                               // non-empty levels, bottom-up
         const uint32_t ej = mt->hdr.lev_end[s];
-        for (uint32_t j = sj + hw; j < ej; j += kXT / 16) {
+        for (uint32_t j = sj + hw; j < ej; j += nhw) {
           const uint4 rr = mt->rec[j];
           const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
           const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
           V* r0 = reinterpret_cast<V*>(s_rows + (size_t)li * C);
           V* r1 = reinterpret_cast<V*>(s_rows + (size_t)k * C);
-          for (int c = l16; c < cv; c += 16) {
+          for (int c = l16; c < cv; c += lpr) {
             const V y0 = r0[c], y1 = r1[c];
             r0[c] = bf_lo(a, b, y0, y1);                                   // low-pass stays at the left index
             r1[c] = bf_hi(a, b, y0, y1);                                   // high-pass at the right index
@@ -732,16 +737,6 @@ __device__ __forceinline__ void dequant_row_inplace(float* row_s, int c, const Q
 }
 
 template <int VEC>
-__device__ __forceinline__ void stage_row(float* row_s, const void* src_row, int C, int l16) {
-  if constexpr (VEC == 4) {
-    for (int c = l16; c < C / 4; c += 16)
-      cp_async16(reinterpret_cast<float4*>(row_s) + c, reinterpret_cast<const float4*>(src_row) + c);
-  } else {
-    for (int c = l16; c < C; c += 16) cp_async4(row_s + c, reinterpret_cast<const float*>(src_row) + c);
-  }
-}
-
-template <int VEC>
 __global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
     const int32_t* __restrict__ in_q, const float* __restrict__ in_f, const uint32_t* __restrict__ weights,
     float* __restrict__ pool, const uint4* __restrict__ rec, const RahtTileHdr* __restrict__ hdr,
@@ -757,8 +752,13 @@ __global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
   __shared__ uint32_t s_srcrow[T];  // source row: coefficient row (finished) or pool row | 0x80000000 (pending)
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int hw = tid >> 4, l16 = tid & 15;
   const int cv = C / VEC;
+  // lanes per row: the smallest power of two >= cv, at most 16 (C = 56: a half-warp per row; C = 3: four lanes per row,
+  // eight butterflies per warp step)
+  int lsh = 4;
+  while (lsh > 0 && (1 << (lsh - 1)) >= cv) --lsh;
+  const int lpr = 1 << lsh, nhw = kXT >> lsh;
+  const int hw = tid >> lsh, l16 = tid & (lpr - 1);
   for (int c = tid; c < C; c += kXT) { qt.inv64[c] = in_q ? (double)qs.step[c] : 0.0; qt.inv32[c] = in_q ? qs.step[c] : 0.f; }
   const uint32_t cv_magic = make_div_magic((uint32_t)(C / VEC));
   const void* coef = in_q ? (const void*)in_q : (const void*)in_f;       // both are 4-byte rows of C entries
@@ -830,13 +830,13 @@ __global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
       for (int s = (int)nseg - 1; s >= 0; --s) {                           // non-empty levels, top-down
         const uint32_t ej = mt->hdr.lev_end[s];
         const uint32_t sj = s > 0 ? mt->hdr.lev_end[s - 1] : 0u;
-        for (uint32_t j = sj + hw; j < ej; j += kXT / 16) {
+        for (uint32_t j = sj + hw; j < ej; j += nhw) {
           const uint4 rr = mt->rec[j];
           const uint32_t k = rr.x & 0xffu, li = (rr.x >> 8) & 0xffu;
           const float a = __uint_as_float(rr.y), b = __uint_as_float(rr.z);
           V* r0 = reinterpret_cast<V*>(s_rows + (size_t)li * C);
           V* r1 = reinterpret_cast<V*>(s_rows + (size_t)k * C);
-          for (int c = l16; c < cv; c += 16) {
+          for (int c = l16; c < cv; c += lpr) {
             const V y0 = r0[c], y1 = r1[c];
             r0[c] = bf_hi(a, b, y1, y0);          // a*y0 - b*y1  (A.6 l.37)
             r1[c] = bf_lo(b, a, y0, y1);          // b*y0 + a*y1  (A.6 l.38)
@@ -845,12 +845,12 @@ __global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
         __syncthreads();
       }
       if (wts && __syncthreads_or((uint32_t)tid < nent && mt->w[tid] != 1u)) {   // [R2] a_i = x_i / sqrt(w_i)
-        for (uint32_t k = hw; k < nent; k += kXT / 16) {
+        for (uint32_t k = hw; k < nent; k += nhw) {
           const uint32_t w = mt->w[k];
           if (w != 1u) {
             const double sw = 1.0 / sqrt((double)w);
             V* r = reinterpret_cast<V*>(s_rows + (size_t)k * C);
-            for (int c = l16; c < cv; c += 16) r[c] = vscale(r[c], sw);
+            for (int c = l16; c < cv; c += lpr) r[c] = vscale(r[c], sw);
           }
         }
         __syncthreads();
