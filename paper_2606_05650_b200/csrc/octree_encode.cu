@@ -50,16 +50,30 @@ __global__ void __launch_bounds__(256) voxelize_kernel(const float* __restrict__
   __shared__ uint32_t s_hist[kSortMaxPasses][256];
   for (int i = threadIdx.x; i < kSortMaxPasses * 256; i += 256) (&s_hist[0][0])[i] = 0;
   __syncthreads();
-  for (uint32_t i = blockIdx.x * 256 + threadIdx.x; i < n; i += gridDim.x * 256) {
-    const float px = xyz[3 * (size_t)i], py = xyz[3 * (size_t)i + 1], pz = xyz[3 * (size_t)i + 2];
-    const uint32_t vx = voxel_coord(px, vp.lo[0], vp.scale[0], vp.vmax);
-    const uint32_t vy = voxel_coord(py, vp.lo[1], vp.scale[1], vp.vmax);
-    const uint32_t vz = voxel_coord(pz, vp.lo[2], vp.scale[2], vp.vmax);
-    const uint64_t key = spread3(vx) | (spread3(vy) << 1) | (spread3(vz) << 2);
-    keys[i] = (KeyT)key;
-    for (int p = 0; p < plan.passes; ++p) {
-      const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
-      atomicAdd(&s_hist[p][d], 1u);
+  const uint32_t stride = gridDim.x * 256u;
+  for (uint32_t i0 = blockIdx.x * 256 + threadIdx.x; i0 < n; i0 += 4u * stride) {
+    float px[4], py[4], pz[4];                      // four points per thread in flight (the loads are the latency)
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t i = i0 + (uint32_t)u * stride;
+      const bool ok = i < n && i >= i0;
+      px[u] = ok ? xyz[3 * (size_t)i] : 0.f;
+      py[u] = ok ? xyz[3 * (size_t)i + 1] : 0.f;
+      pz[u] = ok ? xyz[3 * (size_t)i + 2] : 0.f;
+    }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) {
+      const uint32_t i = i0 + (uint32_t)u * stride;
+      if (i >= n || i < i0) continue;
+      const uint32_t vx = voxel_coord(px[u], vp.lo[0], vp.scale[0], vp.vmax);
+      const uint32_t vy = voxel_coord(py[u], vp.lo[1], vp.scale[1], vp.vmax);
+      const uint32_t vz = voxel_coord(pz[u], vp.lo[2], vp.scale[2], vp.vmax);
+      const uint64_t key = spread3(vx) | (spread3(vy) << 1) | (spread3(vz) << 2);
+      keys[i] = (KeyT)key;
+      for (int p = 0; p < plan.passes; ++p) {
+        const uint32_t d = (uint32_t)(key >> plan.shift[p]) & ((1u << plan.bits[p]) - 1u);
+        atomicAdd(&s_hist[p][d], 1u);
+      }
     }
   }
   __syncthreads();
