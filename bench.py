@@ -269,10 +269,13 @@ def run_ours(args, rank, world, local_rank):
                          "alg_GBps": round(b / (avg_us * 1e-6) / 1e9, 1) if b else None}
     dom = max((k for k in kernels if ab.get(k)), key=lambda k: kernels[k]["ms_per_step"])
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "dram_traffic.json")
+    tpath = os.path.join(ROOT, "profiles", "r1_dram_traffic.csv")       # ncu dram bytes per launch (profiles/r1_dram_traffic.md)
     if os.path.exists(tpath):
         try:
-            traffic = json.load(open(tpath)).get(f"config{args.config}", {}).get(dom)
+            for line in open(tpath).read().splitlines()[1:]:
+                cfg, kname, nbytes = line.split(",")
+                if cfg == f"config{args.config}" and kname == dom and args.n_override is None:
+                    traffic = int(nbytes)
         except Exception:
             traffic = None
     roofline = {"bound": "hbm", "kernel": dom, "achieved": kernels[dom]["alg_GBps"], "peak": peak, "unit": "GB/s",
