@@ -89,7 +89,6 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
   const size_t o_rplan = b.take(sizeof(RahtPlan));
   const size_t o_rrows = b.take(c->raht_pool_rows * (size_t)C * 4);
-  const size_t o_dscan = b.take(256);
   const size_t o_dpar = b.take((c->occ_cap + N + 2) * 4), o_dkm = b.take((N + 1) * 8);
   c->pool_bytes = b.off;
   GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->pool, c->pool_bytes));
@@ -104,9 +103,9 @@ static int create_impl(gsnfs_ctx* c) {
   c->raht_rec = (uint4*)(p + o_rrec); c->raht_gsrc = (uint32_t*)(p + o_rgs);
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
-  c->dec_scan = (uint32_t*)(p + o_dscan); c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);
+  c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);
   GSNFS_CUDA_OK(c, cudaMemset(c->pool, 0, o_rrows));     // everything but the big row pool ...
-  GSNFS_CUDA_OK(c, cudaMemset(p + o_dscan, 0, c->pool_bytes - o_dscan));   // ... and the decoder's scan / parent arrays
+  GSNFS_CUDA_OK(c, cudaMemset(p + o_dpar, 0, c->pool_bytes - o_dpar));   // ... and the decoder's parent / middle-level arrays
   int rc = octree_encode_setup(c);
   if (rc != GSNFS_OK) return rc;
   return raht_setup(c);

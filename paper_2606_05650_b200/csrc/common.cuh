@@ -111,7 +111,6 @@ struct gsnfs_ctx {
   size_t occ_cache_smem[16];
 
   // decode
-  uint32_t* dec_scan;      // (unused)
   uint64_t* dec_kmid;      // Morton codes of the decoder's middle level (max_points + 1 entries)
   uint32_t* dec_parent;    // (parent stream index << 3 | child digit) of every breadth-first node: occ_cap + max_points + 2
   uint64_t occ_cap;
