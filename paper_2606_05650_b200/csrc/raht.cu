@@ -50,6 +50,16 @@ __device__ __forceinline__ void prefetch_row_l2(const float* row, int C) {
   for (const char* q = (const char*)((uintptr_t)b & ~(uintptr_t)127); q <= e; q += 128) prefetch_l2(q);
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// ---- TMA 1-D bulk store of a finished tile (rows are 16-byte multiples when C % 4 == 0) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
+__device__ __forceinline__ void fence_proxy_async_all() { asm volatile("fence.proxy.async;" ::: "memory"); }
+__device__ __forceinline__ void bulk_s2g(void* dst, uint32_t src, uint32_t bytes) {
+  asm volatile("cp.async.bulk.global.shared::cta.bulk_group [%0], [%1], %2;" ::"l"(dst), "r"(src), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
+__device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 __device__ __forceinline__ uint32_t lower_bound_u64(const uint64_t* a, uint32_t lo, uint32_t hi, uint64_t x) {
@@ -855,17 +865,31 @@ __global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
         }
         __syncthreads();
       }
-      {
+      if constexpr (VEC == 4) {        // the tile's rows are contiguous in dst: one TMA bulk store
+        fence_proxy_async();           // this thread's writes to the staged rows -> visible to the async proxy
+        cp_async_wait_all();           // meta(next) before it is read
+        __syncthreads();
+        if (tid == 0) {
+          bulk_s2g(dst + (size_t)ks * C, smem_u32(s_rows), nent * (uint32_t)C * 4u);
+          bulk_commit();
+          bulk_wait_read();            // the rows have left shared memory: the next tile may be staged over them
+        }
+      } else {
         V* g = reinterpret_cast<V*>(dst + (size_t)ks * C);
         const V* s = reinterpret_cast<const V*>(s_rows);
         const uint32_t tot = nent * cv;
         for (uint32_t i = tid; i < tot; i += kXT) g[i] = s[i];
+        cp_async_wait_all();                                                // meta(next) before it is read
       }
-      cp_async_wait_all();                                                  // meta(next) before it is read
       __syncthreads();
       cur ^= 1;
     }
-    if (p > 1) grid.sync();
+    if (p > 1) {
+      if constexpr (VEC == 4) {        // pool rows written by the async proxy: complete and ordered before the grid barrier
+        if (tid == 0) { bulk_wait_all(); fence_proxy_async_all(); }
+      }
+      grid.sync();
+    }
     if (blockIdx.x == 0 && tid == 0) plan->t_xform[p] = globaltimer_ns();
   }
 }
