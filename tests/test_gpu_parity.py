@@ -381,6 +381,14 @@ def test_config4_large_position_exact_and_raht_properties(B, ctx_big):
     assert torch.equal(buf.dec_keys[:nv], buf.voxel_keys[:nv])
     dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], fr.depth)
     assert np.array_equal(buf.dec_xyz[:nv].cpu().numpy().astype(np.uint64), dc)
+    # the transform is orthonormal on sqrt(w)-scaled rows, so the reconstruction error has the quantisation error's
+    # norm: per channel, rms(sqrt(w) (decoded - merged)) <= (1 - f) qstep with f = 1/3, and no single coefficient
+    # error (hence no single attribute error times sqrt(w)) exceeds sqrt(N_v) times that
+    err = (buf.dec_attr[:nv].double() - merged) * torch.sqrt(w)[:, None]
+    qs = torch.from_numpy(fr.qstep.astype(np.float64)).to(DEV)
+    rms = torch.sqrt((err ** 2).mean(0))
+    assert torch.all(rms <= (2.0 / 3.0) * qs * (1 + 1e-3) + 1e-7), (rms / qs).max().item()
+    assert torch.all(rms >= 0.05 * qs)                     # and it is a quantised signal, not a copy
 
 
 def test_host_frame_calls_roundtrip(B, ctx_small):
