@@ -491,3 +491,31 @@ def test_wide_rows_up_to_max_channels(B, channels):
         ctx.close()
     with pytest.raises(B.GsnfsError):
         B.Context(max_points=100, max_channels=B.GSNFS_MAX_CHANNELS + 1, max_depth=5)
+
+
+def test_non_finite_positions_do_not_crash(B, ctx_small):
+    """gsnfs.h: non-finite positions are the caller's error -- the voxel they land in is unspecified, but the call must
+    not fail or write out of bounds, the finite points must keep a valid stream, and decode(encode) must still close."""
+    fr = synth.make_frame(1, n_override=5000)
+    xyz = fr.xyz.copy()
+    xyz[7] = [np.nan, 0.5, 0.5]
+    xyz[100] = [np.inf, -np.inf, 0.25]
+    xyz[4321] = [0.1, np.nan, np.inf]
+    bad = synth.Frame(name="nonfinite", xyz=xyz, attr=fr.attr, qstep=fr.qstep, depth=fr.depth, qdiv=fr.qdiv,
+                      bbox_min=fr.bbox_min, bbox_max=fr.bbox_max)
+    buf, got = gpu_position_encode(B, ctx_small, bad)
+    nv = got["n_voxels"]
+    assert 0 < nv <= bad.n and got["status"] == 0
+    assert np.all(got["occ"] != 0) and int(got["level_sizes"][0]) == 1 and int(got["level_sizes"][bad.depth]) == nv
+    assert sorted(got["perm"].tolist()) == list(range(bad.n))
+    keys = got["voxel_keys"]
+    assert np.all(keys[1:] > keys[:-1]) and int(keys[-1]) < (1 << (3 * bad.depth))
+    # the finite points land exactly where the oracle puts them
+    fin = np.isfinite(xyz).all(axis=1)
+    ref_keys = orc.morton_encode(orc.voxelize(xyz[fin], bad.bbox_min, bad.bbox_max, bad.depth), bad.depth)
+    assert set(np.unique(ref_keys).tolist()) <= set(keys.tolist())
+    B.gsnfs_octree_decode(ctx_small, buf.occ, got["occ_bytes"], got["level_sizes"], bad.depth, buf.dec_xyz, buf.dec_keys,
+                          buf.dec_counts)
+    torch.cuda.synchronize()
+    assert int(buf.dec_counts.cpu()[2]) == 0
+    assert np.array_equal(buf.dec_keys[:nv].cpu().numpy().astype(np.uint64), keys)
