@@ -100,7 +100,8 @@ template <typename KeyT>
 __device__ __forceinline__ uint32_t sort_load_rank(const KeyT* __restrict__ keys_in, const uint32_t* __restrict__ pay_in,
                                                    uint32_t base, uint32_t cnt, int ipt, int shift, uint32_t mask, bool want_pay,
                                                    KeyT (&key)[kSortItems], uint32_t (&pay)[kSortItems],
-                                                   uint32_t (&rank)[kSortItems], uint32_t (*s_whist)[257]) {
+                                                   uint32_t (&rank)[kSortItems], uint32_t (*s_whist)[257],
+                                                   uint32_t (*s_match)[8][257]) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   for (int i = tid; i < 8 * 257; i += kSortThreads) (&s_whist[0][0])[i] = 0;
   const uint32_t lbase = (uint32_t)(warp * ipt * 32 + lane);
@@ -115,26 +116,28 @@ __device__ __forceinline__ uint32_t sort_load_rank(const KeyT* __restrict__ keys
     if (want_pay) pay[j] = valid ? (pay_in ? __ldcg(pay_in + idx) : idx) : 0xffffffffu;
   }
   __syncthreads();
-  // lanes holding the same digit, found with one ballot per digit bit (9 bits: bit 8 marks tail padding):
-  // a fixed ~27 instructions per key, where the hardware match.any serialises over the distinct values
+  // lanes holding the same digit: every lane ORs its bit into a per-warp, per-digit mask in shared memory and reads the
+  // mask back (bin 256 collects the tail padding); the group's lowest lane clears the mask again.  Two mask sets used
+  // alternately, so the clear of item j cannot race with the OR of item j + 1.  ~8 instructions per key where the
+  // ballot-per-digit-bit version needed 27 (and the hardware match.any serialises over the distinct values).
   unsigned peers[kSortItems];
 #pragma unroll
   for (int j = 0; j < kSortItems; ++j) {
     if (j < ipt) {                                           // warp-uniform
       const bool valid = (vmask >> j) & 1u;
       const uint32_t d = valid ? ((uint32_t)(key[j] >> shift) & mask) : 256u;
-      unsigned m = 0xffffffffu;
-#pragma unroll
-      for (int b = 0; b < 9; ++b) {
-        const bool bit = (d >> b) & 1u;
-        const unsigned v = __ballot_sync(0xffffffffu, bit);
-        m &= bit ? v : ~v;
-      }
+      volatile uint32_t* mm = &s_match[j & 1][warp][d];
+      atomicOr(const_cast<uint32_t*>(mm), 1u << lane);
+      __syncwarp();
+      const unsigned m = *mm;
+      __syncwarp();
+      if ((m & lanemask_lt()) == 0u) *mm = 0u;
       peers[j] = m;
     } else {
       peers[j] = 0xffffffffu;
     }
   }
+  __syncwarp();
   // per-warp digit counters: the leader of every peer group adds the group size (shared-memory atomics of
   // one warp execute in program order, so earlier items get the lower ranks) and broadcasts the old value
 #pragma unroll
@@ -168,12 +171,14 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
   KeyT* s_keys = reinterpret_cast<KeyT*>(s_dyn);
   uint32_t* s_pay = reinterpret_cast<uint32_t*>(s_dyn + sizeof(KeyT) * kSortTile);
   __shared__ uint32_t s_whist[8][257];
+  __shared__ uint32_t s_match[2][8][257];    // peer masks of the ranking step; all zero between uses (the group leaders clear them)
   __shared__ uint32_t s_dstart[256];
   __shared__ uint32_t s_goff[256];
   __shared__ uint32_t s_scan[9];
   __shared__ uint32_t s_gbase[kSortMaxPasses][256];   // exclusive scan of every pass's global digit histogram
 
   const int tid = threadIdx.x, warp = tid >> 5;
+  for (int i = tid; i < 2 * 8 * 257; i += kSortThreads) (&s_match[0][0][0])[i] = 0;   // (a block barrier precedes the first use)
   const uint32_t ngroups = (ntiles + kSortGroup - 1) / kSortGroup;
   const bool single = ntiles <= gridDim.x;          // one tile per CTA: registers survive the barrier
   KeyT key[kSortItems];
@@ -202,7 +207,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
     // ---- phase A: digit counts of every tile -> tile_hist, group sums
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       vmask = sort_load_rank<KeyT>(kin, pin, tile * tstride, min(tstride, n - tile * tstride), ipt, shift, mask, single,
-                                   key, pay, rank, s_whist);
+                                   key, pay, rank, s_whist, s_match);
       uint32_t count = 0;
 #pragma unroll
       for (int w = 0; w < 8; ++w) count += s_whist[w][tid];
@@ -221,7 +226,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
     for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
       const uint32_t base = tile * tstride;
       const uint32_t cnt = min(tstride, n - base);
-      if (!single) vmask = sort_load_rank<KeyT>(kin, pin, base, cnt, ipt, shift, mask, true, key, pay, rank, s_whist);
+      if (!single) vmask = sort_load_rank<KeyT>(kin, pin, base, cnt, ipt, shift, mask, true, key, pay, rank, s_whist, s_match);
       // thread d: exclusive prefix over warps of digit d; tile count of digit d
       uint32_t count = 0;
 #pragma unroll
