@@ -140,7 +140,12 @@ int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream,
  *   saturated to int32, evaluated in fp64 from the fp32 coefficient.  d_coeff (unquantised fp32) and
  *   d_qcoeff may each be NULL, not both; d_qcoeff requires qstep.
  * n_voxels is the row count; if d_counts != NULL the actual N_v is read on the device from it and
- * n_voxels is only an upper bound (rows beyond N_v are untouched). */
+ * n_voxels is only an upper bound (rows beyond N_v are untouched).
+ * Schedule reuse: the prelude (sibling pairs, weights, a/b factors: Alg. A.4/A.5) depends on the codes and leaf weights
+ * only.  d_voxel_keys == NULL in gsnfs_raht_forward / gsnfs_raht_inverse means "the same voxel list and weights as the
+ * previous gsnfs_raht_* / gsnfs_merge_raht_forward call on this context, with the same n_voxels": the prelude is skipped
+ * (one rung more of a bitrate ladder costs the transform only).  d_weights must still be passed if it was then.
+ * GSNFS_E_INVALID_ARGUMENT if the context holds no schedule of n_voxels rows; other mismatches are the caller's error. */
 int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
                        const uint64_t* d_voxel_keys, const uint32_t* d_weights, uint64_t n_voxels,
                        const gsnfs_counts* d_counts, int depth,

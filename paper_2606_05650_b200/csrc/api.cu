@@ -246,7 +246,8 @@ int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_oc
 }
 
 static int raht_check(gsnfs_ctx* ctx, const uint64_t* keys, uint64_t n, int depth, int channels) {
-  if (!ctx || (n && !keys)) return GSNFS_E_INVALID_ARGUMENT;
+  if (!ctx) return GSNFS_E_INVALID_ARGUMENT;
+  if (n && !keys && ctx->sched_n != n) return GSNFS_E_INVALID_ARGUMENT;      // NULL keys: reuse needs a schedule of n rows
   if (depth < 1 || depth > GSNFS_MAX_DEPTH || channels < 1 || channels > GSNFS_MAX_CHANNELS || n >= (1ull << 30))
     return GSNFS_E_INVALID_ARGUMENT;
   if (n > ctx->max_points || channels > ctx->max_channels) return GSNFS_E_CAPACITY;

@@ -104,6 +104,7 @@ struct gsnfs_ctx {
   gsnfs::RahtPlan* raht_plan;
   float* raht_rows;        // pending-row pool (phases >= 2)
   uint64_t raht_pool_rows; // capacity (rows) of raht_idx / raht_rows
+  uint64_t sched_n;        // row count of the schedule currently held in raht_rec / raht_hdr / raht_plan (0 = none)
   uint64_t raht_rec_cap;
   uint64_t raht_hdr_cap;
   float* qparams;          // 2 x max_channels doubles (inv step / step) stored as double

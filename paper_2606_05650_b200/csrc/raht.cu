@@ -987,8 +987,8 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   if (fused) d_weights = d_weights_out;        // the transform kernels read the run lengths the schedule writes
   GatherArgs ga;
   ga.gsrc = fused ? ctx->raht_gsrc : nullptr; ga.perm = d_perm; ga.vstart = d_vstart;
-  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
-  {
+  if (d_keys) {                                  // NULL: the schedule of the previous call on this context is reused
+    GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
     int grid = 0;
     int rc = coop_grid(ctx, 0, raht_schedule_kernel, 0, want, &grid);
     if (rc != GSNFS_OK) return rc;
@@ -996,6 +996,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
     GSNFS_KERNEL(ctx, st, "raht_schedule");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)raht_schedule_kernel, dim3(grid), dim3(256), args, 0, st));
     GSNFS_LAUNCH_CHECK(ctx, st);
+    ctx->sched_n = n_voxels;
   }
   QStepParams qs;
   for (int c = 0; c < GSNFS_MAX_CHANNELS; ++c) qs.step[c] = (qstep && c < channels) ? qstep[c] : 1.0f;

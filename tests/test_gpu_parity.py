@@ -519,3 +519,31 @@ def test_non_finite_positions_do_not_crash(B, ctx_small):
     torch.cuda.synchronize()
     assert int(buf.dec_counts.cpu()[2]) == 0
     assert np.array_equal(buf.dec_keys[:nv].cpu().numpy().astype(np.uint64), keys)
+
+
+def test_schedule_reuse_with_null_keys(B, ctx_small):
+    """gsnfs.h: d_voxel_keys == NULL reuses the schedule of the previous RAHT call on the context -- same result bit for
+    bit; without a schedule of that row count the call is refused."""
+    fr = synth.make_dense_frame(20_000, 6, 56)
+    buf, got = gpu_position_encode(B, ctx_small, fr)
+    nv = got["n_voxels"]
+    d_attr = _t(fr.attr)
+    B.gsnfs_voxel_merge(ctx_small, d_attr, fr.channels, fr.n, buf.perm, buf.voxel_start, buf.counts, buf.merged, buf.weights)
+    q1 = torch.empty((fr.n, fr.channels), dtype=torch.int32, device=DEV)
+    q2 = torch.empty_like(q1)
+    qs2 = (fr.qstep * 4).astype(np.float32)
+    B.gsnfs_raht_forward(ctx_small, buf.voxel_keys, buf.weights, nv, None, fr.depth, buf.merged, fr.channels, fr.qstep, None, q1, None)
+    B.gsnfs_raht_forward(ctx_small, None, buf.weights, nv, None, fr.depth, buf.merged, fr.channels, qs2, None, q2, None)
+    ref2 = torch.empty_like(q1)
+    B.gsnfs_raht_forward(ctx_small, buf.voxel_keys, buf.weights, nv, None, fr.depth, buf.merged, fr.channels, qs2, None, ref2, None)
+    torch.cuda.synchronize()
+    assert torch.equal(q2[:nv], ref2[:nv])
+    a1 = torch.empty((fr.n, fr.channels), dtype=torch.float32, device=DEV)
+    a2 = torch.empty_like(a1)
+    B.gsnfs_raht_inverse(ctx_small, buf.voxel_keys, buf.weights, nv, None, fr.depth, q1, None, fr.channels, fr.qstep, None, a1)
+    B.gsnfs_raht_inverse(ctx_small, None, buf.weights, nv, None, fr.depth, q1, None, fr.channels, fr.qstep, None, a2)
+    torch.cuda.synchronize()
+    assert torch.equal(a1[:nv], a2[:nv])
+    with pytest.raises(B.GsnfsError) as e:
+        B.gsnfs_raht_inverse(ctx_small, None, buf.weights, nv - 1, None, fr.depth, q1, None, fr.channels, fr.qstep, None, a2)
+    assert e.value.status == B.GSNFS_E_INVALID_ARGUMENT
