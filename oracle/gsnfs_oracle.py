@@ -18,13 +18,15 @@ Pins (tests/test_oracle_*.py, all `-m "not gpu"`):
                            pointer octree (PAPER.md:L97); Fig. 2/3 stream (tests/golden/fig2_stream.txt);
                            full cube; single point; popcount invariants; decode(encode(P))
   merge_attributes         python-loop mean; single-Gaussian voxels copied exactly
+  raht_coefficient_closed_form   the level-synchronous raht_forward on random sparse voxel sets (every row)
   raht_*                   Eq. (1) two-voxel closed form; explicit orthonormal matrix built from the
                            Morton-prefix ranges; DC = sum(w a)/sqrt(W); Parseval; constant signal;
                            dense separable 3-D Haar on a full cube (PAPER.md:L219 fn. 4);
                            duplicates-expanded equivalence [R2]; perfect reconstruction; linearity
   quantize / dequantize    PARITY UNPINNED by the paper [R10]: it gives only the name "dead-zone
                            quantization" and omits de-quantisation (L259).  Pinned
-                           only to self-consistency properties (dead zone, error bound, symmetry).
+                           only to self-consistency properties (dead zone, error bound, symmetry) and
+                           hand-computed values (quantize at f = 1/3; dequantize with delta = 0 and 0.25).
 """
 from __future__ import annotations
 
@@ -295,6 +297,36 @@ def raht_inverse(Y, M, leaf_w, J):
     return Y / np.sqrt(w)[:, None]
 
 
+def raht_coefficient_closed_form(A, M, leaf_w, rows):
+    """Second, independent definition of single RAHT coefficients (no level loop, no active lists): the
+    closed form that follows from Eq. (1) and the run-length weights / sibling test of
+    Alg. A.4 l.8-10 (L741-747) by induction over the levels.  For row i > 0 let h = msb(M[i-1] xor M[i]);
+    voxel i becomes a right sibling at level h + 1, the right node is S1 = {j : M[j] >> h == M[i] >> h} =
+    [i, r), the left node S0 = {j : M[j] >> (h+1) == M[i] >> (h+1), bit h of M[j] = 0} = [l, i).  A node's
+    low-pass value is T_S / sqrt(W_S) with W_S = sum of leaf weights and T_S = sum of w_j a_j ([R2]:
+    sqrt(w_j) x_j), hence
+        Y[i] = sqrt(W0/(W0+W1)) T_S1/sqrt(W1) - sqrt(W1/(W0+W1)) T_S0/sqrt(W0),   Y[0] = T_all/sqrt(W_all).
+    Used to check sampled coefficients at sizes where the level-synchronous oracle is too slow.
+    Returns an array len(rows) x C (fp64)."""
+    A = np.asarray(A)
+    M = np.asarray(M, dtype=U64)
+    w = np.asarray(leaf_w, dtype=np.float64)
+    out = np.empty((len(rows), A.shape[1]), dtype=np.float64)
+    for n, i in enumerate(rows):
+        i = int(i)
+        if i == 0:
+            out[n] = (w[:, None] * A.astype(np.float64)).sum(0) / np.sqrt(w.sum())
+            continue
+        h = int(M[i] ^ M[i - 1]).bit_length() - 1
+        l = int(np.searchsorted(M, (M[i] >> U64(h + 1)) << U64(h + 1), side="left"))
+        r = int(np.searchsorted(M, ((M[i] >> U64(h)) + U64(1)) << U64(h), side="left"))
+        W0, W1 = w[l:i].sum(), w[i:r].sum()
+        T0 = (w[l:i, None] * A[l:i].astype(np.float64)).sum(0)
+        T1 = (w[i:r, None] * A[i:r].astype(np.float64)).sum(0)
+        out[n] = np.sqrt(W0 / (W0 + W1)) * T1 / np.sqrt(W1) - np.sqrt(W1 / (W0 + W1)) * T0 / np.sqrt(W0)
+    return out
+
+
 # ---------------------------------------------------------------------------------------------
 # Dead-zone quantiser (PAPER.md:L255; de-quantisation omitted by the paper, L259).
 # PARITY UNPINNED [R10]: q = sign(y) floor(|y|/D + f), y^ = sign(q) (|q| + delta [q != 0]) D,
@@ -306,9 +338,13 @@ _I32_MAX = np.float64(2**31 - 1)
 
 
 def quantize(Y, qstep, dz_round=DZ_ROUND_DEFAULT):
+    """q = sign(y) floor(|y| (1/D) + f) [R10].  The integer decision is taken in the arithmetic gsnfs.h states
+    (the kernel's, since the paper fixes none): 1/D rounded once to fp64, the product rounded once, the sum
+    rounded once (no fused multiply-add), then floor."""
     Y = np.asarray(Y, dtype=np.float64)
     step = np.asarray(qstep, dtype=np.float32).astype(np.float64)[None, :]
-    mag = np.floor(np.abs(Y) / step + np.float64(dz_round))
+    inv = np.float64(1.0) / step
+    mag = np.floor(np.abs(Y) * inv + np.float64(dz_round))
     mag = np.minimum(mag, _I32_MAX)                        # saturate to int32
     return (np.sign(Y) * mag).astype(np.int64)
 

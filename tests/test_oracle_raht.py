@@ -227,3 +227,64 @@ def test_quantiser_self_consistency(f):
         got = orc.quantize(yy, np.array([0.5], np.float32), f)[:, 0].tolist()
         assert got == [0, 0, 1, -1, 2, -3]
     assert orc.quantize(np.array([[1e30]]), np.array([1.0], np.float32), f)[0, 0] == 2**31 - 1
+
+
+def test_dequantize_hand_values_and_bias_gating():
+    """[R10] y^ = sign(q) (|q| + delta [q != 0]) D.  Hand-computed: D = 0.5, delta = 0.25: q = +-3 -> +-1.625,
+    q = +-1 -> +-0.625, q = 0 -> 0 whatever delta; delta = 0: q = +-3 -> +-1.5.  A wrong sign of delta, a missing
+    (q != 0) gate or a bias applied after the multiplication each fail one of these."""
+    step = np.array([0.5], np.float32)
+    q = np.array([[0], [3], [-3], [1], [-1]])
+    assert orc.dequantize(q, step, 0.25)[:, 0].tolist() == [0.0, 1.625, -1.625, 0.625, -0.625]
+    assert orc.dequantize(q, step, 0.0)[:, 0].tolist() == [0.0, 1.5, -1.5, 0.5, -0.5]
+    assert orc.dequantize(q, step)[:, 0].tolist() == [0.0, 1.5, -1.5, 0.5, -0.5]            # default delta = 0
+    # per-channel steps, and the bias moves every non-zero magnitude by exactly delta * D towards larger |y|
+    rng = np.random.default_rng(3)
+    qq = rng.integers(-50, 51, (200, 3))
+    st = np.array([0.25, 1.0, 3.0], np.float32)
+    d0, d1 = orc.dequantize(qq, st, 0.0), orc.dequantize(qq, st, 0.375)
+    assert np.array_equal(d1 - d0, np.sign(qq) * 0.375 * st.astype(np.float64)[None, :])
+    assert np.array_equal(d0, qq * st.astype(np.float64)[None, :])
+    # round trip: quantise at f, reconstruct at delta = 1/2 - f lands mid-way in the decision interval of |q| >= 1
+    f = 0.25
+    y = np.array([[0.7], [1.2], [-2.6]])
+    qy = orc.quantize(y, np.array([1.0], np.float32), f)
+    assert qy[:, 0].tolist() == [0, 1, -2]
+    assert orc.dequantize(qy, np.array([1.0], np.float32), 0.5 - f)[:, 0].tolist() == [0.0, 1.25, -2.25]
+
+
+def test_quantize_reciprocal_arithmetic():
+    """gsnfs.h states the arithmetic of the integer decision: floor(|y| * (1/D) + f), every operation rounded once in
+    fp64.  Check against exact rational arithmetic away from the decision boundaries, and that it is the reciprocal
+    form (not the division) at a value where the two differ."""
+    from fractions import Fraction
+    rng = np.random.default_rng(12)
+    step = np.array([0.1, 1.0 / 3.0, 7.0], np.float32)
+    Y = rng.normal(0, 20, (4000, 3))
+    q = orc.quantize(Y, step, 1.0 / 3.0)
+    for (r, c) in rng.integers(0, [4000, 3], (300, 2)).tolist():
+        t = abs(Fraction(float(Y[r, c]))) / Fraction(float(step[c])) + Fraction(1.0 / 3.0)
+        if abs(t - round(t)) > Fraction(1, 10**9):                       # away from a boundary both forms agree with exact
+            assert abs(int(q[r, c])) == int(t // 1) and np.sign(q[r, c]) == np.sign(Y[r, c]) * (int(t // 1) > 0)
+    # search a point where floor(|y| / D + f) and floor(|y| * (1/D) + f) differ; the oracle must follow the reciprocal form
+    D = np.float64(np.float32(0.1))
+    inv = 1.0 / D
+    k = np.arange(1, 200000, dtype=np.float64)
+    y = k * D                                                            # |y| / D is k or k -+ 1 ulp
+    a, b = np.floor(y / D), np.floor(y * inv)
+    diff = np.flatnonzero(a != b)
+    if diff.size:
+        yy = y[diff[:50], None]
+        assert np.array_equal(orc.quantize(yy, np.array([0.1], np.float32), 0.0)[:, 0], b[diff[:50]].astype(np.int64))
+
+
+@pytest.mark.parametrize("J,nv,seed,weighted", [(3, 40, 1, False), (4, 300, 2, True), (7, 1500, 3, True), (2, 9, 4, True)])
+def test_closed_form_coefficients_equal_level_synchronous(J, nv, seed, weighted):
+    """raht_coefficient_closed_form (Morton-prefix ranges, no level loop) == raht_forward (Alg. A.4 + A.6) on every row."""
+    rng = np.random.default_rng(seed)
+    M = _random_voxels(rng, J, nv)
+    w = rng.integers(1, 9, len(M)) if weighted else np.ones(len(M), np.int64)
+    A = rng.normal(0, 1, (len(M), 3))
+    Y = orc.raht_forward(A, M, w, J)
+    Z = orc.raht_coefficient_closed_form(A, M, w, np.arange(len(M)))
+    assert np.allclose(Y, Z, atol=1e-11)
