@@ -52,8 +52,11 @@ typedef struct gsnfs_counts {
 } gsnfs_counts;
 
 /* Dead-zone quantiser parameters (PAPER.md:L255 names the quantiser; rule is reading [R10]):
- *   q = sign(y) * floor(|y| / qstep_c + dz_round),   y^ = sign(q) * (|q| + recon_bias*[q != 0]) * qstep_c.
- * NULL => { 1/3, 0 }. */
+ *   q = sign(y) * floor(|y| * (1/qstep_c) + dz_round),   y^ = sign(q) * (|q| + recon_bias*[q != 0]) * qstep_c.
+ * Arithmetic of the integer decision (normative, the CPU oracle evaluates the same): y is the fp32 coefficient
+ * widened to fp64; 1/qstep_c is the fp64 reciprocal of the fp32 step (one rounding); the product and the sum are
+ * each rounded once in fp64 (no fused multiply-add); floor; saturation to int32.
+ * NULL => { 1/3, 0 }.  Required: 0 <= dz_round <= 1, 0 <= recon_bias < 1, both finite (else INVALID_ARGUMENT). */
 typedef struct gsnfs_quant {
   float dz_round;
   float recon_bias;
@@ -66,7 +69,13 @@ typedef struct gsnfs_quant {
 int gsnfs_create(gsnfs_ctx** out, int device, uint64_t max_points, int max_channels, int max_depth);
 void gsnfs_destroy(gsnfs_ctx* ctx);
 const char* gsnfs_strerror(int status);
-const char* gsnfs_last_error(const gsnfs_ctx* ctx);  /* text of the last GSNFS_E_CUDA on this context */
+const char* gsnfs_last_error(const gsnfs_ctx* ctx);  /* text of the last GSNFS_E_CUDA / overflow on this context */
+/* Errors found on the device after a call has returned (today: a RAHT call whose schedule did not fit the context
+ * scratch -- possible only for voxel keys that are not sorted and unique, see DESIGN.md "RAHT phases" -- in which
+ * case the transform wrote NO output).  The kernel sets gsnfs_counts.status bit 1 (if the call was given d_counts)
+ * and a flag that the next entry point on this context, or this call, reports ONCE as GSNFS_E_CAPACITY.  Does not
+ * synchronise: for a definitive answer synchronise the stream first.  GSNFS_OK if nothing is pending. */
+int gsnfs_poll_status(gsnfs_ctx* ctx);
 const char* gsnfs_version(void);
 /* Number of CUDA kernels this context has launched so far (bench.py's gpu_launches). */
 uint64_t gsnfs_launch_count(const gsnfs_ctx* ctx);
@@ -77,11 +86,6 @@ uint64_t gsnfs_launch_count(const gsnfs_ctx* ctx);
  * "<name> <launches> <total_ms>\n".  Used by bench.py for the live roofline figures. */
 int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records);
 int gsnfs_profile_stop(gsnfs_ctx* ctx, char* out /* host */, uint64_t out_cap);
-
-/* Diagnostics: synchronises and copies the RAHT phase plan of the last forward/inverse call to host:
- * uint32 nphases, overflow, M[32], poff[32], toff[32]; uint64 t_sched[32], t_xform[32] (globaltimer ns at
- * the end of each phase). */
-int gsnfs_debug_read_plan(gsnfs_ctx* ctx, void* h_out /* host */, uint64_t bytes);
 
 /* Upper bound on occupancy bytes for n points at `depth`: sum_{d<depth} min(8^d, n), rounded up to 16. */
 uint64_t gsnfs_occ_capacity(uint64_t n, int depth);
@@ -140,15 +144,20 @@ int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream,
  *   saturated to int32, evaluated in fp64 from the fp32 coefficient.  d_coeff (unquantised fp32) and
  *   d_qcoeff may each be NULL, not both; d_qcoeff requires qstep.
  * n_voxels is the row count; if d_counts != NULL the actual N_v is read on the device from it and
- * n_voxels is only an upper bound (rows beyond N_v are untouched).
+ * n_voxels is only an upper bound (rows beyond N_v are untouched); a d_counts whose status is already non-zero
+ * (a stream the decoder flagged) makes the call a no-op; a schedule overflow ORs bit 1 into d_counts->status.
+ * d_voxel_keys must be sorted and unique, d_weights >= 1 (the caller's responsibility; violations cannot crash
+ * or write out of bounds, and end either in unspecified coefficients or in the overflow report above).
  * Schedule reuse: the prelude (sibling pairs, weights, a/b factors: Alg. A.4/A.5) depends on the codes and leaf weights
  * only.  d_voxel_keys == NULL in gsnfs_raht_forward / gsnfs_raht_inverse means "the same voxel list and weights as the
  * previous gsnfs_raht_* / gsnfs_merge_raht_forward call on this context, with the same n_voxels": the prelude is skipped
  * (one rung more of a bitrate ladder costs the transform only).  d_weights must still be passed if it was then.
- * GSNFS_E_INVALID_ARGUMENT if the context holds no schedule of n_voxels rows; other mismatches are the caller's error. */
+ * The reusing call must be issued on the SAME stream as the call that built the schedule (nothing else orders the
+ * two).  GSNFS_E_INVALID_ARGUMENT if the context holds no schedule of n_voxels rows built on this stream (a failed
+ * RAHT call leaves none); other mismatches are the caller's error.  gsnfs_merge_raht_forward never reuses. */
 int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
                        const uint64_t* d_voxel_keys, const uint32_t* d_weights, uint64_t n_voxels,
-                       const gsnfs_counts* d_counts, int depth,
+                       gsnfs_counts* d_counts, int depth,
                        const float* d_attr /* N_v x channels */, int channels,
                        const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
                        int32_t* d_qcoeff, float* d_coeff);
@@ -172,7 +181,7 @@ int gsnfs_quantize(gsnfs_ctx* ctx, gsnfs_stream stream,
  * d_counts (required) supplies N_v on the device; n is the row capacity as in gsnfs_raht_forward. */
 int gsnfs_merge_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
                              const uint64_t* d_voxel_keys, const uint32_t* d_perm, const uint32_t* d_voxel_start,
-                             uint64_t n, const gsnfs_counts* d_counts, int depth,
+                             uint64_t n, gsnfs_counts* d_counts, int depth,
                              const float* d_attr /* n x channels, input order */, int channels,
                              const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
                              uint32_t* d_weights_out, int32_t* d_qcoeff, float* d_coeff);
@@ -181,7 +190,7 @@ int gsnfs_merge_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
  * schedule top-down with low' = a*y0 - b*y1, high' = b*y0 + a*y1, then divide row i by sqrt(w_i) [R2]. */
 int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream,
                        const uint64_t* d_voxel_keys, const uint32_t* d_weights, uint64_t n_voxels,
-                       const gsnfs_counts* d_counts, int depth,
+                       gsnfs_counts* d_counts, int depth,
                        const int32_t* d_qcoeff, const float* d_coeff, int channels,
                        const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
                        float* d_attr_out /* N_v x channels */);

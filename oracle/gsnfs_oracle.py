@@ -297,7 +297,7 @@ def raht_inverse(Y, M, leaf_w, J):
     return Y / np.sqrt(w)[:, None]
 
 
-def raht_coefficient_closed_form(A, M, leaf_w, rows):
+def raht_coefficient_closed_form(A, M, leaf_w, rows, return_scale=False):
     """Second, independent definition of single RAHT coefficients (no level loop, no active lists): the
     closed form that follows from Eq. (1) and the run-length weights / sibling test of
     Alg. A.4 l.8-10 (L741-747) by induction over the levels.  For row i > 0 let h = msb(M[i-1] xor M[i]);
@@ -307,15 +307,18 @@ def raht_coefficient_closed_form(A, M, leaf_w, rows):
     sqrt(w_j) x_j), hence
         Y[i] = sqrt(W0/(W0+W1)) T_S1/sqrt(W1) - sqrt(W1/(W0+W1)) T_S0/sqrt(W0),   Y[0] = T_all/sqrt(W_all).
     Used to check sampled coefficients at sizes where the level-synchronous oracle is too slow.
-    Returns an array len(rows) x C (fp64)."""
+    Returns an array len(rows) x C (fp64); with return_scale also |T_S1|/sqrt(W1) + |T_S0|/sqrt(W0), the magnitude
+    of the two low-pass values the coefficient is the difference of (what a rounding error is relative to)."""
     A = np.asarray(A)
     M = np.asarray(M, dtype=U64)
     w = np.asarray(leaf_w, dtype=np.float64)
     out = np.empty((len(rows), A.shape[1]), dtype=np.float64)
+    scale = np.empty_like(out)
     for n, i in enumerate(rows):
         i = int(i)
         if i == 0:
             out[n] = (w[:, None] * A.astype(np.float64)).sum(0) / np.sqrt(w.sum())
+            scale[n] = np.abs(out[n])
             continue
         h = int(M[i] ^ M[i - 1]).bit_length() - 1
         l = int(np.searchsorted(M, (M[i] >> U64(h + 1)) << U64(h + 1), side="left"))
@@ -324,7 +327,8 @@ def raht_coefficient_closed_form(A, M, leaf_w, rows):
         T0 = (w[l:i, None] * A[l:i].astype(np.float64)).sum(0)
         T1 = (w[i:r, None] * A[i:r].astype(np.float64)).sum(0)
         out[n] = np.sqrt(W0 / (W0 + W1)) * T1 / np.sqrt(W1) - np.sqrt(W1 / (W0 + W1)) * T0 / np.sqrt(W0)
-    return out
+        scale[n] = np.abs(T1) / np.sqrt(W1) + np.abs(T0) / np.sqrt(W0)
+    return (out, scale) if return_scale else out
 
 
 # ---------------------------------------------------------------------------------------------

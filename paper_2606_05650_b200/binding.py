@@ -45,9 +45,9 @@ _SIGNATURES = {
     "gsnfs_strerror": (c_char_p, [c_int]),
     "gsnfs_last_error": (c_char_p, [c_void_p]),
     "gsnfs_version": (c_char_p, []),
+    "gsnfs_poll_status": (c_int, [c_void_p]),
     "gsnfs_launch_count": (c_uint64, [c_void_p]),
     "gsnfs_occ_capacity": (c_uint64, [c_uint64, c_int]),
-    "gsnfs_debug_read_plan": (c_int, [c_void_p, c_void_p, c_uint64]),
     "gsnfs_profile_start": (c_int, [c_void_p, c_int]),
     "gsnfs_profile_stop": (c_int, [c_void_p, c_char_p, c_uint64]),
     "gsnfs_octree_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, POINTER(c_float), POINTER(c_float),
@@ -182,18 +182,12 @@ class Context:
         except Exception:
             pass
 
+    def poll_status(self) -> int:
+        """GSNFS_OK, or GSNFS_E_CAPACITY once if a kernel of this context reported a scratch overflow."""
+        return int(lib().gsnfs_poll_status(self.handle))
+
     def launch_count(self) -> int:
         return int(lib().gsnfs_launch_count(self.handle))
-
-    def read_raht_plan(self):
-        """Diagnostics: phase sizes and per-phase timestamps of the last RAHT call (synchronises)."""
-        raw = np.zeros(2 + 3 * 32 + 4 * 2 * 32, dtype=np.uint32)
-        self._check(lib().gsnfs_debug_read_plan(self.handle, raw.ctypes.data_as(c_void_p), raw.nbytes), "read_plan")
-        nph = int(raw[0])
-        t = raw[2 + 96:].view(np.uint64)
-        return {"nphases": nph, "overflow": int(raw[1]), "M": raw[2:34][:nph + 2].tolist(),
-                "t_sched_ns": t[:32][:nph + 1].tolist(), "t_xform_ns": t[32:64][:nph + 2].tolist(),
-                "t_dec_ns": t[64:96].tolist(), "t_sort_ns": t[96:128].tolist()}
 
     def profile_start(self, max_records: int = 4096):
         self._check(lib().gsnfs_profile_start(self.handle, int(max_records)), "gsnfs_profile_start")

@@ -20,6 +20,41 @@ struct Bump {
 
 using namespace gsnfs;
 
+namespace {
+// Every entry point runs on the context's device and leaves the caller's current device as it found it.
+struct DeviceGuard {
+  int prev = -1;
+  bool switched = false;
+  cudaError_t enter(int dev) {
+    cudaError_t e = cudaGetDevice(&prev);
+    if (e != cudaSuccess) return e;
+    if (prev != dev) { e = cudaSetDevice(dev); switched = (e == cudaSuccess); }
+    return e;
+  }
+  ~DeviceGuard() { if (switched) cudaSetDevice(prev); }
+};
+#define GSNFS_ON_DEVICE(ctx) DeviceGuard guard__; GSNFS_CUDA_OK(ctx, guard__.enter((ctx)->device))
+
+// A scratch overflow is found on the device, after the call that caused it has returned: the kernel sets
+// gsnfs_counts.status bit 1 (when the call was given a d_counts) and a host-mapped flag that the NEXT entry point
+// on this context (or gsnfs_poll_status) reports once as GSNFS_E_CAPACITY.
+int take_sticky(gsnfs_ctx* ctx) {
+  if (ctx->h_flags && *(volatile uint32_t*)ctx->h_flags) {
+    *(volatile uint32_t*)ctx->h_flags = 0;
+    ctx->sched_n = 0;
+    snprintf(ctx->err, sizeof(ctx->err), "an earlier RAHT call on this context overflowed its schedule scratch "
+             "(unsorted or duplicate voxel keys?); its outputs were not written");
+    return GSNFS_E_CAPACITY;
+  }
+  return GSNFS_OK;
+}
+bool quant_ok(const gsnfs_quant* q) {
+  if (!q) return true;
+  return isfinite(q->dz_round) && q->dz_round >= 0.f && q->dz_round <= 1.f && isfinite(q->recon_bias) &&
+         q->recon_bias >= 0.f && q->recon_bias < 1.f;
+}
+}  // namespace
+
 extern "C" {
 
 const char* gsnfs_version(void) { return "gsnfs-b200 0.1 (sm_100a)"; }
@@ -37,6 +72,7 @@ const char* gsnfs_strerror(int status) {
 }
 
 const char* gsnfs_last_error(const gsnfs_ctx* ctx) { return ctx ? ctx->err : "null context"; }
+int gsnfs_poll_status(gsnfs_ctx* ctx) { return ctx ? take_sticky(ctx) : GSNFS_E_INVALID_ARGUMENT; }
 uint64_t gsnfs_launch_count(const gsnfs_ctx* ctx) { return ctx ? ctx->launches : 0; }
 
 uint64_t gsnfs_occ_capacity(uint64_t n, int depth) {
@@ -50,7 +86,10 @@ uint64_t gsnfs_occ_capacity(uint64_t n, int depth) {
 }
 
 static int create_impl(gsnfs_ctx* c) {
-  GSNFS_CUDA_OK(c, cudaSetDevice(c->device));
+  GSNFS_ON_DEVICE(c);
+  GSNFS_CUDA_OK(c, cudaHostAlloc((void**)&c->h_flags, 64, cudaHostAllocMapped));
+  memset(c->h_flags, 0, 64);
+  GSNFS_CUDA_OK(c, cudaHostGetDevicePointer((void**)&c->d_flags, c->h_flags, 0));
   cudaDeviceProp prop;
   GSNFS_CUDA_OK(c, cudaGetDeviceProperties(&prop, c->device));
   c->num_sms = prop.multiProcessorCount;
@@ -127,6 +166,7 @@ int gsnfs_create(gsnfs_ctx** out, int device, uint64_t max_points, int max_chann
   if (rc != GSNFS_OK) {
     fprintf(stderr, "gsnfs_create failed: %s\n", c->err);
     if (c->pool) cudaFree(c->pool);
+    if (c->h_flags) cudaFreeHost(c->h_flags);
     free(c);
     return rc;
   }
@@ -136,7 +176,9 @@ int gsnfs_create(gsnfs_ctx** out, int device, uint64_t max_points, int max_chann
 
 void gsnfs_destroy(gsnfs_ctx* ctx) {
   if (!ctx) return;
-  cudaSetDevice(ctx->device);
+  DeviceGuard guard;
+  guard.enter(ctx->device);
+  if (ctx->h_flags) cudaFreeHost(ctx->h_flags);
   for (int i = 0; i < ctx->prof_cap; ++i) { cudaEventDestroy(ctx->prof[i].a); cudaEventDestroy(ctx->prof[i].b); }
   free(ctx->prof);
   if (ctx->pool) cudaFree(ctx->pool);
@@ -144,18 +186,9 @@ void gsnfs_destroy(gsnfs_ctx* ctx) {
   free(ctx);
 }
 
-int gsnfs_debug_read_plan(gsnfs_ctx* ctx, void* h_out, uint64_t bytes) {
-  if (!ctx || !h_out) return GSNFS_E_INVALID_ARGUMENT;
-  if (bytes > sizeof(RahtPlan)) bytes = sizeof(RahtPlan);
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  GSNFS_CUDA_OK(ctx, cudaDeviceSynchronize());
-  GSNFS_CUDA_OK(ctx, cudaMemcpy(h_out, ctx->raht_plan, bytes, cudaMemcpyDeviceToHost));
-  return GSNFS_OK;
-}
-
 int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records) {
   if (!ctx || max_records < 1) return GSNFS_E_INVALID_ARGUMENT;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_ON_DEVICE(ctx);
   if (max_records > ctx->prof_cap) {
     ProfRec* np = (ProfRec*)realloc(ctx->prof, sizeof(ProfRec) * (size_t)max_records);
     if (!np) return GSNFS_E_CAPACITY;
@@ -174,7 +207,7 @@ int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records) {
 int gsnfs_profile_stop(gsnfs_ctx* ctx, char* out, uint64_t out_cap) {
   if (!ctx || !out || out_cap < 2) return GSNFS_E_INVALID_ARGUMENT;
   ctx->prof_on = 0;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_ON_DEVICE(ctx);
   GSNFS_CUDA_OK(ctx, cudaDeviceSynchronize());
   // aggregate by kernel name (names are string literals; compare by content)
   struct Agg { const char* name; int count; double ms; };
@@ -216,7 +249,7 @@ int gsnfs_octree_encode(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_xyz,
   }
   if (n > ctx->max_points || depth > ctx->max_depth) return GSNFS_E_CAPACITY;
   if (occ_capacity < gsnfs_occ_capacity(n, depth) || (occ_capacity & 3)) return GSNFS_E_CAPACITY;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_ON_DEVICE(ctx);
   return run_octree_encode(ctx, (cudaStream_t)stream, d_xyz, (uint32_t)n, lo, scale, depth, d_occ, occ_capacity,
                            d_level_sizes, d_perm, d_voxel_keys, d_voxel_start, d_counts);
 }
@@ -228,7 +261,7 @@ int gsnfs_voxel_merge(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr, 
     return GSNFS_E_INVALID_ARGUMENT;
   if (channels < 1 || channels > GSNFS_MAX_CHANNELS || n >= (1ull << 30)) return GSNFS_E_INVALID_ARGUMENT;
   if (n > ctx->max_points) return GSNFS_E_CAPACITY;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_ON_DEVICE(ctx);
   return run_voxel_merge(ctx, (cudaStream_t)stream, d_attr, channels, (uint32_t)n, d_perm, d_voxel_start, d_counts,
                          d_merged, d_weights);
 }
@@ -240,74 +273,81 @@ int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_oc
   if (depth < 1 || depth > GSNFS_MAX_DEPTH) return GSNFS_E_INVALID_ARGUMENT;
   if (level_sizes[depth] && (!d_occ || !d_voxel_xyz)) return GSNFS_E_INVALID_ARGUMENT;
   if (depth > ctx->max_depth) return GSNFS_E_CAPACITY;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_ON_DEVICE(ctx);
   return run_octree_decode(ctx, (cudaStream_t)stream, d_occ, occ_bytes, level_sizes, depth, d_voxel_xyz, d_voxel_keys,
                            d_counts);
 }
 
-static int raht_check(gsnfs_ctx* ctx, const uint64_t* keys, uint64_t n, int depth, int channels) {
+static int raht_check(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* keys, bool keys_required, uint64_t n, int depth,
+                      int channels, const float* qstep, const gsnfs_quant* quant) {
   if (!ctx) return GSNFS_E_INVALID_ARGUMENT;
-  if (n && !keys && ctx->sched_n != n) return GSNFS_E_INVALID_ARGUMENT;      // NULL keys: reuse needs a schedule of n rows
+  int rc = take_sticky(ctx);
+  if (rc != GSNFS_OK) return rc;
   if (depth < 1 || depth > GSNFS_MAX_DEPTH || channels < 1 || channels > GSNFS_MAX_CHANNELS || n >= (1ull << 30))
     return GSNFS_E_INVALID_ARGUMENT;
+  if (n && !keys) {
+    // schedule reuse: only where the header allows it, only a schedule of n rows built on this very stream
+    if (keys_required || ctx->sched_n != n || ctx->sched_stream != (void*)stream) return GSNFS_E_INVALID_ARGUMENT;
+  }
+  if (!quant_ok(quant)) return GSNFS_E_INVALID_ARGUMENT;
+  if (qstep)
+    for (int c = 0; c < channels; ++c)
+      if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
   if (n > ctx->max_points || channels > ctx->max_channels) return GSNFS_E_CAPACITY;
   return GSNFS_OK;
 }
 
+// a failed RAHT call leaves no schedule behind to reuse
+static int raht_done(gsnfs_ctx* ctx, int rc) {
+  if (rc != GSNFS_OK) ctx->sched_n = 0;
+  return rc;
+}
+
 int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_weights,
-                       uint64_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_attr, int channels,
+                       uint64_t n_voxels, gsnfs_counts* d_counts, int depth, const float* d_attr, int channels,
                        const float* qstep, const gsnfs_quant* quant, int32_t* d_qcoeff, float* d_coeff) {
-  int rc = raht_check(ctx, d_voxel_keys, n_voxels, depth, channels);
+  int rc = raht_check(ctx, stream, d_voxel_keys, false, n_voxels, depth, channels, qstep, quant);
   if (rc != GSNFS_OK) return rc;
   if (n_voxels && (!d_attr || (!d_qcoeff && !d_coeff) || (d_qcoeff && !qstep))) return GSNFS_E_INVALID_ARGUMENT;
-  if (qstep)
-    for (int c = 0; c < channels; ++c)
-      if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  return run_raht(ctx, (cudaStream_t)stream, false, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth, d_attr,
-                  nullptr, channels, qstep, quant, d_qcoeff, d_coeff);
+  GSNFS_ON_DEVICE(ctx);
+  return raht_done(ctx, run_raht(ctx, (cudaStream_t)stream, false, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth,
+                                 d_attr, nullptr, channels, qstep, quant, d_qcoeff, d_coeff));
 }
 
 int gsnfs_merge_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_perm,
-                             const uint32_t* d_voxel_start, uint64_t n, const gsnfs_counts* d_counts, int depth,
+                             const uint32_t* d_voxel_start, uint64_t n, gsnfs_counts* d_counts, int depth,
                              const float* d_attr, int channels, const float* qstep, const gsnfs_quant* quant,
                              uint32_t* d_weights_out, int32_t* d_qcoeff, float* d_coeff) {
-  int rc = raht_check(ctx, d_voxel_keys, n, depth, channels);
+  int rc = raht_check(ctx, stream, d_voxel_keys, true, n, depth, channels, qstep, quant);
   if (rc != GSNFS_OK) return rc;
   if (!d_counts || (n && (!d_perm || !d_voxel_start || !d_attr || !d_weights_out || (!d_qcoeff && !d_coeff) || (d_qcoeff && !qstep))))
     return GSNFS_E_INVALID_ARGUMENT;
-  if (qstep)
-    for (int c = 0; c < channels; ++c)
-      if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  return run_raht(ctx, (cudaStream_t)stream, false, d_voxel_keys, nullptr, (uint32_t)n, d_counts, depth, d_attr, nullptr,
-                  channels, qstep, quant, d_qcoeff, d_coeff, d_perm, d_voxel_start, d_weights_out);
+  GSNFS_ON_DEVICE(ctx);
+  return raht_done(ctx, run_raht(ctx, (cudaStream_t)stream, false, d_voxel_keys, nullptr, (uint32_t)n, d_counts, depth, d_attr,
+                                 nullptr, channels, qstep, quant, d_qcoeff, d_coeff, d_perm, d_voxel_start, d_weights_out));
 }
 
 int gsnfs_quantize(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_coeff, uint64_t n_rows,
                    const gsnfs_counts* d_counts, int channels, const float* qstep, const gsnfs_quant* quant,
                    int32_t* d_qcoeff) {
   if (!ctx || !qstep || (n_rows && (!d_coeff || !d_qcoeff))) return GSNFS_E_INVALID_ARGUMENT;
-  if (channels < 1 || channels > GSNFS_MAX_CHANNELS || n_rows >= (1ull << 30)) return GSNFS_E_INVALID_ARGUMENT;
+  if (channels < 1 || channels > GSNFS_MAX_CHANNELS || n_rows >= (1ull << 30) || !quant_ok(quant)) return GSNFS_E_INVALID_ARGUMENT;
   for (int c = 0; c < channels; ++c)
     if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_ON_DEVICE(ctx);
   return run_quantize(ctx, (cudaStream_t)stream, d_coeff, (uint32_t)n_rows, d_counts, channels, qstep, quant, d_qcoeff);
 }
 
 int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_voxel_keys, const uint32_t* d_weights,
-                       uint64_t n_voxels, const gsnfs_counts* d_counts, int depth, const int32_t* d_qcoeff,
+                       uint64_t n_voxels, gsnfs_counts* d_counts, int depth, const int32_t* d_qcoeff,
                        const float* d_coeff, int channels, const float* qstep, const gsnfs_quant* quant,
                        float* d_attr_out) {
-  int rc = raht_check(ctx, d_voxel_keys, n_voxels, depth, channels);
+  int rc = raht_check(ctx, stream, d_voxel_keys, false, n_voxels, depth, channels, qstep, quant);
   if (rc != GSNFS_OK) return rc;
   if (n_voxels && (!d_attr_out || (!d_qcoeff && !d_coeff) || (d_qcoeff && !qstep))) return GSNFS_E_INVALID_ARGUMENT;
-  if (qstep)
-    for (int c = 0; c < channels; ++c)
-      if (!(qstep[c] > 0.f) || !isfinite(qstep[c])) return GSNFS_E_INVALID_ARGUMENT;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
-  return run_raht(ctx, (cudaStream_t)stream, true, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth, d_coeff,
-                  d_qcoeff, channels, d_qcoeff ? qstep : nullptr, quant, nullptr, d_attr_out);
+  GSNFS_ON_DEVICE(ctx);
+  return raht_done(ctx, run_raht(ctx, (cudaStream_t)stream, true, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth,
+                                 d_coeff, d_qcoeff, channels, d_qcoeff ? qstep : nullptr, quant, nullptr, d_attr_out));
 }
 
 // ---- whole-frame calls on host buffers -----------------------------------------------------------
@@ -336,7 +376,7 @@ int gsnfs_frame_encode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_
   if (!ctx || !h_occ || !h_level_sizes || !h_counts || !qstep || (n && (!h_xyz || !h_attr || !h_weights || !h_qcoeff)))
     return GSNFS_E_INVALID_ARGUMENT;
   if (n > ctx->max_points || channels > ctx->max_channels || channels < 1) return GSNFS_E_CAPACITY;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  GSNFS_ON_DEVICE(ctx);
   int rc = frame_pool(ctx);
   if (rc != GSNFS_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
@@ -377,7 +417,15 @@ int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* 
   if (nv && (!h_occ || !h_qcoeff || !h_voxel_xyz || !h_attr)) return GSNFS_E_INVALID_ARGUMENT;
   if (nv > ctx->max_points || channels > ctx->max_channels || channels < 1 || occ_bytes + 1 > ctx->occ_cap)
     return GSNFS_E_CAPACITY;
-  GSNFS_CUDA_OK(ctx, cudaSetDevice(ctx->device));
+  // header checks that need no device [O12]: an inconsistent header is reported before a byte is copied
+  if (!octree_header_ok(level_sizes, depth, occ_bytes)) {
+    h_counts->n_voxels = 0; h_counts->occ_bytes = (uint32_t)occ_bytes; h_counts->status = 1; h_counts->reserved = 0;
+    return GSNFS_OK;
+  }
+  if (h_weights)
+    for (uint64_t i = 0; i < nv; ++i)
+      if (h_weights[i] == 0) return GSNFS_E_INVALID_ARGUMENT;                // a leaf of weight 0 has no transform [R1]
+  GSNFS_ON_DEVICE(ctx);
   int rc = frame_pool(ctx);
   if (rc != GSNFS_OK) return rc;
   cudaStream_t st = (cudaStream_t)stream;
@@ -389,7 +437,9 @@ int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* 
   }
   rc = gsnfs_octree_decode(ctx, stream, ctx->f_occ, occ_bytes, level_sizes, depth, ctx->f_vxyz, ctx->f_vkeys, ctx->f_counts);
   if (rc != GSNFS_OK) return rc;
-  rc = gsnfs_raht_inverse(ctx, stream, ctx->f_vkeys, h_weights ? ctx->f_weights : nullptr, nv, nullptr, depth, ctx->f_q,
+  // f_counts chains the decoder's verdict on the device: a stream found corrupt there leaves N_v = 0, and the
+  // inverse transform is then a no-op instead of a walk over stale codes
+  rc = gsnfs_raht_inverse(ctx, stream, ctx->f_vkeys, h_weights ? ctx->f_weights : nullptr, nv, ctx->f_counts, depth, ctx->f_q,
                           nullptr, channels, qstep, quant, ctx->f_attr);
   if (rc != GSNFS_OK) return rc;
   GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_counts, ctx->f_counts, sizeof(gsnfs_counts), cudaMemcpyDeviceToHost, st));
@@ -398,7 +448,7 @@ int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* 
     GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_attr, ctx->f_attr, nv * C * 4, cudaMemcpyDeviceToHost, st));
   }
   GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
-  return GSNFS_OK;
+  return take_sticky(ctx);
 }
 
 }  // extern "C"

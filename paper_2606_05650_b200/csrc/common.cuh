@@ -38,14 +38,11 @@ static_assert(sizeof(RahtTileHdr) == 176, "RahtTileHdr layout");
 // Device-resident description of the phase structure (data dependent).
 struct RahtPlan {
   uint32_t nphases;
-  uint32_t overflow;
+  uint32_t overflow;                  // the schedule did not fit the scratch, or `invalid`: the transform kernels write nothing
+  uint32_t invalid;                   // voxel codes not sorted and unique, or a zero leaf weight
   uint32_t M[kRahtMaxPhases + 2];     // active entries of phase p (1-based); M[1] = N_v
   uint32_t poff[kRahtMaxPhases + 2];  // row offset of phase p (p >= 2) in the idx / pending-row pools
   uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
-  unsigned long long t_sched[kRahtMaxPhases + 2];  // globaltimer (ns) at the end of each phase, CTA 0 (diagnostics)
-  unsigned long long t_xform[kRahtMaxPhases + 2];
-  unsigned long long t_dec[kRahtMaxPhases + 2];
-  unsigned long long t_sort[kRahtMaxPhases + 2];   // radix sort: start, then after phase A / barrier / phase B of each pass    // octree decode: after scan reduce, after down-sweep, after each level step
 };
 
 struct ProfRec {
@@ -105,6 +102,9 @@ struct gsnfs_ctx {
   float* raht_rows;        // pending-row pool (phases >= 2)
   uint64_t raht_pool_rows; // capacity (rows) of raht_idx / raht_rows
   uint64_t sched_n;        // row count of the schedule currently held in raht_rec / raht_hdr / raht_plan (0 = none)
+  void* sched_stream;      // the stream that schedule was built on (reuse is only ordered on the same stream)
+  uint32_t* h_flags;       // host-mapped: [0] != 0 <=> a kernel of this context found its scratch too small
+  uint32_t* d_flags;       // device alias of h_flags
   uint64_t raht_rec_cap;
   uint64_t raht_hdr_cap;
   float* qparams;          // 2 x max_channels doubles (inv step / step) stored as double
@@ -175,11 +175,6 @@ __device__ __forceinline__ unsigned lanemask_le() {
   asm("mov.u32 %0, %%lanemask_le;" : "=r"(m));
   return m;
 }
-__device__ __forceinline__ unsigned long long globaltimer_ns() {
-  unsigned long long t;
-  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
-  return t;
-}
 __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
   uint32_t v;
   asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
@@ -226,11 +221,12 @@ int run_octree_encode(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint3
 int run_voxel_merge(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, int channels, uint32_t n,
                     const uint32_t* d_perm, const uint32_t* d_voxel_start, const gsnfs_counts* d_counts,
                     float* d_merged, uint32_t* d_weights);
+bool octree_header_ok(const uint32_t* level_sizes, int depth, uint64_t occ_bytes);
 int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uint64_t occ_bytes,
                       const uint32_t* level_sizes, int depth, uint32_t* d_voxel_xyz, uint64_t* d_voxel_keys,
                       gsnfs_counts* d_counts);
 int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_keys, const uint32_t* d_weights,
-             uint32_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_in_f,
+             uint32_t n_voxels, gsnfs_counts* d_counts, int depth, const float* d_in_f,
              const int32_t* d_in_q, int channels, const float* qstep, const gsnfs_quant* quant,
              int32_t* d_out_q, float* d_out_f, const uint32_t* d_perm = nullptr, const uint32_t* d_vstart = nullptr,
              uint32_t* d_weights_out = nullptr);

@@ -55,12 +55,8 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
                                                             uint32_t* __restrict__ tile_sums, uint32_t* __restrict__ PD,
                                                             uint64_t* __restrict__ Kmid,
                                                             uint32_t* __restrict__ xyz, uint64_t* __restrict__ keys_out,
-                                                            gsnfs_counts* __restrict__ counts,
-                                                            unsigned long long* __restrict__ tstamp) {
+                                                            gsnfs_counts* __restrict__ counts) {
   cg::grid_group grid = cg::this_grid();
-  int ts = 0;
-#define GSNFS_STAMP() do { if (blockIdx.x == 0 && threadIdx.x == 0 && ts < kRahtMaxPhases + 2) tstamp[ts] = globaltimer_ns(); ++ts; } while (0)
-  GSNFS_STAMP();
   __shared__ uint32_t s_w[9];
   __shared__ uint16_t s_stage[8 * kScanTile];   // a tile's (node-in-tile << 3 | digit) entries on their way out
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -95,7 +91,6 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
     __syncthreads();
   }
   grid.sync();
-  GSNFS_STAMP();
   // ---- 2. down-sweep: (parent << 3 | digit) of every child.  The children of a tile are one contiguous id range:
   // staged in shared memory as 16-bit (node-in-tile << 3 | digit), written out coalesced.  The tile's base (number of
   // children before it) is carried from the CTA's previous tile by summing the tile sums in between.
@@ -154,7 +149,6 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
     }
   }
   grid.sync();
-  GSNFS_STAMP();
   // ---- header vs stream, level by level [O12]: with the node count right and no childless node, level e + 1 starts
   // at the header's offset iff its first node is the first child of level e's first node and the node before it is
   // the last child of the node before that
@@ -204,7 +198,6 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
       }
     }
     if (stage == 0) grid.sync();
-    GSNFS_STAMP();
   }
 }
 
@@ -215,21 +208,23 @@ __global__ void decode_status_kernel(gsnfs_counts* counts, uint32_t nv, uint32_t
   counts->reserved = 0;
 }
 
+// Header checks that need no device [O12]: the header must describe a tree (one root, no empty level, no level
+// larger than the next one: every internal node has >= 1 child) whose internal nodes are the stream's bytes.
+bool octree_header_ok(const uint32_t* level_sizes, int depth, uint64_t occ_bytes) {
+  if (level_sizes[depth] == 0) return occ_bytes == 0;
+  uint64_t sum = 0;
+  for (int d = 0; d < depth; ++d) {
+    if (level_sizes[d] == 0 || level_sizes[d] > level_sizes[d + 1]) return false;
+    sum += level_sizes[d];
+  }
+  return sum == occ_bytes && level_sizes[0] == 1;
+}
+
 int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uint64_t occ_bytes,
                       const uint32_t* level_sizes, int depth, uint32_t* d_voxel_xyz, uint64_t* d_voxel_keys,
                       gsnfs_counts* d_counts) {
   const uint32_t nv = level_sizes[depth];
-  uint64_t sum = 0;
-  for (int d = 0; d < depth; ++d) sum += level_sizes[d];
-  uint32_t status = 0;
-  if (nv == 0) {
-    if (occ_bytes != 0) status = 1;
-  } else if (sum != occ_bytes || level_sizes[0] != 1) {
-    status = 1;                                               // header inconsistent with the stream [O12]
-  } else {
-    for (int d = 0; d < depth; ++d)
-      if (level_sizes[d] == 0 || level_sizes[d] > level_sizes[d + 1]) status = 1;    // every node has >= 1 child
-  }
+  const uint32_t status = octree_header_ok(level_sizes, depth, occ_bytes) ? 0u : 1u;
   for (int d = 0; d <= depth; ++d)
     if (level_sizes[d] > ctx->max_points) return GSNFS_E_CAPACITY;
   if (occ_bytes + 1 > ctx->occ_cap || occ_bytes >= (1ull << 29)) return GSNFS_E_CAPACITY;   // parent ids are packed with 3 digit bits
@@ -268,9 +263,8 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
   uint32_t grid = (uint32_t)per_sm * (uint32_t)ctx->num_sms;
   if (grid > want) grid = want;
   if (grid < 1) grid = 1;
-  unsigned long long* tstamp = ctx->raht_plan->t_dec;
   void* args[] = {(void*)&d_occ, (void*)&S, (void*)&lv, (void*)&ctx->scan_sums,
-                  (void*)&ctx->dec_parent, (void*)&ctx->dec_kmid, (void*)&d_voxel_xyz, (void*)&d_voxel_keys, (void*)&d_counts, (void*)&tstamp};
+                  (void*)&ctx->dec_parent, (void*)&ctx->dec_kmid, (void*)&d_voxel_xyz, (void*)&d_voxel_keys, (void*)&d_counts};
   GSNFS_KERNEL(ctx, st, "octree_decode");
   GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)octree_decode_kernel, dim3(grid), dim3(256), args, 0, st));
   GSNFS_LAUNCH_CHECK(ctx, st);

@@ -161,12 +161,8 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
                                                                  uint32_t* perm_out, uint32_t n, uint32_t ntiles,
                                                                  uint32_t tstride, int ipt, SortPlan plan,
                                                                  const uint32_t* __restrict__ ghist, uint32_t* tile_hist,
-                                                                 uint32_t* group_hist, uint32_t ngroups_cap,
-                                                                 unsigned long long* __restrict__ tstamp) {
+                                                                 uint32_t* group_hist, uint32_t ngroups_cap) {
   cg::grid_group grid = cg::this_grid();
-  int ts = 0;
-#define GSNFS_SSTAMP() do { if (blockIdx.x == 0 && threadIdx.x == 0 && ts < kRahtMaxPhases + 2) tstamp[ts] = globaltimer_ns(); ++ts; } while (0)
-  GSNFS_SSTAMP();
   extern __shared__ __align__(16) unsigned char s_dyn[];
   KeyT* s_keys = reinterpret_cast<KeyT*>(s_dyn);
   uint32_t* s_pay = reinterpret_cast<uint32_t*>(s_dyn + sizeof(KeyT) * kSortTile);
@@ -215,9 +211,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
       if (count) atomicAdd(&gh[(size_t)(tile / kSortGroup) * 256 + tid], count);
       __syncthreads();
     }
-    GSNFS_SSTAMP();
     grid.sync();
-    GSNFS_SSTAMP();
     // the other parity's group sums are free now: clear them for the next pass
     for (uint32_t i = blockIdx.x * kSortThreads + tid; i < ngroups * 256; i += gridDim.x * kSortThreads) gh_next[i] = 0;
 
@@ -275,9 +269,7 @@ __global__ void __launch_bounds__(kSortThreads) sort_coop_kernel(KeyT* ka, KeyT*
       }
       __syncthreads();
     }
-    GSNFS_SSTAMP();
     if (p + 1 < plan.passes) grid.sync();
-    GSNFS_SSTAMP();
   }
 }
 
@@ -536,11 +528,10 @@ static int encode_impl(gsnfs_ctx* ctx, cudaStream_t st, const float* d_xyz, uint
       uint32_t* th = ctx->sort_tile_hist;
       uint32_t* grp = ctx->sort_group_hist;
       uint32_t gcap = ctx->sort_groups_cap;
-      unsigned long long* tstamp = ctx->raht_plan->t_sort;
       uint32_t ntl = stiles;
       void* args[] = {(void*)&kbuf_a, (void*)&kbuf_b, (void*)&pbuf_a, (void*)&pbuf_b, (void*)&d_perm, (void*)&nn, (void*)&ntl,
                       (void*)&tstride, (void*)&ipt, (void*)&pl,
-                      (void*)&gh, (void*)&th, (void*)&grp, (void*)&gcap, (void*)&tstamp};
+                      (void*)&gh, (void*)&th, (void*)&grp, (void*)&gcap};
       GSNFS_KERNEL(ctx, st, "radix_sort");
       GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)sort_coop_kernel<KeyT>, dim3(grid), dim3(kSortThreads), args, smem, st));
       GSNFS_LAUNCH_CHECK(ctx, st);

@@ -126,7 +126,7 @@ struct SchedPools {
 
 __global__ void __launch_bounds__(256) raht_schedule_kernel(
     const uint64_t* __restrict__ keys, const uint32_t* __restrict__ weights, uint32_t n_host,
-    const uint32_t* __restrict__ n_dev, SchedPools sp, RahtPlan* __restrict__ plan) {
+    gsnfs_counts* __restrict__ counts, SchedPools sp, RahtPlan* __restrict__ plan, uint32_t* __restrict__ sticky) {
   cg::grid_group grid = cg::this_grid();
   __shared__ uint64_t s_key[T];
   __shared__ uint32_t s_wpre[T + 1];       // tile-local exclusive prefix of the entry weights
@@ -142,20 +142,21 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
   __shared__ uint32_t s_hit[2];
 
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const uint32_t Nv = n_dev ? min(*n_dev, n_host) : n_host;
+  // a frame the decoder flagged corrupt (status != 0) has no transform: N_v = 0 makes every later kernel a no-op
+  const uint32_t Nv = counts ? (counts->status ? 0u : min(counts->n_voxels, n_host)) : n_host;
   uint32_t M = Nv, toff = 0, boff = 0;
+  bool overflow = false;
   uint32_t toff_prev = 0, boff_prev = 0, ntiles_prev = 0, poff = 0;
   int p = 1;
   if (blockIdx.x == 0 && tid == 0) {
-    plan->M[0] = 0; plan->M[1] = Nv; plan->poff[1] = 0; plan->toff[1] = 0; plan->overflow = 0; plan->nphases = 1;
-    plan->t_sched[0] = globaltimer_ns();
+    plan->M[0] = 0; plan->M[1] = Nv; plan->poff[1] = 0; plan->toff[1] = 0; plan->nphases = 1;   // overflow / invalid: cleared by the host
   }
   while (true) {
     const uint32_t ntiles = (M + T - 1) / T;
     const uint32_t nb = (ntiles + 255) / 256;
     const uint32_t nb_prev = (ntiles_prev + 255) / 256;
     if (toff + ntiles > sp.hdr_cap || boff + nb > sp.bsum_cap) {      // uniform over the grid
-      if (blockIdx.x == 0 && tid == 0) plan->overflow = 1;
+      overflow = true;
       break;
     }
     // side job (p >= 2): exclusive offsets of the previous phase's pending lists -> its tile headers
@@ -246,6 +247,7 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
         }
       }
       s_key[tid] = mk;
+      if (p == 1 && valid && went == 0u) plan->invalid = 1u;          // a leaf of weight 0 has no transform [R1]
       for (int i = tid; i < 8 * 64; i += 256) (&s_wl[0][0])[i] = 0;
       {
         uint32_t tot;
@@ -262,6 +264,8 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
       int level = 0;
       uint32_t l = 0;
       float fa = 0.f, fb = 0.f;
+      // the codes must be sorted and unique (gsnfs.h); a violation is reported, never silently transformed
+      if (valid && (tid > 0 ? s_key[tid - 1] >= mk : (has_prev && s_edge[0] >= mk))) plan->invalid = 1u;
       if (valid && tid > 0) {
         const uint64_t x = s_key[tid - 1] ^ mk;
         const int h = x ? msb64(x) : 0;                            // x == 0 only for invalid (non-unique) input
@@ -362,20 +366,27 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
     const uint32_t poff_next = (p == 1) ? 0u : poff + M;
     if (blockIdx.x == 0 && tid == 0) {
       plan->M[p + 1] = M_next; plan->poff[p + 1] = poff_next; plan->toff[p + 1] = toff + ntiles;
-      plan->t_sched[p] = globaltimer_ns();
     }
-    if ((uint64_t)poff_next + M_next > sp.pool_rows) {
-      if (blockIdx.x == 0 && tid == 0) plan->overflow = 1;
+    if ((uint64_t)poff_next + M_next > sp.pool_rows || (M_next > 1 && p + 1 > kRahtMaxPhases)) {
+      overflow = true;
       break;
     }
-    if (M_next <= 1 || p + 1 > kRahtMaxPhases) break;
+    if (M_next <= 1) break;
     toff_prev = toff; boff_prev = boff; ntiles_prev = ntiles;
     poff = poff_next;
     toff += ntiles; boff += nb;
     M = M_next;
     ++p;
   }
-  if (blockIdx.x == 0 && tid == 0) plan->nphases = (uint32_t)p;
+  if (blockIdx.x == 0 && tid == 0) {
+    plan->nphases = (uint32_t)p;
+    if (overflow || *(volatile uint32_t*)&plan->invalid) {   // loud: the transform kernels write nothing; the caller sees status bit 1
+      plan->overflow = 1;
+      if (counts) atomicOr(&counts->status, 2u);
+      *sticky = 1u;
+      __threadfence_system();
+    }
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -439,7 +450,7 @@ __device__ __forceinline__ float vscale(float v, double s) { return (float)((dou
 // the caller falls back to quant_exact, so the result always equals the fp64 definition.  Two values per call:
 // the arithmetic is packed fp32x2.
 __device__ __forceinline__ int quant_exact(float y, double inv, double f) {
-  double m = floor(fma(fabs((double)y), inv, f));
+  double m = floor(__dadd_rn(__dmul_rn(fabs((double)y), inv), f));      // product and sum rounded once each, no FMA (gsnfs.h)
   m = fmin(m, 2147483647.0);
   const int q = (int)m;
   return y < 0.f ? -q : q;
@@ -577,7 +588,6 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
   if (!has_q) out_q = nullptr;
   const uint32_t nph = plan->nphases;
   if (plan->overflow) return;                                           // uniform: no grid.sync mismatch
-  if (blockIdx.x == 0 && tid == 0) plan->t_xform[0] = globaltimer_ns();
   for (uint32_t p = 1; p <= nph; ++p) {
     const uint32_t M = plan->M[p], Mnext = plan->M[p + 1];
     const uint32_t ntiles = (M + T - 1) / T, toff = plan->toff[p];
@@ -721,7 +731,6 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
     }
     cp_async_wait_all();
     if (p < nph) grid.sync();
-    if (blockIdx.x == 0 && tid == 0) plan->t_xform[p] = globaltimer_ns();
   }
 }
 
@@ -774,7 +783,6 @@ __global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
   const void* coef = in_q ? (const void*)in_q : (const void*)in_f;       // both are 4-byte rows of C entries
   const uint32_t nph = plan->nphases;
   if (plan->overflow) return;
-  if (blockIdx.x == 0 && tid == 0) plan->t_xform[nph + 1] = globaltimer_ns();
   for (uint32_t p = nph; p >= 1; --p) {
     const uint32_t M = plan->M[p], Mnext = plan->M[p + 1];
     const uint32_t ntiles = (M + T - 1) / T, toff = plan->toff[p];
@@ -890,7 +898,6 @@ __global__ void __launch_bounds__(kXT, 3) raht_inverse_kernel(
       }
       grid.sync();
     }
-    if (blockIdx.x == 0 && tid == 0) plan->t_xform[p] = globaltimer_ns();
   }
 }
 
@@ -948,7 +955,8 @@ static size_t raht_smem_bytes(int C) {
 }
 
 int raht_setup(gsnfs_ctx* ctx) {
-  const size_t smem = raht_smem_bytes(ctx->max_channels);
+  // the attribute belongs to the function on the device, not to this context: always the library-wide maximum
+  const size_t smem = raht_smem_bytes(GSNFS_MAX_CHANNELS);
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(raht_forward_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(raht_forward_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(raht_inverse_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
@@ -971,12 +979,11 @@ static int coop_grid(gsnfs_ctx* ctx, int slot, K kernel, size_t smem, uint32_t w
 }
 
 int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_keys, const uint32_t* d_weights,
-             uint32_t n_voxels, const gsnfs_counts* d_counts, int depth, const float* d_in_f, const int32_t* d_in_q,
+             uint32_t n_voxels, gsnfs_counts* d_counts, int depth, const float* d_in_f, const int32_t* d_in_q,
              int channels, const float* qstep, const gsnfs_quant* quant, int32_t* d_out_q, float* d_out_f,
              const uint32_t* d_perm, const uint32_t* d_vstart, uint32_t* d_weights_out) {
   (void)depth;
   if (n_voxels == 0) return GSNFS_OK;
-  const uint32_t* n_dev = d_counts ? &d_counts->n_voxels : nullptr;
   const uint32_t want = (n_voxels + T - 1) / T;
   SchedPools sp;
   sp.rec = ctx->raht_rec; sp.hdr = ctx->raht_hdr; sp.pend_vidx = ctx->raht_idx; sp.pend_w = ctx->raht_pw;
@@ -989,14 +996,17 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   ga.gsrc = fused ? ctx->raht_gsrc : nullptr; ga.perm = d_perm; ga.vstart = d_vstart;
   if (d_keys) {                                  // NULL: the schedule of the previous call on this context is reused
     GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
+    GSNFS_CUDA_OK(ctx, cudaMemsetAsync(&ctx->raht_plan->overflow, 0, 2 * sizeof(uint32_t), st));   // overflow, invalid
     int grid = 0;
     int rc = coop_grid(ctx, 0, raht_schedule_kernel, 0, want, &grid);
     if (rc != GSNFS_OK) return rc;
-    void* args[] = {(void*)&d_keys, (void*)&d_weights, (void*)&n_voxels, (void*)&n_dev, (void*)&sp, (void*)&ctx->raht_plan};
+    void* args[] = {(void*)&d_keys, (void*)&d_weights, (void*)&n_voxels, (void*)&d_counts, (void*)&sp, (void*)&ctx->raht_plan,
+                    (void*)&ctx->d_flags};
     GSNFS_KERNEL(ctx, st, "raht_schedule");
     GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)raht_schedule_kernel, dim3(grid), dim3(256), args, 0, st));
     GSNFS_LAUNCH_CHECK(ctx, st);
     ctx->sched_n = n_voxels;
+    ctx->sched_stream = (void*)st;
   }
   QStepParams qs;
   for (int c = 0; c < GSNFS_MAX_CHANNELS; ++c) qs.step[c] = (qstep && c < channels) ? qstep[c] : 1.0f;

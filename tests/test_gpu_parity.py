@@ -335,6 +335,14 @@ def test_config3_headline_full_compare(B, ctx_big):
     print(f"config3: fraction of quantised coefficients off by one = {frac:.3e}")
 
 
+def test_config4_full_compare(B, ctx_big):
+    """BASELINE.json configs[3] (3M Gaussians, depth 18, qstep = range/1024) element by element against the oracle:
+    position coder bit-exact, coefficients rel-L2 <= 1e-5, quantised >= 99.99 % identical (rest +-1), decoded
+    attributes <= 1e-4 x range with the oracle's quantised coefficients."""
+    frac = full_pipeline_check(B, ctx_big, synth.make_frame(4))
+    print(f"config4: fraction of quantised coefficients off by one = {frac:.3e}")
+
+
 def test_config4_large_position_exact_and_raht_properties(B, ctx_big):
     fr = synth.make_frame(4)
     ref = orc.position_encode(fr.xyz, fr.bbox_min, fr.bbox_max, fr.depth)
@@ -355,25 +363,16 @@ def test_config4_large_position_exact_and_raht_properties(B, ctx_big):
     scale = torch.sqrt((w[:, None] * merged ** 2).sum(0))
     assert torch.all((Y[0] - dc_ref).abs() <= 2e-6 * scale)
     assert torch.allclose((Y ** 2).sum(0), (w[:, None] * merged ** 2).sum(0), rtol=1e-5)
-    # sampled coefficients, one by one, from the closed form over Morton-prefix ranges (fp64, numpy)
+    # sampled coefficients, one by one, from the oracle's closed form over Morton-prefix ranges (fp64)
     M = ref["voxel_keys"]
     mg = merged.cpu().numpy()
-    wn = ref["weights"].astype(np.float64)
-    P = np.concatenate([[0.0], np.cumsum(wn)])
+    wn = ref["weights"]
     Yn = Y.cpu().numpy()
     rng = np.random.default_rng(0)
     h_all = np.floor(np.log2((M[1:] ^ M[:-1]).astype(np.float64))).astype(np.int64)
     cand = np.concatenate([rng.integers(1, nv, 300), 1 + np.argsort(h_all)[-40:]])      # random + the top of the tree
-    for i in cand.tolist():
-        h = int(M[i] ^ M[i - 1]).bit_length() - 1
-        lo = np.searchsorted(M, (M[i] >> np.uint64(h + 1)) << np.uint64(h + 1))
-        hi = np.searchsorted(M, ((M[i] >> np.uint64(h)) + np.uint64(1)) << np.uint64(h))
-        W0, W1 = P[i] - P[lo], P[hi] - P[i]
-        T0 = (wn[lo:i, None] * mg[lo:i]).sum(0)
-        T1 = (wn[i:hi, None] * mg[i:hi]).sum(0)
-        yref = np.sqrt(W0 / (W0 + W1)) * T1 / np.sqrt(W1) - np.sqrt(W1 / (W0 + W1)) * T0 / np.sqrt(W0)
-        tol = 2e-6 * (np.abs(T1) / np.sqrt(W1) + np.abs(T0) / np.sqrt(W0)) + 1e-6
-        assert np.all(np.abs(Yn[i] - yref) <= tol), i
+    yref, ysc = orc.raht_coefficient_closed_form(mg, M, wn, cand, return_scale=True)
+    assert np.all(np.abs(Yn[cand] - yref) <= 2e-6 * ysc + 1e-6)        # fp32 rounding relative to the low-pass magnitudes
     # decode round trip on the GPU's own stream: voxels bit-exact, attributes within quantisation error
     B.decode_frame(ctx_big, buf, got["level_sizes"], got["occ_bytes"], fr.qstep, None)
     torch.cuda.synchronize()
@@ -547,3 +546,208 @@ def test_schedule_reuse_with_null_keys(B, ctx_small):
     with pytest.raises(B.GsnfsError) as e:
         B.gsnfs_raht_inverse(ctx_small, None, buf.weights, nv - 1, None, fr.depth, q1, None, fr.channels, fr.qstep, None, a2)
     assert e.value.status == B.GSNFS_E_INVALID_ARGUMENT
+
+
+# ---------------------------------------------------------------------------------------------- round 2
+def test_recon_bias_dequantiser(B, ctx_small):
+    """[R10] reconstruction bias delta != 0: the biased de-quantiser branch of the inverse kernel against the oracle's
+    dequantize (pinned by hand values in tests/test_oracle_raht.py), incl. rows of zeros (no bias on q == 0)."""
+    fr = synth.make_dense_frame(n=20_000, depth=6, channels=56, seed=12)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    buf, got = gpu_position_encode(B, ctx_small, fr)
+    nv = got["n_voxels"]
+    q_ref = ref["qcoeff"].copy()
+    q_ref[::7] = 0
+    dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], fr.depth)
+    ch_range = (fr.qstep.astype(np.float64) * fr.qdiv)[None, :]
+    for dz, bias in ((1.0 / 3.0, 0.25), (0.25, 0.25), (1.0 / 3.0, 1.0 / 6.0)):
+        bias32 = float(np.float32(bias))
+        buf.weights[:nv].copy_(_t(ref["weights"].astype(np.int32)))
+        buf.qcoeff[:nv].copy_(_t(q_ref.astype(np.int32)))
+        B.decode_frame(ctx_small, buf, ref["level_sizes"], len(ref["occ"]), fr.qstep, (dz, bias))
+        torch.cuda.synchronize()
+        ref_attr = orc.raht_inverse(orc.dequantize(q_ref, fr.qstep, bias32), dk, ref["weights"], fr.depth)
+        got_attr = buf.dec_attr[:nv].cpu().numpy().astype(np.float64)
+        assert np.all(np.abs(got_attr - ref_attr) <= 1e-4 * ch_range)
+        # and the bias is really applied: the unbiased reconstruction differs by much more than the tolerance
+        unb = orc.raht_inverse(orc.dequantize(q_ref, fr.qstep, 0.0), dk, ref["weights"], fr.depth)
+        assert np.max(np.abs(got_attr - unb) / ch_range) > 1e-3
+    for bad in ((1.5, 0.0), (-0.1, 0.0), (0.3, 1.0), (0.3, float("nan"))):
+        with pytest.raises(B.GsnfsError) as e:
+            B.decode_frame(ctx_small, buf, ref["level_sizes"], len(ref["occ"]), fr.qstep, bad)
+        assert e.value.status == B.GSNFS_E_INVALID_ARGUMENT
+
+
+def test_wide_context_survives_a_narrower_one(B):
+    """The dynamic shared-memory attribute of the transform kernels belongs to the function, not to a context:
+    creating a 56-channel context after a 208-channel one must not break the wide one."""
+    fr = synth.make_uniform_frame(3000, 6, 208, seed=6)
+    wide = B.Context(max_points=fr.n, max_channels=208, max_depth=fr.depth)
+    narrow = B.Context(max_points=fr.n, max_channels=56, max_depth=fr.depth)
+    try:
+        full_pipeline_check(B, narrow, synth.make_uniform_frame(3000, 6, 56, seed=7))
+        full_pipeline_check(B, wide, fr)
+    finally:
+        wide.close()
+        narrow.close()
+
+
+def test_invalid_keys_are_reported_not_silently_ignored(B, ctx_small):
+    """gsnfs.h: voxel keys must be sorted and unique.  A violation is found on the device: no output is written, status
+    bit 1 is set in d_counts, the next call on the context (or gsnfs_poll_status) returns the error once, and the
+    context keeps working afterwards."""
+    fr = synth.make_frame(1, n_override=20_000)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    nv = len(ref["voxel_keys"])
+    merged = _t(ref["merged"].astype(np.float32))
+    w = _t(ref["weights"].astype(np.int32))
+    good = _t(ref["voxel_keys"].astype(np.int64))
+    for kind in ("reversed", "duplicates", "shuffled"):
+        k = ref["voxel_keys"].astype(np.int64).copy()
+        if kind == "reversed":
+            k = k[::-1].copy()
+        elif kind == "duplicates":
+            k[nv // 2] = k[nv // 2 - 1]
+        else:
+            k = k[np.random.default_rng(1).permutation(nv)]
+        counts = torch.tensor([nv, 0, 0, 0], dtype=torch.int32, device=DEV)
+        q = torch.full((nv, fr.channels), 12345, dtype=torch.int32, device=DEV)
+        B.gsnfs_raht_forward(ctx_small, _t(k), w, nv, counts, fr.depth, merged, fr.channels, fr.qstep, None, q, None)
+        torch.cuda.synchronize()
+        assert int(counts.cpu()[2]) & 2, kind
+        assert bool((q == 12345).all()), kind                        # nothing was written
+        assert ctx_small.poll_status() != B.GSNFS_OK
+        assert ctx_small.poll_status() == B.GSNFS_OK                 # reported once
+        # without a poll, the next call reports it
+        B.gsnfs_raht_forward(ctx_small, _t(k), w, nv, None, fr.depth, merged, fr.channels, fr.qstep, None, q, None)
+        torch.cuda.synchronize()
+        with pytest.raises(B.GsnfsError):
+            B.gsnfs_raht_forward(ctx_small, good, w, nv, None, fr.depth, merged, fr.channels, fr.qstep, None, q, None)
+        # a failed call leaves no schedule to reuse
+        with pytest.raises(B.GsnfsError) as e:
+            B.gsnfs_raht_forward(ctx_small, None, w, nv, None, fr.depth, merged, fr.channels, fr.qstep, None, q, None)
+        assert e.value.status == B.GSNFS_E_INVALID_ARGUMENT
+    # and the context still works
+    q = torch.empty((nv, fr.channels), dtype=torch.int32, device=DEV)
+    B.gsnfs_raht_forward(ctx_small, good, w, nv, None, fr.depth, merged, fr.channels, fr.qstep, None, q, None)
+    torch.cuda.synchronize()
+    assert ctx_small.poll_status() == B.GSNFS_OK
+    check_quantised(q.cpu().numpy(), ref["qcoeff"])
+    # gsnfs_merge_raht_forward never reuses a schedule
+    buf, got = gpu_position_encode(B, ctx_small, fr)
+    with pytest.raises(B.GsnfsError) as e:
+        B.gsnfs_merge_raht_forward(ctx_small, None, buf.perm, buf.voxel_start, fr.n, buf.counts, fr.depth, _t(fr.attr),
+                                   fr.channels, fr.qstep, None, buf.weights, buf.qcoeff, None)
+    assert e.value.status == B.GSNFS_E_INVALID_ARGUMENT
+
+
+def test_adversarial_pending_fraction_depth21(B, ctx_small):
+    """voxel sets built to leave as many nodes pending per tile as the bound allows (long
+    single-child chains: every voxel differs from its neighbour in a different, very high bit) at depth 21 -- the
+    schedule must fit the context scratch and the result must still match the oracle."""
+    J = 21
+    rng = np.random.default_rng(5)
+    keys = set()
+    # combs: for many random prefixes, one voxel per bit position (a node with a single leaf hanging off each level)
+    for _ in range(1500):
+        base = int(rng.integers(0, 1 << 62))
+        for b in range(0, 63, 1):
+            keys.add((base ^ (1 << b)) & ((1 << 63) - 1))
+    vk = np.array(sorted(keys), dtype=np.uint64)[:90_000]
+    nv = len(vk)
+    w = rng.integers(1, 4, nv)
+    A = rng.normal(0, 1, (nv, 8))
+    qstep = synth.qstep_from_range(A.astype(np.float32), 256)
+    Yref = orc.raht_forward(A.astype(np.float32), vk, w, J)
+    coeff = torch.empty((nv, 8), dtype=torch.float32, device=DEV)
+    q = torch.empty((nv, 8), dtype=torch.int32, device=DEV)
+    counts = torch.tensor([nv, 0, 0, 0], dtype=torch.int32, device=DEV)
+    B.gsnfs_raht_forward(ctx_small, _t(vk.astype(np.int64)), _t(w.astype(np.int32)), nv, counts, J,
+                         _t(A.astype(np.float32)), 8, qstep, None, q, coeff)
+    torch.cuda.synchronize()
+    assert int(counts.cpu()[2]) == 0 and ctx_small.poll_status() == B.GSNFS_OK
+    assert rel_l2(coeff.cpu().numpy(), Yref).max() <= 1e-5
+    check_quantised(q.cpu().numpy(), orc.quantize(Yref, qstep))
+    back = torch.empty_like(coeff)
+    B.gsnfs_raht_inverse(ctx_small, _t(vk.astype(np.int64)), _t(w.astype(np.int32)), nv, None, J, None, coeff, 8, None, None, back)
+    torch.cuda.synchronize()
+    assert np.max(np.abs(back.cpu().numpy() - A.astype(np.float32))) <= 1e-4 * (A.max() - A.min())
+
+
+def test_decode_host_rejects_bad_header_before_copying(B, ctx_small):
+    fr = synth.make_frame(1, n_override=3000)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    n, C = fr.n, fr.channels
+    nv = len(ref["voxel_keys"])
+    pin = lambda *s, dt: torch.empty(s, dtype=dt).pin_memory()
+    h_occ = torch.from_numpy(ref["occ"].copy()).pin_memory()
+    h_w = torch.from_numpy(ref["weights"].astype(np.int32)).pin_memory()
+    h_q = torch.from_numpy(ref["qcoeff"].astype(np.int32)).pin_memory()
+    h_vx, h_out, h_cnt = pin(n, 3, dt=torch.int32), pin(n, C, dt=torch.float32), pin(4, dt=torch.int32)
+    h_out.fill_(7.0)
+    sizes = ref["level_sizes"].copy()
+    sizes[3] += 1; sizes[4] -= 1                                  # sum still right, levels shifted: caught on the device
+    B.gsnfs_frame_decode_host(ctx_small, h_occ, len(ref["occ"]), sizes, fr.depth, h_w, h_q, C, fr.qstep, None, h_vx, h_out, h_cnt)
+    assert int(h_cnt[2]) & 1
+    sizes = ref["level_sizes"].copy()
+    sizes[2] = 0                                                  # caught on the host: nothing is copied or written
+    h_out.fill_(7.0)
+    B.gsnfs_frame_decode_host(ctx_small, h_occ, len(ref["occ"]), sizes, fr.depth, h_w, h_q, C, fr.qstep, None, h_vx, h_out, h_cnt)
+    assert int(h_cnt[2]) & 1 and bool((h_out == 7.0).all())
+    h_w0 = h_w.clone().pin_memory()
+    h_w0[5] = 0
+    with pytest.raises(B.GsnfsError):
+        B.gsnfs_frame_decode_host(ctx_small, h_occ, len(ref["occ"]), ref["level_sizes"], fr.depth, h_w0, h_q, C, fr.qstep,
+                                  None, h_vx, h_out, h_cnt)
+    B.gsnfs_frame_decode_host(ctx_small, h_occ, len(ref["occ"]), ref["level_sizes"], fr.depth, h_w, h_q, C, fr.qstep, None,
+                              h_vx, h_out, h_cnt)
+    assert int(h_cnt[2]) == 0 and int(h_cnt[0]) == nv
+
+
+def test_beyond_l2_16m_position_exact_and_sampled_coefficients(B):
+    """DESIGN.md's "beyond L2" point (config-3 recipe, N = 16M: key arrays no longer fit the 126 MB L2): position coder
+    bit-exact against the oracle; transform checked on sampled rows against the oracle's closed form and by the
+    size-independent invariants; decode round trip bit-exact on positions."""
+    fr = synth.make_frame(3, n_override=16_000_000)
+    ref = orc.position_encode(fr.xyz, fr.bbox_min, fr.bbox_max, fr.depth)
+    ctx = B.Context(max_points=fr.n, max_channels=fr.channels, max_depth=fr.depth)
+    try:
+        buf, got = gpu_position_encode(B, ctx, fr)
+        check_position(got, ref, fr.n)
+        nv = got["n_voxels"]
+        d_attr = _t(fr.attr)
+        coeff = buf.merged                                           # reuse as the unquantised output buffer
+        B.gsnfs_merge_raht_forward(ctx, buf.voxel_keys, buf.perm, buf.voxel_start, fr.n, buf.counts, fr.depth, d_attr,
+                                   fr.channels, fr.qstep, None, buf.weights, buf.qcoeff, coeff)
+        torch.cuda.synchronize()
+        assert ctx.poll_status() == B.GSNFS_OK
+        M, wn = ref["voxel_keys"], ref["weights"]
+        merged = orc.merge_attributes(fr.attr, ref["perm"], ref["voxel_start"])
+        rng = np.random.default_rng(0)
+        h_all = np.floor(np.log2((M[1:] ^ M[:-1]).astype(np.float64))).astype(np.int64)
+        cand = np.concatenate([[0], rng.integers(1, nv, 400), 1 + np.argsort(h_all)[-60:]])
+        yref, ysc = orc.raht_coefficient_closed_form(merged, M, wn, cand, return_scale=True)
+        Ys = coeff[torch.from_numpy(cand).to(DEV)].cpu().numpy().astype(np.float64)
+        assert np.all(np.abs(Ys - yref) <= 2e-6 * ysc + 1e-6)
+        qs = orc.quantize(yref, fr.qstep)
+        qd = buf.qcoeff[torch.from_numpy(cand).to(DEV)].cpu().numpy().astype(np.int64) - qs
+        assert np.all(np.abs(qd) <= 1) and (qd != 0).mean() <= 2e-3       # 460 x 56 samples: a handful of +-1 at most
+        # Parseval on sqrt(w)-scaled rows, all 16M x 56 coefficients
+        en_in = torch.zeros(fr.channels, dtype=torch.float64, device=DEV)
+        en_out = torch.zeros(fr.channels, dtype=torch.float64, device=DEV)
+        for a in range(0, nv, 2_000_000):
+            en_out += (coeff[a:a + 2_000_000].double() ** 2).sum(0)
+        en_in = torch.from_numpy((wn[:, None] * merged ** 2).sum(0)).to(DEV)
+        assert torch.allclose(en_out, en_in, rtol=1e-5)
+        B.decode_frame(ctx, buf, got["level_sizes"], got["occ_bytes"], fr.qstep)
+        torch.cuda.synchronize()
+        assert int(buf.dec_counts.cpu()[2]) == 0
+        assert torch.equal(buf.dec_keys[:nv], buf.voxel_keys[:nv])
+        dc = orc.morton_decode(M, fr.depth)
+        assert np.array_equal(buf.dec_xyz[:nv].cpu().numpy().astype(np.uint64), dc)
+        err = (buf.dec_attr[:nv].double() - torch.from_numpy(merged).to(DEV)) * torch.sqrt(torch.from_numpy(wn.astype(np.float64)).to(DEV))[:, None]
+        rms = torch.sqrt((err ** 2).mean(0))
+        qsd = torch.from_numpy(fr.qstep.astype(np.float64)).to(DEV)
+        assert torch.all(rms <= (2.0 / 3.0) * qsd * (1 + 1e-3) + 1e-7)
+    finally:
+        ctx.close()

@@ -266,16 +266,18 @@ def test_quantize_reciprocal_arithmetic():
         t = abs(Fraction(float(Y[r, c]))) / Fraction(float(step[c])) + Fraction(1.0 / 3.0)
         if abs(t - round(t)) > Fraction(1, 10**9):                       # away from a boundary both forms agree with exact
             assert abs(int(q[r, c])) == int(t // 1) and np.sign(q[r, c]) == np.sign(Y[r, c]) * (int(t // 1) > 0)
-    # search a point where floor(|y| / D + f) and floor(|y| * (1/D) + f) differ; the oracle must follow the reciprocal form
-    D = np.float64(np.float32(0.1))
+    # points where floor(|y| / D + f) and floor(|y| * (1/D) + f) differ (D = fp32(0.003): y = k D with |y| / D = k exactly
+    # but |y| * (1/D) one ulp below k for many k): the oracle must follow the reciprocal form
+    D = np.float64(np.float32(0.003))
     inv = 1.0 / D
     k = np.arange(1, 200000, dtype=np.float64)
-    y = k * D                                                            # |y| / D is k or k -+ 1 ulp
+    y = k * D
     a, b = np.floor(y / D), np.floor(y * inv)
     diff = np.flatnonzero(a != b)
-    if diff.size:
-        yy = y[diff[:50], None]
-        assert np.array_equal(orc.quantize(yy, np.array([0.1], np.float32), 0.0)[:, 0], b[diff[:50]].astype(np.int64))
+    assert diff.size > 1000
+    yy = y[diff[:200], None]
+    got = orc.quantize(yy, np.array([0.003], np.float32), 0.0)[:, 0]
+    assert np.array_equal(got, b[diff[:200]].astype(np.int64)) and not np.array_equal(got, a[diff[:200]].astype(np.int64))
 
 
 @pytest.mark.parametrize("J,nv,seed,weighted", [(3, 40, 1, False), (4, 300, 2, True), (7, 1500, 3, True), (2, 9, 4, True)])
