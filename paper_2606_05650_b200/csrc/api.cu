@@ -104,7 +104,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->oct_tiles_cap = (uint32_t)otiles;
   c->occ_cap = gsnfs_occ_capacity(N, c->max_depth) + 16;
   c->scan_tiles_cap = (uint32_t)((c->occ_cap > N ? c->occ_cap : N) / kScanTile + 2);
-  c->raht_pool_rows = N + 8192;
+  c->raht_pool_rows = N + 16384;          // sum of the phase sizes M_p, p >= 2
   c->raht_hdr_cap = 2 * N / kRahtTile + 4 * kRahtMaxPhases + 64;
   c->raht_rec_cap = c->raht_hdr_cap * kRahtTile;
 
@@ -120,7 +120,7 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_ometa = b.take((size_t)2 * kOctLevels * 4);
   const size_t o_ssums = b.take((size_t)c->scan_tiles_cap * 4);
   c->raht_bsum_cap = (uint32_t)(c->raht_hdr_cap / 256 + 2 * kRahtMaxPhases + 8);
-  const size_t o_ridx = b.take(c->raht_rec_cap * 4), o_rpw = b.take(c->raht_rec_cap * 4);
+  const size_t o_rpend = b.take(c->raht_hdr_cap * 128 * sizeof(uint4));
   const size_t o_rbs = b.take((size_t)c->raht_bsum_cap * 4);
   const size_t o_rgs = b.take(N * 4);
   const size_t o_rrec = b.take(c->raht_rec_cap * sizeof(uint4));
@@ -138,7 +138,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->sort_zero_bytes = o_zero_end - o_hist;
   c->oct_hist = (uint32_t*)(p + o_ohist); c->oct_base = (uint32_t*)(p + o_obase); c->oct_meta = (uint32_t*)(p + o_ometa);
   c->scan_sums = (uint32_t*)(p + o_ssums);
-  c->raht_idx = (uint32_t*)(p + o_ridx); c->raht_pw = (uint32_t*)(p + o_rpw); c->raht_bsum = (uint32_t*)(p + o_rbs);
+  c->raht_pend = (uint4*)(p + o_rpend); c->raht_bsum = (uint32_t*)(p + o_rbs);
   c->raht_rec = (uint4*)(p + o_rrec); c->raht_gsrc = (uint32_t*)(p + o_rgs);
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
@@ -185,6 +185,17 @@ void gsnfs_destroy(gsnfs_ctx* ctx) {
   if (ctx->fpool) cudaFree(ctx->fpool);
   free(ctx);
 }
+
+#ifdef GSNFS_TIMELINE
+int gsnfs_debug_read_plan(gsnfs_ctx* ctx, void* h_out, uint64_t bytes) {   // developer builds only; not in gsnfs.h
+  if (!ctx || !h_out) return GSNFS_E_INVALID_ARGUMENT;
+  if (bytes > sizeof(RahtPlan)) bytes = sizeof(RahtPlan);
+  GSNFS_ON_DEVICE(ctx);
+  GSNFS_CUDA_OK(ctx, cudaDeviceSynchronize());
+  GSNFS_CUDA_OK(ctx, cudaMemcpy(h_out, ctx->raht_plan, bytes, cudaMemcpyDeviceToHost));
+  return GSNFS_OK;
+}
+#endif
 
 int gsnfs_profile_start(gsnfs_ctx* ctx, int max_records) {
   if (!ctx || max_records < 1) return GSNFS_E_INVALID_ARGUMENT;

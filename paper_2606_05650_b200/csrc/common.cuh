@@ -9,7 +9,7 @@
 namespace gsnfs {
 
 constexpr int kRahtTile = 256;       // entries per RAHT tile (rows staged in shared memory)
-constexpr int kRahtMaxPhases = 30;   // >= worst-case number of tile phases
+constexpr int kRahtMaxPhases = 34;   // >= worst-case number of tile phases
 constexpr int kSortItems = 16;       // keys per thread in a onesweep tile
 constexpr int kSortThreads = 256;
 constexpr int kSortTile = kSortItems * kSortThreads;
@@ -43,6 +43,9 @@ struct RahtPlan {
   uint32_t M[kRahtMaxPhases + 2];     // active entries of phase p (1-based); M[1] = N_v
   uint32_t poff[kRahtMaxPhases + 2];  // row offset of phase p (p >= 2) in the idx / pending-row pools
   uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
+#ifdef GSNFS_TIMELINE                 // developer builds only: globaltimer (ns) stamps written by CTA 0
+  unsigned long long t_stamp[64];
+#endif
 };
 
 struct ProfRec {
@@ -90,8 +93,7 @@ struct gsnfs_ctx {
   uint32_t scan_tiles_cap;
 
   // RAHT
-  uint32_t* raht_idx;      // pending-entry first-voxel indices, tile strided (raht_hdr_cap x kRahtTile)
-  uint32_t* raht_pw;       // pending-entry node weights, same indexing
+  uint4* raht_pend;        // pending entries {code, first voxel, node weight}, tile strided (raht_hdr_cap x 128)
   uint32_t* raht_bsum;     // pending counts summed per 256 tiles
   uint32_t* raht_gsrc;     // fused merge: first Gaussian of every voxel
   uint32_t raht_bsum_cap;
@@ -175,6 +177,16 @@ __device__ __forceinline__ unsigned lanemask_le() {
   asm("mov.u32 %0, %%lanemask_le;" : "=r"(m));
   return m;
 }
+#ifdef GSNFS_TIMELINE
+__device__ __forceinline__ unsigned long long globaltimer_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+#define GSNFS_TSTAMP(plan, i) do { if (blockIdx.x == 0 && threadIdx.x == 0 && (i) < 64) (plan)->t_stamp[(i)] = globaltimer_ns(); } while (0)
+#else
+#define GSNFS_TSTAMP(plan, i) do { } while (0)
+#endif
 __device__ __forceinline__ uint32_t ld_volatile_u32(const uint32_t* p) {
   uint32_t v;
   asm volatile("ld.volatile.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");

@@ -17,7 +17,7 @@
 // cooperative kernel -- the paper's "prelude" -- and is shared by the forward and the inverse transform.
 #include <cooperative_groups.h>
 
-#include "common.cuh"
+#include "raht.cuh"
 
 namespace cg = cooperative_groups;
 
@@ -61,333 +61,6 @@ __device__ __forceinline__ void bulk_commit() { asm volatile("cp.async.bulk.comm
 __device__ __forceinline__ void bulk_wait_read() { asm volatile("cp.async.bulk.wait_group.read 0;" ::: "memory"); }
 __device__ __forceinline__ void bulk_wait_all() { asm volatile("cp.async.bulk.wait_group 0;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
-
-__device__ __forceinline__ uint32_t lower_bound_u64(const uint64_t* a, uint32_t lo, uint32_t hi, uint64_t x) {
-  while (lo < hi) {                      // first index in [lo, hi) with a[idx] >= x, else hi
-    const uint32_t mid = (lo + hi) >> 1;
-    if (a[mid] < x) lo = mid + 1; else hi = mid;
-  }
-  return lo;
-}
-
-// Block-wide search in the exclusive prefix E of vals[0..n) (all vals > 0 where it matters): returns the
-// index i and E(i) with E(i) <= target < E(i+1), and the grand total.  All 256 threads must call it.
-struct PrefixHit { uint32_t idx, before, total; };
-__device__ PrefixHit block_prefix_find(const uint32_t* vals, uint32_t n, uint32_t target, uint32_t* s_scan /*9*/,
-                                       uint32_t* s_hit /*2*/) {
-  uint32_t running = 0;
-  if (threadIdx.x == 0) { s_hit[0] = 0; s_hit[1] = 0; }
-  __syncthreads();
-  for (uint32_t base = 0; base < n; base += 256) {
-    const uint32_t i = base + threadIdx.x;
-    const uint32_t v = i < n ? ((const volatile uint32_t*)vals)[i] : 0u;
-    uint32_t tot;
-    const uint32_t ex = block_excl_scan_256(v, s_scan, &tot) + running;
-    if (v && ex <= target && target < ex + v) { s_hit[0] = i; s_hit[1] = ex; }
-    running += tot;
-  }
-  __syncthreads();
-  PrefixHit h;
-  h.idx = s_hit[0]; h.before = s_hit[1]; h.total = running;
-  __syncthreads();
-  return h;
-}
-
-// ------------------------------------------------------------------------------------------------
-// Schedule ("prelude"): all phases in one cooperative launch, one grid-wide barrier per phase.
-//
-// Phase p works on a list of M_p nodes (phase 1: the voxels), each with the index of its first voxel
-// (vidx), its weight and -- through vidx -- its Morton code.  Tile t of the phase:
-//   * finds, for every entry k > 0 of the tile, whether its butterfly is local (both sibling ranges, found
-//     by binary search of the Morton prefixes, end inside the tile or at a tile edge whose neighbour has a
-//     higher differing bit); computes W0, W1 from a tile-local weight prefix and a = sqrt(W0/(W0+W1)), b;
-//   * sorts the local butterflies by level into records {k | left<<8 | level<<16, a, b, vidx};
-//   * emits the pending entries (vidx, weight of the merged node) tile-strided for the next phase, their
-//     count, and adds the count into a per-256-tiles bucket sum.
-// After the barrier, phase p+1 maps its entry index to (source tile, rank) through the bucket sums and
-// the per-tile counts, so the pending lists never have to be compacted.
-// ------------------------------------------------------------------------------------------------
-struct SchedPools {
-  uint4* rec;            // (toff + tile) * T + j
-  RahtTileHdr* hdr;      // toff + tile
-  uint32_t* pend_vidx;   // (toff + tile) * T + rank
-  uint32_t* pend_w;      // same indexing
-  uint32_t* tile_pend;   // toff + tile
-  uint32_t* bsum;        // boff + tile / 256
-  uint32_t hdr_cap;
-  uint32_t bsum_cap;
-  uint32_t pool_rows;    // capacity of the pending-row pool used by the transform kernels
-  // fused merge (gsnfs_merge_raht_forward): leaf weight = run length in the sorted permutation
-  const uint32_t* perm;      // NULL unless fused
-  const uint32_t* vstart;
-  uint32_t* gsrc;            // out: index of the first Gaussian of every voxel
-  uint32_t* weights_out;     // out: run lengths
-};
-
-__global__ void __launch_bounds__(256) raht_schedule_kernel(
-    const uint64_t* __restrict__ keys, const uint32_t* __restrict__ weights, uint32_t n_host,
-    gsnfs_counts* __restrict__ counts, SchedPools sp, RahtPlan* __restrict__ plan, uint32_t* __restrict__ sticky) {
-  cg::grid_group grid = cg::this_grid();
-  __shared__ uint64_t s_key[T];
-  __shared__ uint32_t s_wpre[T + 1];       // tile-local exclusive prefix of the entry weights
-  __shared__ uint32_t s_E[T + 1];          // exclusive prefix of source-tile pending counts
-  __shared__ uint16_t s_wl[8][64];
-  __shared__ uint32_t s_tot[64];
-  __shared__ uint32_t s_lstart[64];
-  __shared__ uint16_t s_segend[64];
-  __shared__ uint32_t s_nseg;
-  __shared__ uint32_t s_pmask[8];
-  __shared__ uint64_t s_edge[2];
-  __shared__ uint32_t s_scan[9];
-  __shared__ uint32_t s_hit[2];
-
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  // a frame the decoder flagged corrupt (status != 0) has no transform: N_v = 0 makes every later kernel a no-op
-  const uint32_t Nv = counts ? (counts->status ? 0u : min(counts->n_voxels, n_host)) : n_host;
-  uint32_t M = Nv, toff = 0, boff = 0;
-  bool overflow = false;
-  uint32_t toff_prev = 0, boff_prev = 0, ntiles_prev = 0, poff = 0;
-  int p = 1;
-  if (blockIdx.x == 0 && tid == 0) {
-    plan->M[0] = 0; plan->M[1] = Nv; plan->poff[1] = 0; plan->toff[1] = 0; plan->nphases = 1;   // overflow / invalid: cleared by the host
-  }
-  while (true) {
-    const uint32_t ntiles = (M + T - 1) / T;
-    const uint32_t nb = (ntiles + 255) / 256;
-    const uint32_t nb_prev = (ntiles_prev + 255) / 256;
-    if (toff + ntiles > sp.hdr_cap || boff + nb > sp.bsum_cap) {      // uniform over the grid
-      overflow = true;
-      break;
-    }
-    // side job (p >= 2): exclusive offsets of the previous phase's pending lists -> its tile headers
-    if (p >= 2) {
-      for (uint32_t b = blockIdx.x; b < nb_prev; b += gridDim.x) {
-        uint32_t part = 0;
-        for (uint32_t i = tid; i < b; i += 256) part += ((const volatile uint32_t*)sp.bsum)[boff_prev + i];
-        part = __reduce_add_sync(0xffffffffu, part);
-        if (lane == 0) s_scan[warp] = part;
-        __syncthreads();
-        uint32_t bpre = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) bpre += s_scan[w];
-        __syncthreads();
-        const uint32_t t = b * 256 + tid;
-        const uint32_t v = t < ntiles_prev ? ((const volatile uint32_t*)sp.tile_pend)[toff_prev + t] : 0u;
-        const uint32_t ex = block_excl_scan_256(v, s_scan, nullptr);
-        if (t < ntiles_prev) sp.hdr[toff_prev + t].pend_off = bpre + ex;
-      }
-    }
-
-    for (uint32_t tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-      const uint32_t ks = tile * T;
-      const uint32_t cnt = min((uint32_t)T, M - ks);
-      const bool valid = (uint32_t)tid < cnt;
-      const bool has_prev = ks > 0, has_next = ks + cnt < M;
-      uint32_t vidx = 0xffffffffu, went = 0;
-      uint64_t mk = ~0ull;
-      if (p == 1) {
-        if (valid) {
-          vidx = ks + tid;
-          mk = keys[vidx];
-          if (sp.perm) {
-            const uint32_t s0 = sp.vstart[vidx], s1 = sp.vstart[vidx + 1];
-            went = s1 - s0;
-            sp.gsrc[vidx] = sp.perm[s0];
-            sp.weights_out[vidx] = went;
-          } else {
-            went = weights ? weights[vidx] : 1u;
-          }
-        }
-        if (tid == 0) {
-          s_edge[0] = has_prev ? keys[ks - 1] : 0ull;
-          s_edge[1] = has_next ? keys[ks + cnt] : 0ull;
-        }
-      } else {
-        // entry (ks + k) of this phase = rank-th pending entry of source tile t: E(t) <= ks + k < E(t+1)
-        const PrefixHit hb = block_prefix_find(sp.bsum + boff_prev, nb_prev, ks, s_scan, s_hit);
-        const uint32_t tb = hb.idx * 256;
-        const uint32_t nin = min(256u, ntiles_prev - tb);
-        const PrefixHit ht = block_prefix_find(sp.tile_pend + toff_prev + tb, nin, ks - hb.before, s_scan, s_hit);
-        const uint32_t t0 = tb + ht.idx;                 // source tile holding entry ks
-        const uint32_t e0 = hb.before + ht.before;       // E(t0)
-        {
-          const uint32_t t = t0 + tid;
-          const uint32_t v = t < ntiles_prev ? ((const volatile uint32_t*)sp.tile_pend)[toff_prev + t] : 0u;
-          uint32_t tot;
-          const uint32_t ex = block_excl_scan_256(v, s_scan, &tot);
-          s_E[tid] = e0 + ex;
-          if (tid == 0) s_E[T] = e0 + tot;
-        }
-        __syncthreads();
-        if (valid) {
-          const uint32_t gk = ks + tid;
-          uint32_t lo = 0, hi = T;                       // last i in [0, T] with s_E[i] <= gk
-          while (lo < hi) { const uint32_t mid = (lo + hi + 1) >> 1; if (s_E[mid] <= gk) lo = mid; else hi = mid - 1; }
-          const size_t src = (size_t)(toff_prev + t0 + lo) * T + (gk - s_E[lo]);
-          vidx = ((const volatile uint32_t*)sp.pend_vidx)[src];
-          went = ((const volatile uint32_t*)sp.pend_w)[src];
-          mk = keys[vidx];
-        }
-        if (tid == 0) {
-          uint64_t kp = 0, kn = 0;
-          if (has_prev) {                                // entry ks - 1: rank-1 in t0, or the last of tile t0-1
-            const uint32_t r0 = ks - e0;
-            const size_t src = r0 > 0 ? (size_t)(toff_prev + t0) * T + (r0 - 1)
-                                      : (size_t)(toff_prev + t0 - 1) * T +
-                                            (((const volatile uint32_t*)sp.tile_pend)[toff_prev + t0 - 1] - 1);
-            kp = keys[((const volatile uint32_t*)sp.pend_vidx)[src]];
-          }
-          if (has_next) {
-            const uint32_t gk = ks + cnt;
-            uint32_t lo = 0, hi = T;
-            while (lo < hi) { const uint32_t mid = (lo + hi + 1) >> 1; if (s_E[mid] <= gk) lo = mid; else hi = mid - 1; }
-            kn = keys[((const volatile uint32_t*)sp.pend_vidx)[(size_t)(toff_prev + t0 + lo) * T + (gk - s_E[lo])]];
-          }
-          s_edge[0] = kp; s_edge[1] = kn;
-        }
-      }
-      s_key[tid] = mk;
-      if (p == 1 && valid && went == 0u) plan->invalid = 1u;          // a leaf of weight 0 has no transform [R1]
-      for (int i = tid; i < 8 * 64; i += 256) (&s_wl[0][0])[i] = 0;
-      {
-        uint32_t tot;
-        const uint32_t ex = block_excl_scan_256(went, s_scan, &tot);     // (contains the barriers)
-        s_wpre[tid] = ex;
-        if (tid == 0) s_wpre[T] = tot;
-      }
-      __syncthreads();
-      const uint64_t x_first = s_edge[0] ^ s_key[0];
-      const uint64_t x_end = s_edge[1] ^ s_key[cnt - 1];
-      const int hfirst = has_prev ? (x_first ? msb64(x_first) : 0) : 64;
-      const int hend = has_next ? (x_end ? msb64(x_end) : 0) : 64;
-      bool local = false;
-      int level = 0;
-      uint32_t l = 0;
-      float fa = 0.f, fb = 0.f;
-      // the codes must be sorted and unique (gsnfs.h); a violation is reported, never silently transformed
-      if (valid && (tid > 0 ? s_key[tid - 1] >= mk : (has_prev && s_edge[0] >= mk))) plan->invalid = 1u;
-      if (valid && tid > 0) {
-        const uint64_t x = s_key[tid - 1] ^ mk;
-        const int h = x ? msb64(x) : 0;                            // x == 0 only for invalid (non-unique) input
-        const uint64_t lowp = (mk >> (h + 1)) << (h + 1);
-        const uint64_t hip = ((mk >> h) + 1ull) << h;
-        l = lower_bound_u64(s_key, 0, tid, lowp);
-        const uint32_t r = lower_bound_u64(s_key, tid + 1, cnt, hip);
-        local = (l > 0 || hfirst > h) && (r < cnt || hend > h);
-        if (local) {
-          level = h + 1;
-          const uint32_t pk = s_wpre[tid];
-          const uint32_t pr = (r == cnt) ? s_wpre[T] : s_wpre[r];       // entries >= cnt carry weight 0
-          const double w0 = (double)(pk - s_wpre[l]);
-          const double w1 = (double)(pr - pk);
-          fa = (float)sqrt(w0 / (w0 + w1));
-          fb = (float)sqrt(w1 / (w0 + w1));
-        }
-      }
-      // rank among the tile's butterflies of the same level (warp match, then prefix over warps)
-      const unsigned peers = __match_any_sync(0xffffffffu, level);
-      const unsigned lt = peers & lanemask_lt();
-      if (local && lt == 0) s_wl[warp][level - 1] = (uint16_t)__popc(peers);
-      const unsigned pend_b = __ballot_sync(0xffffffffu, valid && !local);
-      if (lane == 0) s_pmask[warp] = pend_b;
-      __syncthreads();
-      if (tid < 64) {
-        uint32_t run = 0;
-#pragma unroll
-        for (int w = 0; w < 8; ++w) { const uint32_t c = s_wl[w][tid]; s_wl[w][tid] = (uint16_t)run; run += c; }
-        s_tot[tid] = run;
-      }
-      __syncthreads();
-      if (warp == 0) {                      // exclusive scan of the 64 level totals + compact list of non-empty levels
-        const uint32_t t0 = s_tot[2 * lane], t1 = s_tot[2 * lane + 1];
-        uint32_t inc = t0 + t1;
-#pragma unroll
-        for (int o = 1; o < 32; o <<= 1) { uint32_t y = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += y; }
-        const uint32_t ex = inc - (t0 + t1);
-        s_lstart[2 * lane] = ex;
-        s_lstart[2 * lane + 1] = ex + t0;
-        const unsigned b0 = __ballot_sync(0xffffffffu, t0 > 0), b1 = __ballot_sync(0xffffffffu, t1 > 0);
-        const uint32_t pos = __popc(b0 & lanemask_lt()) + __popc(b1 & lanemask_lt());
-        if (t0 > 0) s_segend[pos] = (uint16_t)(ex + t0);
-        if (t1 > 0) s_segend[pos + (t0 > 0 ? 1 : 0)] = (uint16_t)(ex + t0 + t1);
-        if (lane == 0) s_nseg = __popc(b0) + __popc(b1);
-      }
-      __syncthreads();
-      const size_t tbase = (size_t)(toff + tile) * T;
-      RahtTileHdr* h_out = sp.hdr + toff + tile;
-      if (local) {
-        const uint32_t j = s_lstart[level - 1] + s_wl[warp][level - 1] + __popc(lt);
-        uint4 rr;
-        rr.x = (uint32_t)tid | (l << 8) | ((uint32_t)level << 16);
-        rr.y = __float_as_uint(fa);
-        rr.z = __float_as_uint(fb);
-        rr.w = vidx;
-        sp.rec[tbase + j] = rr;
-      }
-      uint32_t np = 0, before = 0;
-#pragma unroll
-      for (int w = 0; w < 8; ++w) { const uint32_t c = __popc(s_pmask[w]); if (w < warp) before += c; np += c; }
-      if (valid && !local) {
-        // pending node = this entry plus everything merged into it: up to the next pending entry
-        const uint32_t rank = before + __popc(s_pmask[warp] & lanemask_lt());
-        uint32_t nxt = cnt;                                          // next pending entry after tid
-        {
-          unsigned m = s_pmask[warp] & ~lanemask_le();
-          int w = warp;
-          while (m == 0 && ++w < 8) m = s_pmask[w];
-          if (m) nxt = (uint32_t)(w * 32 + __ffs(m) - 1);
-        }
-        const uint32_t pn = (nxt >= cnt) ? s_wpre[T] : s_wpre[nxt];
-        sp.pend_vidx[tbase + rank] = vidx;
-        sp.pend_w[tbase + rank] = pn - s_wpre[tid];
-      }
-      if (tid < 64) h_out->lev_end[tid] = tid < (int)s_nseg ? s_segend[tid] : (uint16_t)0;
-      if (tid < 8) h_out->pendmask[tid] = s_pmask[tid];
-      if (tid == 0) {
-        h_out->npend = np;
-        h_out->nent = cnt | (s_nseg << 16);
-        h_out->nmerge = cnt - np;
-        h_out->pend_off = 0;
-        sp.tile_pend[toff + tile] = np;
-        atomicAdd(&sp.bsum[boff + tile / 256], np);
-      }
-      __syncthreads();
-    }
-    grid.sync();
-    uint32_t part = 0;
-    for (uint32_t i = tid; i < nb; i += 256) part += ((const volatile uint32_t*)sp.bsum)[boff + i];
-    part = __reduce_add_sync(0xffffffffu, part);
-    if (lane == 0) s_scan[warp] = part;
-    __syncthreads();
-    uint32_t M_next = 0;
-#pragma unroll
-    for (int w = 0; w < 8; ++w) M_next += s_scan[w];
-    __syncthreads();
-    const uint32_t poff_next = (p == 1) ? 0u : poff + M;
-    if (blockIdx.x == 0 && tid == 0) {
-      plan->M[p + 1] = M_next; plan->poff[p + 1] = poff_next; plan->toff[p + 1] = toff + ntiles;
-    }
-    if ((uint64_t)poff_next + M_next > sp.pool_rows || (M_next > 1 && p + 1 > kRahtMaxPhases)) {
-      overflow = true;
-      break;
-    }
-    if (M_next <= 1) break;
-    toff_prev = toff; boff_prev = boff; ntiles_prev = ntiles;
-    poff = poff_next;
-    toff += ntiles; boff += nb;
-    M = M_next;
-    ++p;
-  }
-  if (blockIdx.x == 0 && tid == 0) {
-    plan->nphases = (uint32_t)p;
-    if (overflow || *(volatile uint32_t*)&plan->invalid) {   // loud: the transform kernels write nothing; the caller sees status bit 1
-      plan->overflow = 1;
-      if (counts) atomicOr(&counts->status, 2u);
-      *sticky = 1u;
-      __threadfence_system();
-    }
-  }
-}
 
 // ------------------------------------------------------------------------------------------------
 // Transform kernels.  VEC = 4: channels % 4 == 0 (float4 rows);  VEC = 1: any channel count.
@@ -986,7 +659,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   if (n_voxels == 0) return GSNFS_OK;
   const uint32_t want = (n_voxels + T - 1) / T;
   SchedPools sp;
-  sp.rec = ctx->raht_rec; sp.hdr = ctx->raht_hdr; sp.pend_vidx = ctx->raht_idx; sp.pend_w = ctx->raht_pw;
+  sp.rec = ctx->raht_rec; sp.hdr = ctx->raht_hdr; sp.pend = reinterpret_cast<PendRec*>(ctx->raht_pend);
   sp.tile_pend = ctx->raht_tile_pend; sp.bsum = ctx->raht_bsum;
   sp.hdr_cap = (uint32_t)ctx->raht_hdr_cap; sp.bsum_cap = ctx->raht_bsum_cap; sp.pool_rows = (uint32_t)ctx->raht_pool_rows;
   const bool fused = d_perm != nullptr;
@@ -995,16 +668,8 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   GatherArgs ga;
   ga.gsrc = fused ? ctx->raht_gsrc : nullptr; ga.perm = d_perm; ga.vstart = d_vstart;
   if (d_keys) {                                  // NULL: the schedule of the previous call on this context is reused
-    GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
-    GSNFS_CUDA_OK(ctx, cudaMemsetAsync(&ctx->raht_plan->overflow, 0, 2 * sizeof(uint32_t), st));   // overflow, invalid
-    int grid = 0;
-    int rc = coop_grid(ctx, 0, raht_schedule_kernel, 0, want, &grid);
+    int rc = launch_raht_schedule(ctx, st, d_keys, d_weights, n_voxels, d_counts, sp);
     if (rc != GSNFS_OK) return rc;
-    void* args[] = {(void*)&d_keys, (void*)&d_weights, (void*)&n_voxels, (void*)&d_counts, (void*)&sp, (void*)&ctx->raht_plan,
-                    (void*)&ctx->d_flags};
-    GSNFS_KERNEL(ctx, st, "raht_schedule");
-    GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)raht_schedule_kernel, dim3(grid), dim3(256), args, 0, st));
-    GSNFS_LAUNCH_CHECK(ctx, st);
     ctx->sched_n = n_voxels;
     ctx->sched_stream = (void*)st;
   }
