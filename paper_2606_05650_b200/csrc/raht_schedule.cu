@@ -90,6 +90,7 @@ struct __align__(16) TileSmem {   // double buffered: tile i+1 fills its set whi
   uint32_t hist[64];         // butterflies per depth bucket
   uint32_t start[64];
   uint32_t pmask[8];
+  uint32_t nonunit[8];       // per warp: some entry weight != 1 (phase 1: the transform kernels scale those rows [R2])
   uint64_t edge[2];
   uint64_t scan64[9];
   int dmax;
@@ -276,7 +277,8 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
         if (lane == 0 && dm >= 0) atomicMax(&S.dmax, dm + 1);
       }
       const unsigned pend_b = __ballot_sync(0xffffffffu, valid && !local);
-      if (lane == 0) S.pmask[warp] = pend_b;
+      const unsigned nu_b = __ballot_sync(0xffffffffu, valid && went != 1u);
+      if (lane == 0) { S.pmask[warp] = pend_b; S.nonunit[warp] = nu_b; }
       __syncthreads();                                                                       // (6)
       const int dmax = S.dmax - 1;                       // stored biased by one: 0 = no butterfly in the tile
       float fa = 0.f, fb = 0.f;
@@ -344,7 +346,10 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
       if (tid == 0) {
         if (np > (uint32_t)kPendCap) plan->invalid = 1u;             // impossible for sorted unique codes
         h_out->npend = np;
-        h_out->nent = cnt | (nseg << 16);
+        uint32_t nu = 0;
+#pragma unroll
+        for (int w = 0; w < 8; ++w) nu |= S.nonunit[w];
+        h_out->nent = cnt | (nseg << 16) | (nu ? 0x80000000u : 0u);
         h_out->nmerge = cnt - np;
         h_out->pend_off = 0;
         sp.tile_pend[toff + tile] = np;
