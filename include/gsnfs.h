@@ -195,6 +195,48 @@ int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream,
                        const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
                        float* d_attr_out /* N_v x channels */);
 
+/* ---- entropy coder for the quantised coefficients: block-parallel adaptive RLGR ---------------------
+ * PAPER.md:L257 (section 3.4: Run-Length Golomb-Rice [25], run-length coding of zeros, Golomb-Rice coding of non-zero
+ * magnitudes with an adaptive parameter, blocks of successive coefficients coded by one GPU thread each), L803
+ * (Appendix H: each attribute channel partitioned into fixed-size blocks, encoded independently), Table A.5 (block
+ * sizes 256 .. 8192).  The paper gives the coder by citation only; the bit-exact rules are reading [R14]:
+ *   u(x) = 2x (x >= 0), -2x - 1 (x < 0);  GR(u, kR): p = u >> kR, p < 32: p ones, a zero, kR low bits of u; else 32
+ *   ones and u in 32 bits;  state kP, kRP (k = kP >> 2, kR = kRP >> 2), every block starts at kP = 0, kRP = 8;
+ *   k == 0: GR(u(x), kR), then kP += 3 if x == 0 else kP -= 1;  k > 0: 2^k zeros -> bit 0, kP += 2; r < 2^k zeros then
+ *   x != 0 -> bit 1, r in k bits, GR(u(x) - 1, kR), kP -= 3; a block ending inside a run -> bit 0 (a 0 bit means
+ *   min(2^k, coefficients left) zeros);  after a GR: p == 0: kRP -= 2, p > 1: kRP += min(p, 32) + 1;
+ *   0 <= kP <= 64, 0 <= kRP <= 127;  bits MSB first, every block padded to a multiple of 32 bits.
+ * Layout: d_qcoeff is n_rows x channels row-major (canonical order [R8]); block (b, c) = rows [b*B, min((b+1)*B, n))
+ * of column c; d_block_bits[b * channels + c] = its padded bit length (the stream header); d_stream holds the block
+ * streams back to back in that order.  Nothing is transposed: the threads of a CTA are the channels of one row block.
+ * All pointers are caller-owned device memory; d_stream 4-byte aligned.  Asynchronous on `stream`. */
+#define GSNFS_RLGR_MIN_BLOCK 64
+#define GSNFS_RLGR_MAX_BLOCK 65536
+typedef struct gsnfs_rlgr_info {  /* device-resident result of the RLGR calls */
+  uint64_t stream_bytes;          /* total bytes of the block streams                                          */
+  uint32_t n_blocks;              /* entries of d_block_bits                                                   */
+  uint32_t status;                /* 0 = ok; bit 0 = corrupt / inconsistent stream (decode);                   */
+} gsnfs_rlgr_info;                /*         bit 1 = stream_capacity too small (encode: nothing was written)   */
+/* Entries of d_block_bits: ceil(n_rows / block_size) * channels (0 for an invalid block_size). */
+uint64_t gsnfs_rlgr_blocks(uint64_t n_rows, int channels, int block_size);
+/* A stream capacity that always suffices in practice: the raw size 4 * n_rows * channels plus the per-block padding
+ * (an RLGR stream longer than the raw coefficients is reported through status bit 1, never written). */
+uint64_t gsnfs_rlgr_capacity(uint64_t n_rows, int channels, int block_size);
+/* n_rows is the row count; if d_counts != NULL the actual N_v is read on the device and n_rows is an upper bound
+ * (blocks beyond N_v get bit length 0).  Errors: INVALID_ARGUMENT (NULL, block_size outside [64, 65536], misaligned
+ * d_stream), CAPACITY (beyond the context). */
+int gsnfs_rlgr_encode(gsnfs_ctx* ctx, gsnfs_stream stream,
+                      const int32_t* d_qcoeff /* n_rows x channels */, uint64_t n_rows, const gsnfs_counts* d_counts,
+                      int channels, int block_size,
+                      uint32_t* d_block_bits /* gsnfs_rlgr_blocks() entries */,
+                      uint8_t* d_stream, uint64_t stream_capacity, gsnfs_rlgr_info* d_info);
+/* Inverse: block streams -> d_qcoeff (n_rows x channels).  A block that runs out of bits, or a header that does not
+ * fit stream_bytes, sets status bit 0 (the block's remaining coefficients are zero); never reads out of bounds. */
+int gsnfs_rlgr_decode(gsnfs_ctx* ctx, gsnfs_stream stream,
+                      const uint8_t* d_stream, uint64_t stream_bytes, const uint32_t* d_block_bits,
+                      uint64_t n_rows, int channels, int block_size,
+                      int32_t* d_qcoeff /* n_rows x channels */, gsnfs_rlgr_info* d_info);
+
 /* ---- whole-frame calls on HOST buffers (copies inside; used for end-to-end timing) --------------- */
 /* encode = H2D(xyz, attr) -> octree_encode -> voxel_merge -> raht_forward(weights = counts) -> D2H.
  * Host outputs: h_occ[occ_capacity], h_level_sizes[depth+1], h_weights[n] (first N_v valid),

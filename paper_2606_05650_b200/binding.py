@@ -64,6 +64,12 @@ _SIGNATURES = {
                                    c_void_p, c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p]),
     "gsnfs_quantize": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, POINTER(c_float),
                                POINTER(GsnfsQuant), c_void_p]),
+    "gsnfs_rlgr_blocks": (c_uint64, [c_uint64, c_int, c_int]),
+    "gsnfs_rlgr_capacity": (c_uint64, [c_uint64, c_int, c_int]),
+    "gsnfs_rlgr_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_int, c_void_p, c_void_p,
+                                  c_uint64, c_void_p]),
+    "gsnfs_rlgr_decode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_uint64, c_int, c_int, c_void_p,
+                                  c_void_p]),
     "gsnfs_frame_encode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_int, POINTER(c_float),
                                         POINTER(c_float), c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p,
                                         c_uint64, c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -279,6 +285,39 @@ def gsnfs_raht_inverse(ctx: Context, d_voxel_keys, d_weights, n_voxels, d_counts
         int(depth), _dptr(d_qcoeff, torch.int32, "d_qcoeff"), _dptr(d_coeff, torch.float32, "d_coeff"),
         int(channels), _farr(qstep, channels), _quant(quant), _dptr(d_attr_out, torch.float32, "d_attr_out"))
     ctx._check(rc, "gsnfs_raht_inverse")
+
+
+def gsnfs_rlgr_blocks(n_rows: int, channels: int, block_size: int) -> int:
+    return int(lib().gsnfs_rlgr_blocks(int(n_rows), int(channels), int(block_size)))
+
+
+def gsnfs_rlgr_capacity(n_rows: int, channels: int, block_size: int) -> int:
+    return int(lib().gsnfs_rlgr_capacity(int(n_rows), int(channels), int(block_size)))
+
+
+def rlgr_info(d_info):
+    """Host view of a device gsnfs_rlgr_info (an int64[2] tensor): (stream_bytes, n_blocks, status); synchronises."""
+    v = d_info.cpu().numpy().view(np.uint64)
+    return int(v[0]), int(v[1] & np.uint64(0xffffffff)), int(v[1] >> np.uint64(32))
+
+
+def gsnfs_rlgr_encode(ctx: Context, d_qcoeff, n_rows, d_counts, channels, block_size, d_block_bits, d_stream, d_info,
+                      stream=None):
+    rc = lib().gsnfs_rlgr_encode(
+        ctx.handle, _stream(stream), _dptr(d_qcoeff, torch.int32, "d_qcoeff"), int(n_rows),
+        _dptr(d_counts, torch.int32, "d_counts"), int(channels), int(block_size),
+        _dptr(d_block_bits, torch.int32, "d_block_bits"), _dptr(d_stream, torch.uint8, "d_stream"), int(d_stream.numel()),
+        _dptr(d_info, torch.int64, "d_info"))
+    ctx._check(rc, "gsnfs_rlgr_encode")
+
+
+def gsnfs_rlgr_decode(ctx: Context, d_stream, stream_bytes, d_block_bits, n_rows, channels, block_size, d_qcoeff, d_info,
+                      stream=None):
+    rc = lib().gsnfs_rlgr_decode(
+        ctx.handle, _stream(stream), _dptr(d_stream, torch.uint8, "d_stream"), int(stream_bytes),
+        _dptr(d_block_bits, torch.int32, "d_block_bits"), int(n_rows), int(channels), int(block_size),
+        _dptr(d_qcoeff, torch.int32, "d_qcoeff"), _dptr(d_info, torch.int64, "d_info"))
+    ctx._check(rc, "gsnfs_rlgr_decode")
 
 
 def gsnfs_frame_encode_host(ctx: Context, h_xyz, h_attr, n, channels, bbox_min, bbox_max, depth, qstep, quant,

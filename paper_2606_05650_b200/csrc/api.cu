@@ -128,6 +128,8 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
   const size_t o_rplan = b.take(sizeof(RahtPlan));
   const size_t o_rrows = b.take(c->raht_pool_rows * (size_t)C * 4);
+  c->rlgr_off_cap = (N / GSNFS_RLGR_MIN_BLOCK + 1) * (uint64_t)C + 1;
+  const size_t o_rlo = b.take(c->rlgr_off_cap * 8);
   const size_t o_dpar = b.take((c->occ_cap + N + 2) * 4), o_dkm = b.take((N + 1) * 8);
   c->pool_bytes = b.off;
   GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->pool, c->pool_bytes));
@@ -143,6 +145,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
   c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);
+  c->rlgr_off = (uint64_t*)(p + o_rlo);
   GSNFS_CUDA_OK(c, cudaMemset(c->pool, 0, o_rrows));     // everything but the big row pool ...
   GSNFS_CUDA_OK(c, cudaMemset(p + o_dpar, 0, c->pool_bytes - o_dpar));   // ... and the decoder's parent / middle-level arrays
   int rc = octree_encode_setup(c);
@@ -359,6 +362,43 @@ int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_vo
   GSNFS_ON_DEVICE(ctx);
   return raht_done(ctx, run_raht(ctx, (cudaStream_t)stream, true, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth,
                                  d_coeff, d_qcoeff, channels, d_qcoeff ? qstep : nullptr, quant, nullptr, d_attr_out));
+}
+
+// ---- RLGR entropy coder for the quantised coefficients ----------------------------------------------
+uint64_t gsnfs_rlgr_blocks(uint64_t n_rows, int channels, int block_size) {
+  if (block_size < GSNFS_RLGR_MIN_BLOCK || block_size > GSNFS_RLGR_MAX_BLOCK || channels < 1) return 0;
+  return ((n_rows + (uint64_t)block_size - 1) / (uint64_t)block_size) * (uint64_t)channels;
+}
+
+uint64_t gsnfs_rlgr_capacity(uint64_t n_rows, int channels, int block_size) {
+  const uint64_t nb = gsnfs_rlgr_blocks(n_rows, channels, block_size);
+  return nb ? n_rows * (uint64_t)channels * 4ull + nb * 4ull : 0;
+}
+
+int gsnfs_rlgr_encode(gsnfs_ctx* ctx, gsnfs_stream stream, const int32_t* d_qcoeff, uint64_t n_rows,
+                      const gsnfs_counts* d_counts, int channels, int block_size, uint32_t* d_block_bits,
+                      uint8_t* d_stream, uint64_t stream_capacity, gsnfs_rlgr_info* d_info) {
+  if (!ctx || !d_info || (n_rows && (!d_qcoeff || !d_block_bits || !d_stream))) return GSNFS_E_INVALID_ARGUMENT;
+  if (channels < 1 || channels > GSNFS_MAX_CHANNELS || n_rows >= (1ull << 30) || block_size < GSNFS_RLGR_MIN_BLOCK ||
+      block_size > GSNFS_RLGR_MAX_BLOCK || ((uintptr_t)d_stream & 3))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (n_rows > ctx->max_points || channels > ctx->max_channels) return GSNFS_E_CAPACITY;
+  GSNFS_ON_DEVICE(ctx);
+  return run_rlgr_encode(ctx, (cudaStream_t)stream, d_qcoeff, (uint32_t)n_rows, d_counts, channels, (uint32_t)block_size,
+                         d_block_bits, d_stream, stream_capacity, d_info);
+}
+
+int gsnfs_rlgr_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_stream, uint64_t stream_bytes,
+                      const uint32_t* d_block_bits, uint64_t n_rows, int channels, int block_size, int32_t* d_qcoeff,
+                      gsnfs_rlgr_info* d_info) {
+  if (!ctx || !d_info || (n_rows && (!d_qcoeff || !d_block_bits || (!d_stream && stream_bytes)))) return GSNFS_E_INVALID_ARGUMENT;
+  if (channels < 1 || channels > GSNFS_MAX_CHANNELS || n_rows >= (1ull << 30) || block_size < GSNFS_RLGR_MIN_BLOCK ||
+      block_size > GSNFS_RLGR_MAX_BLOCK || ((uintptr_t)d_stream & 3))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (n_rows > ctx->max_points || channels > ctx->max_channels) return GSNFS_E_CAPACITY;
+  GSNFS_ON_DEVICE(ctx);
+  return run_rlgr_decode(ctx, (cudaStream_t)stream, d_stream, stream_bytes, d_block_bits, (uint32_t)n_rows, channels,
+                         (uint32_t)block_size, d_qcoeff, d_info);
 }
 
 // ---- whole-frame calls on host buffers -----------------------------------------------------------

@@ -113,6 +113,10 @@ struct gsnfs_ctx {
   int occ_cache[16];       // cached cudaOccupancyMaxActiveBlocksPerMultiprocessor results (0 = not yet queried)
   size_t occ_cache_smem[16];
 
+  // RLGR: byte offset of every block stream (exclusive scan of the block sizes)
+  uint64_t* rlgr_off;
+  uint64_t rlgr_off_cap;
+
   // decode
   uint64_t* dec_kmid;      // Morton codes of the decoder's middle level (max_points + 1 entries)
   uint32_t* dec_parent;    // (parent stream index << 3 | child digit) of every breadth-first node: occ_cap + max_points + 2
@@ -244,6 +248,12 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
              uint32_t* d_weights_out = nullptr);
 int run_quantize(gsnfs_ctx* ctx, cudaStream_t st, const float* d_coeff, uint32_t n, const gsnfs_counts* d_counts,
                  int channels, const float* qstep, const gsnfs_quant* quant, int32_t* d_qcoeff);
+int run_rlgr_encode(gsnfs_ctx* ctx, cudaStream_t st, const int32_t* d_q, uint32_t n, const gsnfs_counts* d_counts,
+                    int channels, uint32_t block, uint32_t* d_block_bits, uint8_t* d_stream, uint64_t capacity,
+                    gsnfs_rlgr_info* d_info);
+int run_rlgr_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_stream, uint64_t stream_bytes,
+                    const uint32_t* d_block_bits, uint32_t n, int channels, uint32_t block, int32_t* d_q,
+                    gsnfs_rlgr_info* d_info);
 int raht_setup(gsnfs_ctx* ctx);   // occupancy queries + attributes, called from gsnfs_create
 
 }  // namespace gsnfs

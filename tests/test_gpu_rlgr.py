@@ -1,0 +1,153 @@
+"""GPU parity for the block-parallel RLGR coder (Table A.5): the CUDA path
+through the C ABI against oracle/rlgr_oracle.c -- integer work, so block sizes and stream bytes are compared bit for bit."""
+import numpy as np
+import pytest
+import torch
+
+from oracle import gsnfs_oracle as orc
+from oracle import rlgr as orl
+from paper_2606_05650_b200 import synth
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2606_05650_b200 import binding
+    binding.lib()
+    return binding
+
+
+@pytest.fixture(scope="module")
+def ctx(B):
+    c = B.Context(max_points=1_000_000, max_channels=64, max_depth=16)
+    yield c
+    c.close()
+
+
+def gpu_encode(B, ctx, q, block, capacity=None, counts=None, n_rows=None):
+    n, C = q.shape
+    n_rows = n if n_rows is None else n_rows
+    d_q = torch.from_numpy(np.ascontiguousarray(q, dtype=np.int32)).to(DEV)
+    nb = B.gsnfs_rlgr_blocks(n_rows, C, block)
+    cap = B.gsnfs_rlgr_capacity(n_rows, C, block) if capacity is None else capacity
+    bits = torch.full((max(nb, 1),), -1, dtype=torch.int32, device=DEV)
+    stream = torch.zeros(max(cap, 4), dtype=torch.uint8, device=DEV)
+    info = torch.zeros(2, dtype=torch.int64, device=DEV)
+    B.gsnfs_rlgr_encode(ctx, d_q if n else torch.zeros((1, C), dtype=torch.int32, device=DEV), n_rows, counts, C, block, bits,
+                        stream, info)
+    torch.cuda.synchronize()
+    nbytes, nblocks, status = B.rlgr_info(info)
+    return bits[:nb].cpu().numpy().view(np.uint32), stream, nbytes, nblocks, status, d_q
+
+
+def gpu_decode(B, ctx, stream, nbytes, bits, n, C, block):
+    d_bits = torch.from_numpy(np.ascontiguousarray(bits).view(np.int32)).to(DEV)
+    out = torch.full((max(n, 1), C), 77, dtype=torch.int32, device=DEV)
+    info = torch.zeros(2, dtype=torch.int64, device=DEV)
+    B.gsnfs_rlgr_decode(ctx, stream, nbytes, d_bits, n, C, block, out, info)
+    torch.cuda.synchronize()
+    return out[:n].cpu().numpy(), B.rlgr_info(info)
+
+
+def check_case(B, ctx, q, block, capacity=None):
+    n, C = q.shape
+    ref_bits, ref_stream = orl.encode(q, block)
+    bits, stream, nbytes, nblocks, status, _ = gpu_encode(B, ctx, q, block, capacity)
+    assert status == 0 and nblocks == ref_bits.size and nbytes == ref_stream.size
+    assert np.array_equal(bits, ref_bits)
+    assert np.array_equal(stream[:nbytes].cpu().numpy(), ref_stream)
+    back, (_, _, st) = gpu_decode(B, ctx, stream, nbytes, bits, n, C, block)
+    assert st == 0 and np.array_equal(back, q)
+    return nbytes
+
+
+@pytest.mark.parametrize("kind,n,C,block", [
+    ("laplace", 5000, 56, 512), ("laplace", 4097, 56, 4096), ("sparse", 20000, 56, 2048), ("zeros", 3000, 8, 256),
+    ("huge", 1500, 12, 256), ("dense", 777, 3, 8192), ("mixed", 1, 1, 64), ("mixed", 65, 7, 64), ("mixed", 33000, 35, 1024),
+    ("laplace", 2000, 208, 512)])
+def test_streams_bit_exact(B, kind, n, C, block):
+    ctx = B.Context(max_points=max(n, 64), max_channels=max(C, 4), max_depth=8)
+    try:
+        rng = np.random.default_rng(n * 7 + C)
+        q = {
+            "laplace": lambda: np.rint(rng.laplace(0, 40, (n, C))),
+            "sparse": lambda: (rng.random((n, C)) < 0.03) * rng.integers(-6, 7, (n, C)),
+            "zeros": lambda: np.zeros((n, C)),
+            "huge": lambda: rng.integers(-2**31, 2**31, (n, C)),
+            "dense": lambda: rng.integers(-300, 301, (n, C)),
+            "mixed": lambda: np.rint(rng.laplace(0, 3, (n, C))) * (rng.random((n, C)) < 0.5),
+        }[kind]().astype(np.int32)
+        # incompressible input expands (escape codes): the recommended capacity is the raw size, so give it room
+        check_case(B, ctx, q, block, capacity=12 * n * C + 64 if kind == "huge" else None)
+    finally:
+        ctx.close()
+
+
+def test_real_coefficients_all_table_a5_block_sizes(B, ctx):
+    """Quantised RAHT coefficients of config 2 through every block size of Table A.5; the size ordering of the table
+    (smaller blocks cost a little more) holds for the GPU streams too."""
+    fr = synth.make_frame(2)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    q = ref["qcoeff"].astype(np.int32)
+    sizes = {}
+    for block in (256, 512, 1024, 2048, 4096, 8192):
+        sizes[block] = check_case(B, ctx, q, block)
+    assert sizes[256] >= sizes[512] >= sizes[2048] >= sizes[8192]
+    assert sizes[512] <= 1.05 * sizes[8192]
+
+
+def test_config3_full_size_sampled_blocks_and_roundtrip(B, ctx):
+    """BASELINE.json configs[2] at full size in bench.py's launch configuration (block 2048): header compared in full
+    with the oracle, decode(encode(q)) = q on the device, 200 sampled block streams compared byte for byte."""
+    rng = np.random.default_rng(11)
+    n, C, block = 1_000_000, 56, 2048
+    scale = np.concatenate([np.full(3, 60.0), np.full(4, 40.0), [30.0], np.full(3, 25.0), np.full(45, 6.0)])
+    q = np.rint(rng.laplace(0, 1, (n, C)) * scale[None, :]).astype(np.int32)
+    bits, stream, nbytes, nblocks, status, d_q = gpu_encode(B, ctx, q, block)
+    assert status == 0
+    ref_bits = np.zeros(nblocks, np.uint32)
+    orl._L().rlgr_oracle_encode(q.ctypes.data, n, C, block, ref_bits.ctypes.data, None)
+    assert np.array_equal(bits, ref_bits) and nbytes == int(ref_bits.astype(np.int64).sum()) // 8
+    off = np.concatenate([[0], np.cumsum(ref_bits.astype(np.int64) // 8)])
+    host = stream[:nbytes].cpu().numpy()
+    for e in rng.integers(0, nblocks, 200).tolist():
+        b, c = divmod(e, C)
+        s, bl = orl.encode_block(q[b * block:(b + 1) * block, c])
+        assert host[off[e]:off[e + 1]].tobytes() == s
+    d_bits = torch.from_numpy(bits.view(np.int32)).to(DEV)
+    out = torch.empty((n, C), dtype=torch.int32, device=DEV)
+    info = torch.zeros(2, dtype=torch.int64, device=DEV)
+    B.gsnfs_rlgr_decode(ctx, stream, nbytes, d_bits, n, C, block, out, info)
+    torch.cuda.synchronize()
+    assert B.rlgr_info(info)[2] == 0 and torch.equal(out, d_q)
+
+
+def test_device_counts_chain_capacity_and_corruption(B, ctx):
+    rng = np.random.default_rng(3)
+    n, C, block = 10_000, 56, 512
+    q = np.rint(rng.laplace(0, 20, (n, C))).astype(np.int32)
+    # N_v read on the device: rows beyond it are not coded, their blocks have length 0
+    counts = torch.tensor([7_000, 0, 0, 0], dtype=torch.int32, device=DEV)
+    bits, stream, nbytes, nblocks, status, _ = gpu_encode(B, ctx, q, block, counts=counts)
+    ref_bits, ref_stream = orl.encode(q[:7000], block)
+    assert status == 0 and nbytes == ref_stream.size
+    assert np.array_equal(bits[:ref_bits.size], ref_bits) and np.all(bits[ref_bits.size:] == 0)
+    assert np.array_equal(stream[:nbytes].cpu().numpy(), ref_stream)
+    # a stream buffer that is too small: reported, nothing written
+    bits, stream, nbytes, nblocks, status, _ = gpu_encode(B, ctx, q, block, capacity=4096)
+    assert status & 2 and nbytes > 4096 and bool((stream == 0).all())
+    # corrupt / truncated streams are flagged, the call stays in bounds
+    bits, stream, nbytes, nblocks, status, _ = gpu_encode(B, ctx, q, block)
+    back, (_, _, st) = gpu_decode(B, ctx, stream, nbytes // 2, bits, n, C, block)
+    assert st & 1
+    bad_bits = bits.copy()
+    bad_bits[5] -= 32                                     # a block shorter than what its coefficients need
+    back, (_, _, st) = gpu_decode(B, ctx, stream, nbytes, bad_bits, n, C, block)
+    assert st & 1
+    back, (_, _, st) = gpu_decode(B, ctx, stream, nbytes, bits, n, C, block)
+    assert st == 0 and np.array_equal(back, q)
+    for bad_block in (32, 100_000):
+        with pytest.raises(B.GsnfsError):
+            gpu_encode(B, ctx, q, bad_block, capacity=1 << 20)
