@@ -3,10 +3,13 @@
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--config 3] [--impl ours|reference]
 
-A "step" is one pass of the whole hot path over one frame: gsnfs_octree_encode -> gsnfs_voxel_merge ->
-gsnfs_raht_forward (encode), the decoder's header read-back, then gsnfs_octree_decode ->
-gsnfs_raht_inverse (decode).  `value` is whole-job Mgaussians/s with inputs resident in HBM; `e2e` is the
-same metric through the *_host ABI calls with pinned host buffers (H2D/D2H inside the timed region).
+A "step" is one pass of the whole hot path over one frame: gsnfs_octree_encode -> gsnfs_merge_raht_forward (duplicate
+merge fused into the forward transform + quantiser) on the encoder side, the decoder's header read-back, then
+gsnfs_octree_decode -> gsnfs_raht_inverse.  `value` is whole-job Mgaussians/s with inputs resident in HBM; `e2e` is the
+same metric through the *_host_packed ABI calls with pinned host buffers (H2D/D2H inside the timed region; the
+coefficients cross PCIe as RLGR bytes), `e2e_raw` through the *_host calls (raw int32 coefficients).  `entropy` times
+the RLGR coder on the frame's quantised coefficients, outside the step.  `--config pc` is the
+point-cloud shaped workload (NEXT-4: 1M points, depth 10, 3 colour channels).
 Multi-GPU: frames are independent (intra-only codec) => replicas only, one frame stream per
 rank, no collective on the data path ("scaling": "weak").  `--impl reference` times the fp64 oracle on the
 host cores (a deliberately slow baseline, not the target).  At N = 1 the line also carries `ladder`: the 300-frame
@@ -90,6 +93,21 @@ class ClockSampler:
                 "reasons": sorted(reasons), "samples": len(sm)}
 
 
+def load_frame(synth, args):
+    if args.config == "pc":
+        return synth.make_pointcloud_frame()
+    return synth.make_frame(int(args.config), n_override=args.n_override)
+
+
+def workload_name(args, fr):
+    if args.config == "pc":
+        return (f"point-cloud mode (PAPER.md L434-436 shape; SURVEY 8(f) NEXT-4): N={fr.n} points, C={fr.channels} colour "
+                f"channels, octree depth {fr.depth}, qstep 0.1, synth.make_pointcloud_frame()")
+    return (f"BASELINE.json configs[{int(args.config) - 1}]{' recipe with N overridden' if args.n_override else ''}: N={fr.n} "
+            f"Gaussians, C={fr.channels} fp32 channels, octree depth {fr.depth}, qstep=range/{fr.qdiv}, seed per "
+            f"synth.make_frame({args.config})")
+
+
 # ------------------------------------------------------------------------------------------------
 def algorithmic_bytes(n, nv, s_occ, channels, depth):
     """SURVEY.md section 8(d) / DESIGN.md 'Algorithmic bytes': what each kernel must move, per launch."""
@@ -102,9 +120,10 @@ def algorithmic_bytes(n, nv, s_occ, channels, depth):
         "octree_count": k * n,
         "octree_emit": k * n + 12 * nv + s_occ,
         "merge": 4 * n + 8 * nv + c4 * n + c4 * nv + 4 * nv,
-        "raht_schedule": 12 * nv + 16 * nv + 8 * nv,
-        "raht_forward": c4 * nv + c4 * nv + 16 * nv + 8 * nv,   # fused merge: gathers the N input rows itself
-        "raht_inverse": c4 * nv + c4 * nv + 16 * nv,
+        "raht_schedule": (k + 4) * nv + 16 * nv,                # codes + weights in, <= 16 B/voxel of schedule out
+        "raht_forward": 4 * n + c4 * n + c4 * nv,               # fused merge + forward: perm + the N input rows in, N_v rows out
+        "raht_inverse": c4 * nv + c4 * nv,                      # 4C*N_v read + 4C*N_v write
+        "rlgr_count": c4 * nv, "rlgr_write": c4 * nv, "rlgr_decode": c4 * nv,
         "scan_reduce": None, "scan_sums": None, "scan_down": None,   # used twice with different inputs
         "octree_decode": s_occ + 20 * nv,                       # stream in, leaf codes + coordinates out
         "quantize": 8 * channels * nv,
@@ -189,7 +208,7 @@ def run_ours(args, rank, world, local_rank):
 
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
-    fr = synth.make_frame(args.config, n_override=args.n_override)
+    fr = load_frame(synth, args)
     n, C, J = fr.n, fr.channels, fr.depth
     ctx = B.Context(max_points=n, max_channels=C, max_depth=J, device=local_rank)
     buf = B.FrameBuffers(n, C, J, dev)
@@ -269,12 +288,12 @@ def run_ours(args, rank, world, local_rank):
                          "alg_GBps": round(b / (avg_us * 1e-6) / 1e9, 1) if b else None}
     dom = max((k for k in kernels if ab.get(k)), key=lambda k: kernels[k]["ms_per_step"])
     traffic = None
-    tpath = os.path.join(ROOT, "profiles", "r1_dram_traffic.csv")       # ncu dram bytes per launch (profiles/r1_dram_traffic.md)
+    tpath = os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")       # ncu dram bytes per launch (profiles/r2_dram_traffic.md)
     if os.path.exists(tpath):
         try:
             for line in open(tpath).read().splitlines()[1:]:
                 cfg, kname, nbytes = line.split(",")
-                if cfg == f"config{args.config}" and kname == dom and args.n_override is None:
+                if cfg == f"config{args.config}" and kname == dom and args.n_override is None:     # same workload only
                     traffic = int(nbytes)
         except Exception:
             traffic = None
@@ -285,7 +304,8 @@ def run_ours(args, rank, world, local_rank):
     sort_frac = (ab["_sort_total"] / (sort_ms * 1e-3) / 1e9 / peak) if sort_ms else None
 
     # ---- end to end through the host-buffer ABI calls (pinned host memory, copies inside the timed region)
-    e2e = None
+    RLGR_BLOCK = 2048                      # PAPER.md L257 "blocks (e.g., 2K or 4K successive coefficients)"
+    e2e = e2e_raw = entropy = None
     if rank == 0 or world > 1:
         cap = B.gsnfs_occ_capacity(n, J)
         pin = lambda *s, dt: torch.empty(s, dtype=dt).pin_memory()
@@ -293,36 +313,82 @@ def run_ours(args, rank, world, local_rank):
         h_occ, h_lev = pin(cap, dt=torch.uint8), pin(J + 1, dt=torch.int32)
         h_w, h_q, h_cnt = pin(n, dt=torch.int32), pin(n, C, dt=torch.int32), pin(4, dt=torch.int32)
         h_vx, h_out, h_cnt2 = pin(n, 3, dt=torch.int32), pin(n, C, dt=torch.float32), pin(4, dt=torch.int32)
+        h_bits = pin(B.gsnfs_rlgr_blocks(n, C, RLGR_BLOCK), dt=torch.int32)
+        h_stream, h_info = pin(n * C * 4, dt=torch.uint8), pin(2, dt=torch.int64)
 
-        def e2e_step():
+        def raw_step():
             B.gsnfs_frame_encode_host(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None,
                                       h_occ, h_lev, h_w, h_q, h_cnt)
             B.gsnfs_frame_decode_host(ctx, h_occ, int(h_cnt[1]), h_lev.numpy(), J, h_w, h_q, C, fr.qstep, None,
                                       h_vx, h_out, h_cnt2)
 
-        for _ in range(2):
-            e2e_step()
-        barrier()
-        ks = max(2, min(args.steps, 10))
-        e0.record(stream)
-        for _ in range(ks):
-            e2e_step()
-        e1.record(stream)
-        barrier()
-        ms_e = e0.elapsed_time(e1)
-        ms_e = gdist.max_over_ranks(ms_e, dev) / ks
-        nv_e = int(h_cnt[0])
-        h2d = n * 12 + n * C * 4 + int(h_cnt[1]) + nv_e * 4 + nv_e * C * 4
-        d2h = 16 + 4 * (J + 1) + int(h_cnt[1]) + nv_e * 4 + nv_e * C * 4 + 16 + nv_e * 12 + nv_e * C * 4
-        e2e = {"value": round(world * n / (ms_e * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_e, 4),
-               "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h, "steps": ks}
+        def packed_step():
+            B.gsnfs_frame_encode_host_packed(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None,
+                                             RLGR_BLOCK, h_occ, h_lev, h_w, h_bits, h_stream, h_cnt, h_info)
+            B.gsnfs_frame_decode_host_packed(ctx, h_occ, int(h_cnt[1]), h_lev.numpy(), J, h_w, h_bits, h_stream,
+                                             int(h_info[0]), RLGR_BLOCK, C, fr.qstep, None, h_vx, h_out, h_cnt2)
+
+        def time_e2e(fn):
+            for _ in range(2):
+                fn()
+            barrier()
+            ks = max(2, min(args.steps, 10))
+            e0.record(stream)
+            for _ in range(ks):
+                fn()
+            e1.record(stream)
+            barrier()
+            return gdist.max_over_ranks(e0.elapsed_time(e1), dev) / ks, ks
+
+        ms_p, ks = time_e2e(packed_step)
+        nv_e, ob_e, sb = int(h_cnt[0]), int(h_cnt[1]), int(h_info[0])
+        nbits4 = 4 * B.gsnfs_rlgr_blocks(n, C, RLGR_BLOCK)
+        side = ob_e + nv_e * 4 + nbits4 + sb                      # occupancy bytes, weights, block header, block streams
+        e2e = {"value": round(world * n / (ms_p * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_p, 4),
+               "h2d_bytes_per_step": n * 12 + n * C * 4 + side,
+               "d2h_bytes_per_step": 16 + 4 * (J + 1) + 16 + side + 16 + 16 + nv_e * 12 + nv_e * C * 4, "steps": ks,
+               "api": "gsnfs_frame_encode_host_packed + gsnfs_frame_decode_host_packed (coefficients as RLGR bytes, "
+                      f"block {RLGR_BLOCK})", "coefficient_stream_bytes": sb}
+        ms_r, ks = time_e2e(raw_step)
+        e2e_raw = {"value": round(world * n / (ms_r * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_r, 4),
+                   "h2d_bytes_per_step": n * 12 + n * C * 4 + ob_e + nv_e * 4 + nv_e * C * 4,
+                   "d2h_bytes_per_step": 16 + 4 * (J + 1) + ob_e + nv_e * 4 + nv_e * C * 4 + 16 + nv_e * 12 + nv_e * C * 4,
+                   "steps": ks, "api": "gsnfs_frame_encode_host + gsnfs_frame_decode_host (raw int32 coefficients)"}
+
+    # ---- entropy coder, on the device, on this frame's quantised coefficients
+    if rank == 0 and world == 1:
+        B.encode_frame(ctx, buf, d_xyz, d_attr, fr.bbox_min, fr.bbox_max, fr.qstep)
+        d_bits = torch.empty(B.gsnfs_rlgr_blocks(n, C, RLGR_BLOCK), dtype=torch.int32, device=dev)
+        d_stream = torch.empty(n * C * 4, dtype=torch.uint8, device=dev)
+        d_info = torch.zeros(2, dtype=torch.int64, device=dev)
+        d_back = torch.empty((n, C), dtype=torch.int32, device=dev)
+        ev3 = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+        enc_t, dec_t = [], []
+        for it in range(8):
+            ev3[0].record(stream)
+            B.gsnfs_rlgr_encode(ctx, buf.qcoeff, n, buf.counts, C, RLGR_BLOCK, d_bits, d_stream, d_info)
+            ev3[1].record(stream)
+            torch.cuda.synchronize()
+            sbytes, _, st = B.rlgr_info(d_info)
+            B.gsnfs_rlgr_decode(ctx, d_stream, sbytes, d_bits, nv, C, RLGR_BLOCK, d_back, d_info)
+            ev3[2].record(stream)
+            torch.cuda.synchronize()
+            if it >= 3:
+                enc_t.append(ev3[0].elapsed_time(ev3[1]))
+                dec_t.append(ev3[1].elapsed_time(ev3[2]))
+        ok = bool(torch.equal(d_back[:nv], buf.qcoeff[:nv])) and B.rlgr_info(d_info)[2] == 0
+        entropy = {"coder": f"block-parallel RLGR, block {RLGR_BLOCK} (PAPER.md L257, L803)", "encode_ms": round(float(np.median(enc_t)), 4),
+                   "decode_ms": round(float(np.median(dec_t)), 4), "stream_bytes": sbytes, "raw_bytes": nv * C * 4,
+                   "ratio": round(nv * C * 4 / max(sbytes, 1), 3), "roundtrip_exact": ok,
+                   "note": "synthetic attributes are i.i.d. (SURVEY 8(d)): the ratio is not a compression claim"}
 
     ladder = None
-    if rank == 0 and world == 1 and args.ladder_frames > 0 and args.config == 3 and args.n_override is None:
+    if rank == 0 and world == 1 and args.ladder_frames > 0 and args.config == "3" and args.n_override is None:
         ladder = run_ladder(B, synth, torch, ctx, buf, dev, args.ladder_frames)
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = oracle_time(fr, sample_n=min(fr.n, 1_000_000))
+        cpu["all_cores"] = oracle_all_cores(args)
     ctx.close()
     if rank != 0:
         return
@@ -330,13 +396,12 @@ def run_ours(args, rank, world, local_rank):
         "metric": METRIC, "value": round(value, 3), "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": max(args.warmup, 3), "ms_per_step": round(ms_step, 4), "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config - 1}]{' recipe with N overridden' if args.n_override else ''}: N={n} Gaussians, C={C} fp32 channels, "
-                               f"octree depth {J}, qstep=range/{fr.qdiv}, seed per synth.make_frame({args.config})",
+        "config": {"workload": workload_name(args, fr),
                    "n_gaussians": n, "n_voxels": nv, "occ_bytes": s_occ, "channels": C, "depth": J,
                    "replicas": world, "l2_policy": "inputs larger than L2 (236 MB frame vs 126 MB L2); "
                    "intermediates stay wherever the pipeline leaves them"},
         "encode_ms": round(float(np.median(enc_ms)), 4), "decode_ms": round(float(np.median(dec_ms)), 4),
-        "clocks": clocks, "e2e": e2e, "gpu_launches": int(launches),
+        "clocks": clocks, "e2e": e2e, "e2e_raw": e2e_raw, "entropy": entropy, "gpu_launches": int(launches),
         "gpu_launches_per_step": launches / args.steps,
         "roofline": roofline,
         "sort": {"alg_bytes": ab["_sort_total"], "ms_per_step": sort_ms, "passes": ab["_passes"],
@@ -365,15 +430,42 @@ def oracle_time(fr, sample_n=None, steps=1):
                       f"{dt:.2f} s/step", "ms_per_step": round(dt * 1e3, 2)}
 
 
+def _oracle_worker(config):
+    from paper_2606_05650_b200 import synth
+
+    class A:
+        pass
+    a = A()
+    a.config, a.n_override = config, None
+    fr = load_frame(synth, a)
+    t0 = time.perf_counter()
+    oracle_time(fr)
+    return fr.n, time.perf_counter() - t0
+
+
+def oracle_all_cores(args):
+    """The oracle on all host cores: one independent frame per core (frames are the codec's independent unit; the oracle
+    itself is single-threaded numpy and is not tuned for this)."""
+    import multiprocessing as mp
+    cores = len(os.sched_getaffinity(0))
+    workers = max(1, min(cores, 16))
+    t0 = time.perf_counter()
+    with mp.get_context("spawn").Pool(workers) as pool:
+        res = pool.map(_oracle_worker, [args.config] * workers)
+    wall = time.perf_counter() - t0
+    longest = max(r[1] for r in res)
+    n_tot = sum(r[0] for r in res)
+    return {"value": round(n_tot / longest / 1e6, 5), "unit": UNIT, "cores": workers, "kind": "oracle, one frame per core",
+            "sample": f"{workers} whole frames in parallel, slowest {longest:.2f} s (wall incl. process start {wall:.1f} s)"}
+
+
 def run_reference(args, rank, world):
     if rank != 0:
         return
     from paper_2606_05650_b200 import synth
-    fr = synth.make_frame(args.config)
-    total = args.steps + args.warmup
-    # bounded sample: the whole run should end within a few minutes (~15 us per Gaussian per step)
-    budget_s = 150.0
-    sample_n = int(min(fr.n, max(10_000, budget_s / max(total, 1) / 16e-6)))
+    fr = load_frame(synth, args)
+    # the whole frame, every step (config 3: ~7 s per step on one core; the driver allows 30 minutes)
+    sample_n = fr.n
     for _ in range(args.warmup):
         oracle_time(fr, sample_n)
     t0 = time.perf_counter()
@@ -385,8 +477,8 @@ def run_reference(args, rank, world):
     out = {"impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
            "warmup": args.warmup, "ms_per_step": round(dt * 1e3, 3), "higher_is_better": True, "scaling": "weak",
            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-           "config": {"workload": f"BASELINE.json configs[{args.config - 1}] (bounded sample of {sample_n} Gaussians per step)",
-                      "n_gaussians": sample_n, "channels": fr.channels, "depth": fr.depth},
+           "config": {"workload": workload_name(args, fr), "n_gaussians": sample_n, "channels": fr.channels,
+                      "depth": fr.depth},
            "cpu_baseline": cpu,
            "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(out))
@@ -397,7 +489,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=100)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config (1-based); 3 = headline 1M frame")
+    ap.add_argument("--config", default="3", choices=["1", "2", "3", "4", "pc"],
+                    help="BASELINE.json config (1-based); 3 = headline 1M frame; pc = point-cloud shaped frame (NEXT-4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--n-override", type=int, default=None,

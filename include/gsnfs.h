@@ -257,6 +257,27 @@ int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream,
                             const float* qstep, const gsnfs_quant* quant,
                             uint32_t* h_voxel_xyz, float* h_attr, gsnfs_counts* h_counts);
 
+/* The same two frame calls with the quantised coefficients entropy coded on the device (gsnfs_rlgr_encode /
+ * gsnfs_rlgr_decode, block size rlgr_block), so that RLGR bytes instead of raw int32 coefficients cross PCIe
+ * (everything stays GPU-resident until the bitstream).  Host outputs of the encoder: h_occ,
+ * h_level_sizes, h_weights as above; h_block_bits[gsnfs_rlgr_blocks(n, channels, rlgr_block)], h_stream (first
+ * h_info->stream_bytes valid), h_counts, h_info.  The attribute tensor is copied on an internal copy stream while the
+ * position coder runs on `stream`.  GSNFS_E_CAPACITY if stream_capacity (or the context's 4*n*channels staging) is
+ * too small for the stream. */
+int gsnfs_frame_encode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream,
+                                   const float* h_xyz, const float* h_attr, uint64_t n, int channels,
+                                   const float bbox_min[3], const float bbox_max[3], int depth,
+                                   const float* qstep, const gsnfs_quant* quant, int rlgr_block,
+                                   uint8_t* h_occ, uint64_t occ_capacity, uint32_t* h_level_sizes, uint32_t* h_weights,
+                                   uint32_t* h_block_bits, uint8_t* h_stream, uint64_t stream_capacity,
+                                   gsnfs_counts* h_counts, gsnfs_rlgr_info* h_info);
+int gsnfs_frame_decode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream,
+                                   const uint8_t* h_occ, uint64_t occ_bytes, const uint32_t* level_sizes, int depth,
+                                   const uint32_t* h_weights, const uint32_t* h_block_bits, const uint8_t* h_stream,
+                                   uint64_t stream_bytes, int rlgr_block, int channels,
+                                   const float* qstep, const gsnfs_quant* quant,
+                                   uint32_t* h_voxel_xyz, float* h_attr, gsnfs_counts* h_counts);
+
 #ifdef __cplusplus
 }
 #endif

@@ -76,6 +76,13 @@ _SIGNATURES = {
     "gsnfs_frame_decode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, POINTER(c_uint32), c_int, c_void_p,
                                         c_void_p, c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p, c_void_p,
                                         c_void_p]),
+    "gsnfs_frame_encode_host_packed": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_int, POINTER(c_float),
+                                               POINTER(c_float), c_int, POINTER(c_float), POINTER(GsnfsQuant), c_int,
+                                               c_void_p, c_uint64, c_void_p, c_void_p, c_void_p, c_void_p, c_uint64,
+                                               c_void_p, c_void_p]),
+    "gsnfs_frame_decode_host_packed": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, POINTER(c_uint32), c_int, c_void_p,
+                                               c_void_p, c_void_p, c_uint64, c_int, c_int, POINTER(c_float),
+                                               POINTER(GsnfsQuant), c_void_p, c_void_p, c_void_p]),
 }
 
 
@@ -341,6 +348,33 @@ def gsnfs_frame_decode_host(ctx: Context, h_occ, occ_bytes, level_sizes, depth, 
         _farr(qstep, channels), _quant(quant), _hptr(h_voxel_xyz, torch.int32, "h_voxel_xyz"),
         _hptr(h_attr, torch.float32, "h_attr"), _hptr(h_counts, torch.int32, "h_counts"))
     ctx._check(rc, "gsnfs_frame_decode_host")
+
+
+def gsnfs_frame_encode_host_packed(ctx: Context, h_xyz, h_attr, n, channels, bbox_min, bbox_max, depth, qstep, quant,
+                                   rlgr_block, h_occ, h_level_sizes, h_weights, h_block_bits, h_stream, h_counts, h_info,
+                                   stream=None):
+    rc = lib().gsnfs_frame_encode_host_packed(
+        ctx.handle, _stream(stream), _hptr(h_xyz, torch.float32, "h_xyz"), _hptr(h_attr, torch.float32, "h_attr"),
+        int(n), int(channels), _f3(bbox_min), _f3(bbox_max), int(depth), _farr(qstep, channels), _quant(quant),
+        int(rlgr_block), _hptr(h_occ, torch.uint8, "h_occ"), int(h_occ.numel()),
+        _hptr(h_level_sizes, torch.int32, "h_level_sizes"), _hptr(h_weights, torch.int32, "h_weights"),
+        _hptr(h_block_bits, torch.int32, "h_block_bits"), _hptr(h_stream, torch.uint8, "h_stream"), int(h_stream.numel()),
+        _hptr(h_counts, torch.int32, "h_counts"), _hptr(h_info, torch.int64, "h_info"))
+    ctx._check(rc, "gsnfs_frame_encode_host_packed")
+
+
+def gsnfs_frame_decode_host_packed(ctx: Context, h_occ, occ_bytes, level_sizes, depth, h_weights, h_block_bits, h_stream,
+                                   stream_bytes, rlgr_block, channels, qstep, quant, h_voxel_xyz, h_attr, h_counts,
+                                   stream=None):
+    ls = np.ascontiguousarray(np.asarray(level_sizes, dtype=np.uint32).reshape(-1))
+    arr = (c_uint32 * (depth + 1))(*ls.tolist())
+    rc = lib().gsnfs_frame_decode_host_packed(
+        ctx.handle, _stream(stream), _hptr(h_occ, torch.uint8, "h_occ"), int(occ_bytes), arr, int(depth),
+        _hptr(h_weights, torch.int32, "h_weights"), _hptr(h_block_bits, torch.int32, "h_block_bits"),
+        _hptr(h_stream, torch.uint8, "h_stream"), int(stream_bytes), int(rlgr_block), int(channels),
+        _farr(qstep, channels), _quant(quant), _hptr(h_voxel_xyz, torch.int32, "h_voxel_xyz"),
+        _hptr(h_attr, torch.float32, "h_attr"), _hptr(h_counts, torch.int32, "h_counts"))
+    ctx._check(rc, "gsnfs_frame_decode_host_packed")
 
 
 # ----------------------------------------------------------------------------- buffer bundle

@@ -185,7 +185,12 @@ void gsnfs_destroy(gsnfs_ctx* ctx) {
   for (int i = 0; i < ctx->prof_cap; ++i) { cudaEventDestroy(ctx->prof[i].a); cudaEventDestroy(ctx->prof[i].b); }
   free(ctx->prof);
   if (ctx->pool) cudaFree(ctx->pool);
-  if (ctx->fpool) cudaFree(ctx->fpool);
+  if (ctx->fpool) {
+    cudaFree(ctx->fpool);
+    cudaStreamDestroy(ctx->copy_stream);
+    cudaEventDestroy(ctx->ev_a);
+    cudaEventDestroy(ctx->ev_b);
+  }
   free(ctx);
 }
 
@@ -410,6 +415,7 @@ static int frame_pool(gsnfs_ctx* c) {
   const size_t o_xyz = b.take(N * 12), o_attr = b.take(N * C * 4), o_mrg = b.take(N * C * 4), o_q = b.take(N * C * 4);
   const size_t o_occ = b.take(c->occ_cap), o_lev = b.take(256), o_perm = b.take(N * 4), o_vk = b.take(N * 8);
   const size_t o_vs = b.take((N + 1) * 4), o_w = b.take(N * 4), o_vx = b.take(N * 12), o_cnt = b.take(256);
+  const size_t o_bits = b.take(c->rlgr_off_cap * 4), o_info = b.take(256);
   c->fpool_bytes = b.off;
   GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->fpool, c->fpool_bytes));
   char* p = c->fpool;
@@ -417,6 +423,12 @@ static int frame_pool(gsnfs_ctx* c) {
   c->f_q = (int32_t*)(p + o_q); c->f_occ = (uint8_t*)(p + o_occ); c->f_levels = (uint32_t*)(p + o_lev);
   c->f_perm = (uint32_t*)(p + o_perm); c->f_vkeys = (uint64_t*)(p + o_vk); c->f_vstart = (uint32_t*)(p + o_vs);
   c->f_weights = (uint32_t*)(p + o_w); c->f_vxyz = (uint32_t*)(p + o_vx); c->f_counts = (gsnfs_counts*)(p + o_cnt);
+  c->f_bits = (uint32_t*)(p + o_bits); c->f_info = (gsnfs_rlgr_info*)(p + o_info);
+  c->f_stream = (uint8_t*)c->f_merged;                 // the fused encoder never materialises the merged tensor
+  c->f_stream_cap = N * C * 4;
+  GSNFS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
+  GSNFS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_a, cudaEventDisableTiming));
+  GSNFS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_b, cudaEventDisableTiming));
   return GSNFS_OK;
 }
 
@@ -499,6 +511,116 @@ int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* 
     GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_attr, ctx->f_attr, nv * C * 4, cudaMemcpyDeviceToHost, st));
   }
   GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  return take_sticky(ctx);
+}
+
+// ---- the same two frame calls with the coefficients entropy coded (RLGR) before they leave the device ----------
+int gsnfs_frame_encode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
+                                   int channels, const float bbox_min[3], const float bbox_max[3], int depth,
+                                   const float* qstep, const gsnfs_quant* quant, int rlgr_block, uint8_t* h_occ,
+                                   uint64_t occ_capacity, uint32_t* h_level_sizes, uint32_t* h_weights,
+                                   uint32_t* h_block_bits, uint8_t* h_stream, uint64_t stream_capacity,
+                                   gsnfs_counts* h_counts, gsnfs_rlgr_info* h_info) {
+  if (!ctx || !h_occ || !h_level_sizes || !h_counts || !h_info || !qstep ||
+      (n && (!h_xyz || !h_attr || !h_weights || !h_block_bits || !h_stream)))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (n > ctx->max_points || channels > ctx->max_channels || channels < 1) return GSNFS_E_CAPACITY;
+  if (rlgr_block < GSNFS_RLGR_MIN_BLOCK || rlgr_block > GSNFS_RLGR_MAX_BLOCK) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_ON_DEVICE(ctx);
+  int rc = frame_pool(ctx);
+  if (rc != GSNFS_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream, cs = ctx->copy_stream;
+  const uint64_t cap = gsnfs_occ_capacity(n, depth);
+  if (cap == 0 || occ_capacity < cap || cap > ctx->occ_cap) return depth < 1 || depth > GSNFS_MAX_DEPTH ? GSNFS_E_INVALID_ARGUMENT : GSNFS_E_CAPACITY;
+  const size_t C = (size_t)channels;
+  const uint64_t nbits = gsnfs_rlgr_blocks(n, channels, rlgr_block);
+  // positions on the caller's stream, the (19x larger) attribute tensor on the copy stream: the position coder runs
+  // while the attributes are still crossing PCIe
+  GSNFS_CUDA_OK(ctx, cudaEventRecord(ctx->ev_a, st));                     // earlier work on st (previous frame) first
+  GSNFS_CUDA_OK(ctx, cudaStreamWaitEvent(cs, ctx->ev_a, 0));
+  if (n) {
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_xyz, h_xyz, n * 12, cudaMemcpyHostToDevice, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_attr, h_attr, n * C * 4, cudaMemcpyHostToDevice, cs));
+  }
+  GSNFS_CUDA_OK(ctx, cudaEventRecord(ctx->ev_b, cs));
+  rc = gsnfs_octree_encode(ctx, stream, ctx->f_xyz, n, bbox_min, bbox_max, depth, ctx->f_occ, cap, ctx->f_levels,
+                           ctx->f_perm, ctx->f_vkeys, ctx->f_vstart, ctx->f_counts);
+  if (rc != GSNFS_OK) return rc;
+  GSNFS_CUDA_OK(ctx, cudaStreamWaitEvent(st, ctx->ev_b, 0));
+  rc = gsnfs_merge_raht_forward(ctx, stream, ctx->f_vkeys, ctx->f_perm, ctx->f_vstart, n, ctx->f_counts, depth, ctx->f_attr,
+                                channels, qstep, quant, ctx->f_weights, ctx->f_q, nullptr);
+  if (rc != GSNFS_OK) return rc;
+  rc = gsnfs_rlgr_encode(ctx, stream, ctx->f_q, n, ctx->f_counts, channels, rlgr_block, ctx->f_bits, ctx->f_stream,
+                         ctx->f_stream_cap < stream_capacity ? ctx->f_stream_cap : stream_capacity, ctx->f_info);
+  if (rc != GSNFS_OK) return rc;
+  // header first: the sizes of the remaining copies depend on it
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_counts, ctx->f_counts, sizeof(gsnfs_counts), cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_level_sizes, ctx->f_levels, sizeof(uint32_t) * (depth + 1), cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_info, ctx->f_info, sizeof(gsnfs_rlgr_info), cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  const uint64_t nv = h_counts->n_voxels, ob = h_counts->occ_bytes;
+  if (h_info->status) return GSNFS_E_CAPACITY;                            // stream buffer too small: nothing was written
+  if (nv) {
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_occ, ctx->f_occ, ob, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_weights, ctx->f_weights, nv * 4, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_block_bits, ctx->f_bits, nbits * 4, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_stream, ctx->f_stream, h_info->stream_bytes, cudaMemcpyDeviceToHost, st));
+    GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  }
+  return take_sticky(ctx);
+}
+
+int gsnfs_frame_decode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
+                                   const uint32_t* level_sizes, int depth, const uint32_t* h_weights,
+                                   const uint32_t* h_block_bits, const uint8_t* h_stream, uint64_t stream_bytes,
+                                   int rlgr_block, int channels, const float* qstep, const gsnfs_quant* quant,
+                                   uint32_t* h_voxel_xyz, float* h_attr, gsnfs_counts* h_counts) {
+  if (!ctx || !level_sizes || !h_counts || !qstep) return GSNFS_E_INVALID_ARGUMENT;
+  if (depth < 1 || depth > GSNFS_MAX_DEPTH) return GSNFS_E_INVALID_ARGUMENT;
+  if (rlgr_block < GSNFS_RLGR_MIN_BLOCK || rlgr_block > GSNFS_RLGR_MAX_BLOCK) return GSNFS_E_INVALID_ARGUMENT;
+  const uint64_t nv = level_sizes[depth];
+  if (nv && (!h_occ || !h_block_bits || (!h_stream && stream_bytes) || !h_voxel_xyz || !h_attr)) return GSNFS_E_INVALID_ARGUMENT;
+  if (nv > ctx->max_points || channels > ctx->max_channels || channels < 1 || occ_bytes + 1 > ctx->occ_cap)
+    return GSNFS_E_CAPACITY;
+  if (!octree_header_ok(level_sizes, depth, occ_bytes)) {
+    h_counts->n_voxels = 0; h_counts->occ_bytes = (uint32_t)occ_bytes; h_counts->status = 1; h_counts->reserved = 0;
+    return GSNFS_OK;
+  }
+  if (h_weights)
+    for (uint64_t i = 0; i < nv; ++i)
+      if (h_weights[i] == 0) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_ON_DEVICE(ctx);
+  int rc = frame_pool(ctx);
+  if (rc != GSNFS_OK) return rc;
+  if (stream_bytes > ctx->f_stream_cap) return GSNFS_E_CAPACITY;
+  cudaStream_t st = (cudaStream_t)stream, cs = ctx->copy_stream;
+  const size_t C = (size_t)channels;
+  const uint64_t nbits = gsnfs_rlgr_blocks(nv, channels, rlgr_block);
+  GSNFS_CUDA_OK(ctx, cudaEventRecord(ctx->ev_a, st));
+  GSNFS_CUDA_OK(ctx, cudaStreamWaitEvent(cs, ctx->ev_a, 0));
+  if (nv) {
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_occ, h_occ, occ_bytes, cudaMemcpyHostToDevice, st));
+    // the coefficient stream travels on the copy stream while the position decoder runs
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_bits, h_block_bits, nbits * 4, cudaMemcpyHostToDevice, cs));
+    GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_stream, h_stream, stream_bytes, cudaMemcpyHostToDevice, cs));
+    if (h_weights) GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(ctx->f_weights, h_weights, nv * 4, cudaMemcpyHostToDevice, cs));
+  }
+  GSNFS_CUDA_OK(ctx, cudaEventRecord(ctx->ev_b, cs));
+  rc = gsnfs_octree_decode(ctx, stream, ctx->f_occ, occ_bytes, level_sizes, depth, ctx->f_vxyz, ctx->f_vkeys, ctx->f_counts);
+  if (rc != GSNFS_OK) return rc;
+  if (nv) GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_voxel_xyz, ctx->f_vxyz, nv * 12, cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaStreamWaitEvent(st, ctx->ev_b, 0));
+  rc = gsnfs_rlgr_decode(ctx, stream, ctx->f_stream, stream_bytes, ctx->f_bits, nv, channels, rlgr_block, ctx->f_q, ctx->f_info);
+  if (rc != GSNFS_OK) return rc;
+  rc = gsnfs_raht_inverse(ctx, stream, ctx->f_vkeys, h_weights ? ctx->f_weights : nullptr, nv, ctx->f_counts, depth, ctx->f_q,
+                          nullptr, channels, qstep, quant, ctx->f_attr);
+  if (rc != GSNFS_OK) return rc;
+  gsnfs_rlgr_info info;
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_counts, ctx->f_counts, sizeof(gsnfs_counts), cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(&info, ctx->f_info, sizeof(info), cudaMemcpyDeviceToHost, st));
+  if (nv) GSNFS_CUDA_OK(ctx, cudaMemcpyAsync(h_attr, ctx->f_attr, nv * C * 4, cudaMemcpyDeviceToHost, st));
+  GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
+  if (info.status) h_counts->status |= 1u;                                 // a corrupt coefficient stream is a corrupt frame
   return take_sticky(ctx);
 }
 

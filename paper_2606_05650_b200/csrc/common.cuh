@@ -137,6 +137,12 @@ struct gsnfs_ctx {
   uint32_t* f_weights;
   uint32_t* f_vxyz;
   gsnfs_counts* f_counts;
+  uint32_t* f_bits;        // RLGR block header
+  gsnfs_rlgr_info* f_info;
+  uint8_t* f_stream;       // RLGR block streams (aliases f_merged)
+  uint64_t f_stream_cap;
+  cudaStream_t copy_stream;   // the large H2D copies of the *_host_packed calls overlap the position coder
+  cudaEvent_t ev_a, ev_b;
 };
 
 namespace gsnfs {

@@ -751,3 +751,23 @@ def test_beyond_l2_16m_position_exact_and_sampled_coefficients(B):
         assert torch.all(rms <= (2.0 / 3.0) * qsd * (1 + 1e-3) + 1e-7)
     finally:
         ctx.close()
+
+
+def test_pointcloud_mode_full_compare(B, ctx_big):
+    """SURVEY 8(f) NEXT-4, point-cloud half (Table A.4): 1M points, depth 10, three colour channels,
+    qstep 0.1, a fifth of the points merged as duplicates -- the whole path element by element against the oracle."""
+    fr = synth.make_pointcloud_frame()
+    ctx = B.Context(max_points=fr.n, max_channels=4, max_depth=fr.depth)
+    try:
+        frac = full_pipeline_check(B, ctx, fr)
+        # and the fused merge + transform on the same frame
+        ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+        buf, got = gpu_position_encode(B, ctx, fr)
+        nv = got["n_voxels"]
+        assert (ref["weights"] > 1).sum() > 50_000
+        B.gsnfs_merge_raht_forward(ctx, buf.voxel_keys, buf.perm, buf.voxel_start, fr.n, buf.counts, fr.depth, _t(fr.attr),
+                                   fr.channels, fr.qstep, None, buf.weights, buf.qcoeff, None)
+        torch.cuda.synchronize()
+        check_quantised(buf.qcoeff[:nv].cpu().numpy(), ref["qcoeff"])
+    finally:
+        ctx.close()

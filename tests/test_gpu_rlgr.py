@@ -151,3 +151,51 @@ def test_device_counts_chain_capacity_and_corruption(B, ctx):
     for bad_block in (32, 100_000):
         with pytest.raises(B.GsnfsError):
             gpu_encode(B, ctx, q, bad_block, capacity=1 << 20)
+
+
+def test_packed_host_frame_calls(B):
+    """gsnfs_frame_{encode,decode}_host_packed: the end-to-end path with RLGR bytes crossing PCIe instead of raw
+    coefficients; stream and header bit-exact against the oracle chain, decoded attributes as in the raw-coefficient path."""
+    fr = synth.make_frame(2)
+    ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep)
+    n, C, J, blk = fr.n, fr.channels, fr.depth, 2048
+    ctx = B.Context(max_points=n, max_channels=C, max_depth=J)
+    try:
+        pin = lambda *s, dt: torch.empty(s, dtype=dt).pin_memory()
+        h_xyz, h_attr = torch.from_numpy(fr.xyz).pin_memory(), torch.from_numpy(fr.attr).pin_memory()
+        h_occ, h_lev = pin(B.gsnfs_occ_capacity(n, J), dt=torch.uint8), pin(J + 1, dt=torch.int32)
+        h_w, h_cnt, h_info = pin(n, dt=torch.int32), pin(4, dt=torch.int32), pin(2, dt=torch.int64)
+        h_bits = pin(B.gsnfs_rlgr_blocks(n, C, blk), dt=torch.int32)
+        h_stream = pin(B.gsnfs_rlgr_capacity(n, C, blk), dt=torch.uint8)
+        for _ in range(2):      # twice: the second call reuses the staging pool and the copy stream
+            B.gsnfs_frame_encode_host_packed(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None, blk,
+                                             h_occ, h_lev, h_w, h_bits, h_stream, h_cnt, h_info)
+        nv, ob = int(h_cnt[0]), int(h_cnt[1])
+        nbytes = int(h_info.numpy().view(np.uint64)[0])
+        assert nv == len(ref["voxel_keys"]) and np.array_equal(h_occ[:ob].numpy(), ref["occ"])
+        # the GPU's quantised coefficients differ from the oracle's in <= 1e-4 of the entries (+-1), so the stream is
+        # compared with the oracle coder applied to the GPU's own coefficients, which the raw-path call returns
+        h_q = pin(n, C, dt=torch.int32)
+        B.gsnfs_frame_encode_host(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None,
+                                  h_occ, h_lev, h_w, h_q, h_cnt)
+        ref_bits, ref_stream = orl.encode(h_q[:nv].numpy(), blk)
+        assert nbytes == ref_stream.size and np.array_equal(h_stream[:nbytes].numpy(), ref_stream)
+        assert np.array_equal(h_bits[:ref_bits.size].numpy().view(np.uint32), ref_bits)
+        assert nbytes < 0.5 * nv * C * 4                       # and it is worth shipping
+        h_vx, h_out, h_cnt2 = pin(n, 3, dt=torch.int32), pin(n, C, dt=torch.float32), pin(4, dt=torch.int32)
+        B.gsnfs_frame_decode_host_packed(ctx, h_occ, ob, h_lev.numpy(), J, h_w, h_bits, h_stream, nbytes, blk, C, fr.qstep,
+                                         None, h_vx, h_out, h_cnt2)
+        assert int(h_cnt2[2]) == 0
+        h_out2 = pin(n, C, dt=torch.float32)
+        B.gsnfs_frame_decode_host(ctx, h_occ, ob, h_lev.numpy(), J, h_w, h_q, C, fr.qstep, None, h_vx, h_out2, h_cnt2)
+        assert torch.equal(h_out[:nv], h_out2[:nv])             # same coefficients in, same attributes out
+        dk, dc, ok = orc.octree_decode(ref["occ"], ref["level_sizes"], J)
+        assert np.array_equal(h_vx[:nv].numpy().astype(np.uint64), dc)
+        # a damaged coefficient stream is reported as a corrupt frame
+        bad = h_bits.clone().pin_memory()
+        bad[3] -= 64
+        B.gsnfs_frame_decode_host_packed(ctx, h_occ, ob, h_lev.numpy(), J, h_w, bad, h_stream, nbytes, blk, C, fr.qstep,
+                                         None, h_vx, h_out, h_cnt2)
+        assert int(h_cnt2[2]) & 1
+    finally:
+        ctx.close()
