@@ -23,6 +23,9 @@ Pins (tests/test_oracle_*.py, all `-m "not gpu"`):
                            Morton-prefix ranges; DC = sum(w a)/sqrt(W); Parseval; constant signal;
                            dense separable 3-D Haar on a full cube (PAPER.md:L219 fn. 4);
                            duplicates-expanded equivalence [R2]; perfect reconstruction; linearity
+  rgb_to_yuv / klt_*       rows of the matrix (luma weights sum to 1, chroma rows to 0), grey -> zero chroma,
+                           inverse o forward = identity; KLT against an SVD of the centred data (library PCA),
+                           known synthetic covariance, orthonormality, diagonal output covariance, energy
   quantize / dequantize    PARITY UNPINNED by the paper [R10]: it gives only the name "dead-zone
                            quantization" and omits de-quantisation (L259).  Pinned
                            only to self-consistency properties (dead zone, error bound, symmetry) and
@@ -358,6 +361,86 @@ def dequantize(q, qstep, recon_bias=RECON_BIAS_DEFAULT):
     step = np.asarray(qstep, dtype=np.float32).astype(np.float64)[None, :]
     mag = np.abs(q).astype(np.float64) + np.float64(recon_bias) * (q != 0)
     return np.sign(q) * mag * step
+
+
+# =============================================================================================
+# Colour decorrelation before RAHT (section 4; Table A.8): RGB -> YUV on every
+# SH function, then one Karhunen-Loeve transform per YUV channel over the SH AC coefficients.
+# [R15] the paper names neither the YUV matrix nor the channel layout: BT.601 analogue YUV; channel layout of
+# SURVEY 8(d) (scale 3, rotation 4, opacity 1, SH DC 3, SH AC 3 x K colour-major: AC(c, j) = 11 + K c + j).
+# [R16] KLT = eigenvectors of the covariance about the mean (the textbook definition [34]), columns sorted by
+# descending eigenvalue, each eigenvector signed so that its largest-magnitude component is positive;
+# y = (x - mu) E, x = y E^T + mu; mu, E are side information of the frame.
+# =============================================================================================
+YUV_FROM_RGB = np.array([[0.299, 0.587, 0.114],
+                         [-0.14713, -0.28886, 0.436],
+                         [0.615, -0.51499, -0.10001]], dtype=np.float64)
+SH_DC_OFFSET = 8
+
+
+def sh_layout(channels):
+    """(dc[3], ac[3][K]) channel indices; K = (channels - 11) / 3 SH AC coefficients per colour."""
+    if channels < 11 or (channels - 11) % 3:
+        raise ValueError("channels must be 11 + 3K")
+    K = (channels - 11) // 3
+    dc = [SH_DC_OFFSET + c for c in range(3)]
+    ac = [[11 + K * c + j for j in range(K)] for c in range(3)]
+    return dc, ac
+
+
+def _apply_3x3(attr, M):
+    a = np.array(attr, dtype=np.float64, copy=True)
+    dc, ac = sh_layout(a.shape[1])
+    triples = [dc] + [[ac[0][j], ac[1][j], ac[2][j]] for j in range(len(ac[0]))]
+    for t in triples:                       # every SH function: (R, G, B) -> M (R, G, B)^T  (PAPER.md:L265)
+        a[:, t] = a[:, t] @ M.T
+    return a
+
+
+def rgb_to_yuv(attr):
+    return _apply_3x3(attr, YUV_FROM_RGB)
+
+
+def yuv_to_rgb(attr):
+    return _apply_3x3(attr, np.linalg.inv(YUV_FROM_RGB))
+
+
+def klt_fit(attr_yuv):
+    """Three KLTs, one per YUV channel, over the SH AC coefficients.  Returns mu[3, K], lam[3, K]
+    (descending), E[3, K, K] (columns = eigenvectors) and the covariance matrices S[3, K, K]."""
+    a = np.asarray(attr_yuv, dtype=np.float64)
+    _, ac = sh_layout(a.shape[1])
+    K = len(ac[0])
+    mu, lam, E, S = np.zeros((3, K)), np.zeros((3, K)), np.zeros((3, K, K)), np.zeros((3, K, K))
+    for c in range(3):
+        X = a[:, ac[c]]
+        mu[c] = X.mean(axis=0)
+        Xc = X - mu[c]
+        S[c] = Xc.T @ Xc / X.shape[0]
+        w, V = np.linalg.eigh(S[c])
+        order = np.argsort(-w, kind="stable")
+        w, V = w[order], V[:, order]
+        for j in range(K):
+            if V[np.argmax(np.abs(V[:, j])), j] < 0:
+                V[:, j] = -V[:, j]
+        lam[c], E[c] = w, V
+    return mu, lam, E, S
+
+
+def klt_forward(attr_yuv, mu, E):
+    a = np.array(attr_yuv, dtype=np.float64, copy=True)
+    _, ac = sh_layout(a.shape[1])
+    for c in range(3):
+        a[:, ac[c]] = (a[:, ac[c]] - mu[c]) @ E[c]
+    return a
+
+
+def klt_inverse(attr_klt, mu, E):
+    a = np.array(attr_klt, dtype=np.float64, copy=True)
+    _, ac = sh_layout(a.shape[1])
+    for c in range(3):
+        a[:, ac[c]] = a[:, ac[c]] @ E[c].T + mu[c]
+    return a
 
 
 # =============================================================================================
