@@ -195,6 +195,28 @@ int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream,
                        const float* qstep /* host */, const gsnfs_quant* quant /* host, may be NULL */,
                        float* d_attr_out /* N_v x channels */);
 
+/* ---- colour decorrelation in front of RAHT (section 4; Table A.8) ---------------
+ * "It first transforms RGB to YUV for each SH function ... to all SH coefficients (both DC and AC)"; "a decorrelating
+ * transform, Karhunen-Loeve transform, only to the AC coefficients ... three different KLTs, one to each channel in
+ * YUV color space"; "We apply KLT before RAHT".
+ * Readings: [R15] BT.601 analogue YUV (Y = 0.299 R + 0.587 G + 0.114 B, U = -0.14713 R - 0.28886 G + 0.436 B,
+ * V = 0.615 R - 0.51499 G - 0.10001 B; the inverse is the fp64 matrix inverse); channel layout: 8 geometry channels
+ * (scale 3, rotation 4, opacity 1), SH DC (R, G, B) at 8..10, SH AC colour-major: AC(c, j) = 11 + K c + j, K = (channels
+ * - 11) / 3 in {0, .., 15}.  [R16] KLT of YUV channel c: covariance about the mean of its K AC coefficients over the n
+ * rows (fp64 accumulation), eigenvectors by descending eigenvalue, each signed so that its largest-magnitude
+ * component is positive; y = (x - mu) E, x = y E^T + mu.
+ * d_klt (device, gsnfs_klt_floats(channels) floats) is the frame's side information: per YUV channel mean[K],
+ * eigenvalue[K], basis[K][K] (basis[i][j] = component i of eigenvector j).  d_klt == NULL in the transform calls means
+ * YUV only.  d_out may equal d_attr (rows are independent).  n_rows / d_counts as in gsnfs_raht_forward.  The fit is
+ * deterministic (fixed reduction order).  Errors: INVALID_ARGUMENT (channels not 11 + 3K, K <= 15; NULL), CAPACITY. */
+uint64_t gsnfs_klt_floats(int channels);
+int gsnfs_klt_fit(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr /* n_rows x channels, RGB */, uint64_t n_rows,
+                  const gsnfs_counts* d_counts, int channels, float* d_klt);
+int gsnfs_color_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr /* RGB */, uint64_t n_rows,
+                        const gsnfs_counts* d_counts, int channels, const float* d_klt, float* d_out /* YUV + KLT */);
+int gsnfs_color_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr /* YUV + KLT */, uint64_t n_rows,
+                        const gsnfs_counts* d_counts, int channels, const float* d_klt, float* d_out /* RGB */);
+
 /* ---- entropy coder for the quantised coefficients: block-parallel adaptive RLGR ---------------------
  * PAPER.md:L257 (section 3.4: Run-Length Golomb-Rice [25], run-length coding of zeros, Golomb-Rice coding of non-zero
  * magnitudes with an adaptive parameter, blocks of successive coefficients coded by one GPU thread each), L803

@@ -64,6 +64,10 @@ _SIGNATURES = {
                                    c_void_p, c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p]),
     "gsnfs_quantize": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, POINTER(c_float),
                                POINTER(GsnfsQuant), c_void_p]),
+    "gsnfs_klt_floats": (c_uint64, [c_int]),
+    "gsnfs_klt_fit": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p]),
+    "gsnfs_color_forward": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p, c_void_p]),
+    "gsnfs_color_inverse": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_void_p, c_void_p]),
     "gsnfs_rlgr_blocks": (c_uint64, [c_uint64, c_int, c_int]),
     "gsnfs_rlgr_capacity": (c_uint64, [c_uint64, c_int, c_int]),
     "gsnfs_rlgr_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_int, c_int, c_void_p, c_void_p,
@@ -292,6 +296,30 @@ def gsnfs_raht_inverse(ctx: Context, d_voxel_keys, d_weights, n_voxels, d_counts
         int(depth), _dptr(d_qcoeff, torch.int32, "d_qcoeff"), _dptr(d_coeff, torch.float32, "d_coeff"),
         int(channels), _farr(qstep, channels), _quant(quant), _dptr(d_attr_out, torch.float32, "d_attr_out"))
     ctx._check(rc, "gsnfs_raht_inverse")
+
+
+def gsnfs_klt_floats(channels: int) -> int:
+    return int(lib().gsnfs_klt_floats(int(channels)))
+
+
+def gsnfs_klt_fit(ctx: Context, d_attr, n_rows, d_counts, channels, d_klt, stream=None):
+    rc = lib().gsnfs_klt_fit(ctx.handle, _stream(stream), _dptr(d_attr, torch.float32, "d_attr"), int(n_rows),
+                             _dptr(d_counts, torch.int32, "d_counts"), int(channels), _dptr(d_klt, torch.float32, "d_klt"))
+    ctx._check(rc, "gsnfs_klt_fit")
+
+
+def gsnfs_color_forward(ctx: Context, d_attr, n_rows, d_counts, channels, d_klt, d_out, stream=None):
+    rc = lib().gsnfs_color_forward(ctx.handle, _stream(stream), _dptr(d_attr, torch.float32, "d_attr"), int(n_rows),
+                                   _dptr(d_counts, torch.int32, "d_counts"), int(channels),
+                                   _dptr(d_klt, torch.float32, "d_klt"), _dptr(d_out, torch.float32, "d_out"))
+    ctx._check(rc, "gsnfs_color_forward")
+
+
+def gsnfs_color_inverse(ctx: Context, d_attr, n_rows, d_counts, channels, d_klt, d_out, stream=None):
+    rc = lib().gsnfs_color_inverse(ctx.handle, _stream(stream), _dptr(d_attr, torch.float32, "d_attr"), int(n_rows),
+                                   _dptr(d_counts, torch.int32, "d_counts"), int(channels),
+                                   _dptr(d_klt, torch.float32, "d_klt"), _dptr(d_out, torch.float32, "d_out"))
+    ctx._check(rc, "gsnfs_color_inverse")
 
 
 def gsnfs_rlgr_blocks(n_rows: int, channels: int, block_size: int) -> int:

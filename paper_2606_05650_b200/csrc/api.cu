@@ -128,6 +128,8 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
   const size_t o_rplan = b.take(sizeof(RahtPlan));
   const size_t o_rrows = b.take(c->raht_pool_rows * (size_t)C * 4);
+  c->color_parts_cap = (uint32_t)c->num_sms * 2u;
+  const size_t o_colp = b.take((size_t)c->color_parts_cap * 3 * 135 * sizeof(double));
   c->rlgr_off_cap = (N / GSNFS_RLGR_MIN_BLOCK + 1) * (uint64_t)C + 1;
   const size_t o_rlo = b.take(c->rlgr_off_cap * 8);
   const size_t o_dpar = b.take((c->occ_cap + N + 2) * 4), o_dkm = b.take((N + 1) * 8);
@@ -146,9 +148,12 @@ static int create_impl(gsnfs_ctx* c) {
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
   c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);
   c->rlgr_off = (uint64_t*)(p + o_rlo);
+  c->color_partial = (double*)(p + o_colp);
   GSNFS_CUDA_OK(c, cudaMemset(c->pool, 0, o_rrows));     // everything but the big row pool ...
   GSNFS_CUDA_OK(c, cudaMemset(p + o_dpar, 0, c->pool_bytes - o_dpar));   // ... and the decoder's parent / middle-level arrays
   int rc = octree_encode_setup(c);
+  if (rc != GSNFS_OK) return rc;
+  rc = color_setup(c);
   if (rc != GSNFS_OK) return rc;
   return raht_setup(c);
 }
@@ -367,6 +372,43 @@ int gsnfs_raht_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const uint64_t* d_vo
   GSNFS_ON_DEVICE(ctx);
   return raht_done(ctx, run_raht(ctx, (cudaStream_t)stream, true, d_voxel_keys, d_weights, (uint32_t)n_voxels, d_counts, depth,
                                  d_coeff, d_qcoeff, channels, d_qcoeff ? qstep : nullptr, quant, nullptr, d_attr_out));
+}
+
+// ---- colour decorrelation in front of RAHT -----------------------------------------------------------
+static bool color_channels_ok(int channels) { return channels >= 11 && (channels - 11) % 3 == 0 && (channels - 11) / 3 <= 15; }
+
+uint64_t gsnfs_klt_floats(int channels) {
+  if (!color_channels_ok(channels)) return 0;
+  const uint64_t K = (uint64_t)(channels - 11) / 3;
+  return 3 * (2 * K + K * K);
+}
+
+int gsnfs_klt_fit(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr, uint64_t n_rows, const gsnfs_counts* d_counts,
+                  int channels, float* d_klt) {
+  if (!ctx || !color_channels_ok(channels) || n_rows >= (1ull << 30)) return GSNFS_E_INVALID_ARGUMENT;
+  if (channels > 11 && (!d_klt || (n_rows && !d_attr))) return GSNFS_E_INVALID_ARGUMENT;
+  if (n_rows > ctx->max_points || channels > GSNFS_MAX_CHANNELS) return GSNFS_E_CAPACITY;
+  GSNFS_ON_DEVICE(ctx);
+  return run_klt_fit(ctx, (cudaStream_t)stream, d_attr, (uint32_t)n_rows, d_counts, channels, d_klt);
+}
+
+static int color_apply(gsnfs_ctx* ctx, gsnfs_stream stream, bool inverse, const float* d_in, uint64_t n_rows,
+                       const gsnfs_counts* d_counts, int channels, const float* d_klt, float* d_out) {
+  if (!ctx || !color_channels_ok(channels) || n_rows >= (1ull << 30) || (n_rows && (!d_in || !d_out)))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (n_rows > ctx->max_points) return GSNFS_E_CAPACITY;
+  GSNFS_ON_DEVICE(ctx);
+  return run_color_apply(ctx, (cudaStream_t)stream, inverse, d_in, (uint32_t)n_rows, d_counts, channels, d_klt, d_out);
+}
+
+int gsnfs_color_forward(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr, uint64_t n_rows,
+                        const gsnfs_counts* d_counts, int channels, const float* d_klt, float* d_out) {
+  return color_apply(ctx, stream, false, d_attr, n_rows, d_counts, channels, d_klt, d_out);
+}
+
+int gsnfs_color_inverse(gsnfs_ctx* ctx, gsnfs_stream stream, const float* d_attr, uint64_t n_rows,
+                        const gsnfs_counts* d_counts, int channels, const float* d_klt, float* d_out) {
+  return color_apply(ctx, stream, true, d_attr, n_rows, d_counts, channels, d_klt, d_out);
 }
 
 // ---- RLGR entropy coder for the quantised coefficients ----------------------------------------------

@@ -113,6 +113,10 @@ struct gsnfs_ctx {
   int occ_cache[16];       // cached cudaOccupancyMaxActiveBlocksPerMultiprocessor results (0 = not yet queried)
   size_t occ_cache_smem[16];
 
+  // colour decorrelation: per-CTA partial moments of the KLT fit
+  double* color_partial;
+  uint32_t color_parts_cap;
+
   // RLGR: byte offset of every block stream (exclusive scan of the block sizes)
   uint64_t* rlgr_off;
   uint64_t rlgr_off_cap;
@@ -260,6 +264,11 @@ int run_rlgr_encode(gsnfs_ctx* ctx, cudaStream_t st, const int32_t* d_q, uint32_
 int run_rlgr_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_stream, uint64_t stream_bytes,
                     const uint32_t* d_block_bits, uint32_t n, int channels, uint32_t block, int32_t* d_q,
                     gsnfs_rlgr_info* d_info);
+int run_klt_fit(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, uint32_t n, const gsnfs_counts* d_counts, int channels,
+                float* d_klt);
+int run_color_apply(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const float* d_in, uint32_t n, const gsnfs_counts* d_counts,
+                    int channels, const float* d_klt, float* d_out);
+int color_setup(gsnfs_ctx* ctx);
 int raht_setup(gsnfs_ctx* ctx);   // occupancy queries + attributes, called from gsnfs_create
 
 }  // namespace gsnfs
