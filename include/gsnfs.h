@@ -259,6 +259,31 @@ int gsnfs_rlgr_decode(gsnfs_ctx* ctx, gsnfs_stream stream,
                       uint64_t n_rows, int channels, int block_size,
                       int32_t* d_qcoeff /* n_rows x channels */, gsnfs_rlgr_info* d_info);
 
+/* ---- entropy coder for the occupancy bytes: static order-0 rANS -------------------------------------
+ * PAPER.md:L170 ("To improve compression efficiency, GS-NFS then runs a GPU-based entropy encoder, ANS"), L283 (nvCOMP),
+ * L801 ("adds only ~0.3 ms but roughly halves the compressed size").  The paper calls a closed library; this is the
+ * published rANS construction, reading [R17]:
+ *   model: hist over the whole stream, quantised to sum 4096: f[s] = max(1, floor(hist[s] * 4096 / n)) for hist[s] > 0;
+ *   the remainder goes to the most frequent symbol, an excess is taken one at a time from the largest f;
+ *   blocks of GSNFS_RANS_BLOCK bytes are independent: 32-bit state, lower bound 2^16, 16-bit renormalisation, symbols
+ *   walked backwards from x = 2^16: if x >= f << 20: emit low 16 bits, x >>= 16; x = (x / f) * 4096 + x % f + cum[s];
+ *   block stream = final state (4 bytes LE) + its words (2 bytes LE each) in the order the decoder reads them.
+ * Stream header: d_freq[256] (uint16), d_nwords[gsnfs_rans_blocks(n)] (uint16); d_payload holds the blocks back to back.
+ * n is the byte count; if d_counts != NULL the actual count is read on the device from d_counts->occ_bytes (chained
+ * after gsnfs_octree_encode) and n is an upper bound.  d_info: stream_bytes = payload bytes, n_blocks, status (bit 0:
+ * corrupt stream / model on decode, bit 1: payload_capacity too small on encode -- nothing written).  d_data 4-byte
+ * aligned.  All pointers are caller-owned device memory; asynchronous on `stream`. */
+#define GSNFS_RANS_BLOCK 1024
+typedef gsnfs_rlgr_info gsnfs_rans_info;
+uint64_t gsnfs_rans_blocks(uint64_t n);
+uint64_t gsnfs_rans_capacity(uint64_t n);    /* payload bytes that always suffice (12 bits per byte + block states) */
+int gsnfs_rans_encode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_data, uint64_t n, const gsnfs_counts* d_counts,
+                      uint16_t* d_freq, uint16_t* d_nwords, uint8_t* d_payload, uint64_t payload_capacity,
+                      gsnfs_rans_info* d_info);
+int gsnfs_rans_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_payload, uint64_t payload_bytes,
+                      const uint16_t* d_freq, const uint16_t* d_nwords, uint64_t n, uint8_t* d_out,
+                      gsnfs_rans_info* d_info);
+
 /* ---- whole-frame calls on HOST buffers (copies inside; used for end-to-end timing) --------------- */
 /* encode = H2D(xyz, attr) -> octree_encode -> voxel_merge -> raht_forward(weights = counts) -> D2H.
  * Host outputs: h_occ[occ_capacity], h_level_sizes[depth+1], h_weights[n] (first N_v valid),

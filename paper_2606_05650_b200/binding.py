@@ -74,6 +74,11 @@ _SIGNATURES = {
                                   c_uint64, c_void_p]),
     "gsnfs_rlgr_decode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_uint64, c_int, c_int, c_void_p,
                                   c_void_p]),
+    "gsnfs_rans_blocks": (c_uint64, [c_uint64]),
+    "gsnfs_rans_capacity": (c_uint64, [c_uint64]),
+    "gsnfs_rans_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p, c_void_p, c_void_p, c_uint64,
+                                  c_void_p]),
+    "gsnfs_rans_decode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p]),
     "gsnfs_frame_encode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_int, POINTER(c_float),
                                         POINTER(c_float), c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p,
                                         c_uint64, c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -353,6 +358,30 @@ def gsnfs_rlgr_decode(ctx: Context, d_stream, stream_bytes, d_block_bits, n_rows
         _dptr(d_block_bits, torch.int32, "d_block_bits"), int(n_rows), int(channels), int(block_size),
         _dptr(d_qcoeff, torch.int32, "d_qcoeff"), _dptr(d_info, torch.int64, "d_info"))
     ctx._check(rc, "gsnfs_rlgr_decode")
+
+
+def gsnfs_rans_blocks(n: int) -> int:
+    return int(lib().gsnfs_rans_blocks(int(n)))
+
+
+def gsnfs_rans_capacity(n: int) -> int:
+    return int(lib().gsnfs_rans_capacity(int(n)))
+
+
+def gsnfs_rans_encode(ctx: Context, d_data, n, d_counts, d_freq, d_nwords, d_payload, d_info, stream=None):
+    rc = lib().gsnfs_rans_encode(
+        ctx.handle, _stream(stream), _dptr(d_data, torch.uint8, "d_data"), int(n), _dptr(d_counts, torch.int32, "d_counts"),
+        _dptr(d_freq, torch.int16, "d_freq"), _dptr(d_nwords, torch.int16, "d_nwords"),
+        _dptr(d_payload, torch.uint8, "d_payload"), int(d_payload.numel()), _dptr(d_info, torch.int64, "d_info"))
+    ctx._check(rc, "gsnfs_rans_encode")
+
+
+def gsnfs_rans_decode(ctx: Context, d_payload, payload_bytes, d_freq, d_nwords, n, d_out, d_info, stream=None):
+    rc = lib().gsnfs_rans_decode(
+        ctx.handle, _stream(stream), _dptr(d_payload, torch.uint8, "d_payload"), int(payload_bytes),
+        _dptr(d_freq, torch.int16, "d_freq"), _dptr(d_nwords, torch.int16, "d_nwords"), int(n),
+        _dptr(d_out, torch.uint8, "d_out"), _dptr(d_info, torch.int64, "d_info"))
+    ctx._check(rc, "gsnfs_rans_decode")
 
 
 def gsnfs_frame_encode_host(ctx: Context, h_xyz, h_attr, n, channels, bbox_min, bbox_max, depth, qstep, quant,

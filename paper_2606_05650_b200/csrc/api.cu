@@ -128,6 +128,9 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
   const size_t o_rplan = b.take(sizeof(RahtPlan));
   const size_t o_rrows = b.take(c->raht_pool_rows * (size_t)C * 4);
+  c->rans_blocks_cap = c->occ_cap / GSNFS_RANS_BLOCK + 64;
+  const size_t o_rah = b.take(256 * 4), o_ras = b.take(c->rans_blocks_cap * GSNFS_RANS_BLOCK * 2);
+  const size_t o_rast = b.take(c->rans_blocks_cap * 4), o_rao = b.take((c->rans_blocks_cap + 1) * 8);
   c->color_parts_cap = (uint32_t)c->num_sms * 2u;
   const size_t o_colp = b.take((size_t)c->color_parts_cap * 3 * 135 * sizeof(double));
   c->rlgr_off_cap = (N / GSNFS_RLGR_MIN_BLOCK + 1) * (uint64_t)C + 1;
@@ -149,11 +152,15 @@ static int create_impl(gsnfs_ctx* c) {
   c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);
   c->rlgr_off = (uint64_t*)(p + o_rlo);
   c->color_partial = (double*)(p + o_colp);
+  c->rans_hist = (uint32_t*)(p + o_rah); c->rans_scratch = (uint16_t*)(p + o_ras);
+  c->rans_states = (uint32_t*)(p + o_rast); c->rans_off = (uint64_t*)(p + o_rao);
   GSNFS_CUDA_OK(c, cudaMemset(c->pool, 0, o_rrows));     // everything but the big row pool ...
   GSNFS_CUDA_OK(c, cudaMemset(p + o_dpar, 0, c->pool_bytes - o_dpar));   // ... and the decoder's parent / middle-level arrays
   int rc = octree_encode_setup(c);
   if (rc != GSNFS_OK) return rc;
   rc = color_setup(c);
+  if (rc != GSNFS_OK) return rc;
+  rc = rans_setup(c);
   if (rc != GSNFS_OK) return rc;
   return raht_setup(c);
 }
@@ -446,6 +453,29 @@ int gsnfs_rlgr_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_stre
   GSNFS_ON_DEVICE(ctx);
   return run_rlgr_decode(ctx, (cudaStream_t)stream, d_stream, stream_bytes, d_block_bits, (uint32_t)n_rows, channels,
                          (uint32_t)block_size, d_qcoeff, d_info);
+}
+
+// ---- rANS entropy coder for the occupancy bytes -------------------------------------------------------
+uint64_t gsnfs_rans_blocks(uint64_t n) { return (n + GSNFS_RANS_BLOCK - 1) / GSNFS_RANS_BLOCK; }
+uint64_t gsnfs_rans_capacity(uint64_t n) { return n + n / 2 + 4 * gsnfs_rans_blocks(n) + 16; }     // 12 bits per byte at worst
+
+int gsnfs_rans_encode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_data, uint64_t n, const gsnfs_counts* d_counts,
+                      uint16_t* d_freq, uint16_t* d_nwords, uint8_t* d_payload, uint64_t payload_capacity,
+                      gsnfs_rans_info* d_info) {
+  if (!ctx || !d_freq || !d_info || (n && (!d_data || !d_nwords || !d_payload)) || ((uintptr_t)d_data & 3))
+    return GSNFS_E_INVALID_ARGUMENT;
+  if (n >= (1ull << 32)) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_ON_DEVICE(ctx);
+  return run_rans_encode(ctx, (cudaStream_t)stream, d_data, n, d_counts ? &d_counts->occ_bytes : nullptr, d_freq, d_nwords,
+                         d_payload, payload_capacity, d_info);
+}
+
+int gsnfs_rans_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_payload, uint64_t payload_bytes,
+                      const uint16_t* d_freq, const uint16_t* d_nwords, uint64_t n, uint8_t* d_out, gsnfs_rans_info* d_info) {
+  if (!ctx || !d_freq || !d_info || (n && (!d_payload || !d_nwords || !d_out))) return GSNFS_E_INVALID_ARGUMENT;
+  if (n >= (1ull << 32)) return GSNFS_E_INVALID_ARGUMENT;
+  GSNFS_ON_DEVICE(ctx);
+  return run_rans_decode(ctx, (cudaStream_t)stream, d_payload, payload_bytes, d_freq, d_nwords, n, d_out, d_info);
 }
 
 // ---- whole-frame calls on host buffers -----------------------------------------------------------

@@ -117,6 +117,13 @@ struct gsnfs_ctx {
   double* color_partial;
   uint32_t color_parts_cap;
 
+  // rANS (occupancy bytes): histogram, strided word scratch, block states and offsets
+  uint32_t* rans_hist;
+  uint16_t* rans_scratch;
+  uint32_t* rans_states;
+  uint64_t* rans_off;
+  uint64_t rans_blocks_cap;
+
   // RLGR: byte offset of every block stream (exclusive scan of the block sizes)
   uint64_t* rlgr_off;
   uint64_t rlgr_off_cap;
@@ -264,6 +271,11 @@ int run_rlgr_encode(gsnfs_ctx* ctx, cudaStream_t st, const int32_t* d_q, uint32_
 int run_rlgr_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_stream, uint64_t stream_bytes,
                     const uint32_t* d_block_bits, uint32_t n, int channels, uint32_t block, int32_t* d_q,
                     gsnfs_rlgr_info* d_info);
+int run_rans_encode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_data, uint64_t n, const uint32_t* n_dev, uint16_t* d_freq,
+                    uint16_t* d_nwords, uint8_t* d_payload, uint64_t capacity, gsnfs_rlgr_info* d_info);
+int run_rans_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_payload, uint64_t payload_bytes, const uint16_t* d_freq,
+                    const uint16_t* d_nwords, uint64_t n, uint8_t* d_out, gsnfs_rlgr_info* d_info);
+int rans_setup(gsnfs_ctx* ctx);
 int run_klt_fit(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, uint32_t n, const gsnfs_counts* d_counts, int channels,
                 float* d_klt);
 int run_color_apply(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const float* d_in, uint32_t n, const gsnfs_counts* d_counts,
