@@ -284,6 +284,46 @@ int gsnfs_rans_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_payl
                       const uint16_t* d_freq, const uint16_t* d_nwords, uint64_t n, uint8_t* d_out,
                       gsnfs_rans_info* d_info);
 
+/* ---- bitstream container (host only) -----------------------------------------------------------------
+ * PAPER.md:L176 ("J ... and the number of occupied nodes n_d at each level ... is encoded in the bitstream as
+ * metadata"), L526 ("The header stores the number of levels and the node count of each level"), L255 (per-attribute
+ * quantisation steps).  One coded frame = a fixed description + tagged sections (the arrays the device calls produce,
+ * copied to the host by the caller), framed into one checksummed byte buffer:
+ *   header (magic "GSNF", version, section count, gsnfs_frame_desc, CRC-32 of the whole file, total bytes)
+ *   | section table (id, offset, bytes) | payloads, each 8-byte aligned.  Little endian.
+ * gsnfs_container_unpack() does not copy: the returned sections point into `buf`.  A bad magic / version / checksum /
+ * section bound returns GSNFS_E_CORRUPT_STREAM.  This build's [R1] reading needs the leaf weights at the decoder
+ * (section GSNFS_SEC_WEIGHTS; absent = unit weights = the paper's stream). */
+#define GSNFS_MAX_SECTIONS 16
+enum {
+  GSNFS_SEC_LEVEL_SIZES = 1,  /* uint32[depth + 1]                                                */
+  GSNFS_SEC_QSTEP = 2,        /* float[channels]                                                  */
+  GSNFS_SEC_KLT = 3,          /* float[gsnfs_klt_floats(channels)] (optional)                     */
+  GSNFS_SEC_OCC_RAW = 4,      /* the occupancy bytes as they are                                  */
+  GSNFS_SEC_OCC_FREQ = 5,     /* rANS model: uint16[256]                                          */
+  GSNFS_SEC_OCC_NWORDS = 6,   /* rANS block word counts: uint16[gsnfs_rans_blocks(occ_bytes)]     */
+  GSNFS_SEC_OCC_PAYLOAD = 7,  /* rANS block streams                                               */
+  GSNFS_SEC_WEIGHTS = 8,      /* uint32[n_voxels] leaf weights (optional)                         */
+  GSNFS_SEC_COEF_BITS = 9,    /* RLGR header: uint32[gsnfs_rlgr_blocks(n_voxels, channels, rlgr_block)] */
+  GSNFS_SEC_COEF_STREAM = 10  /* RLGR block streams                                               */
+};
+typedef struct gsnfs_frame_desc {
+  uint32_t depth, channels, n_voxels, occ_bytes, rlgr_block, flags;   /* flags: free for the application */
+  float bbox_min[3], bbox_max[3];
+  float dz_round, recon_bias;
+} gsnfs_frame_desc;
+typedef struct gsnfs_section {
+  uint32_t id;
+  uint32_t reserved;
+  const uint8_t* data;   /* host */
+  uint64_t bytes;
+} gsnfs_section;
+uint64_t gsnfs_container_size(const gsnfs_section* sections, int n_sections);
+int gsnfs_container_pack(const gsnfs_frame_desc* desc, const gsnfs_section* sections, int n_sections,
+                         uint8_t* out /* host */, uint64_t capacity, uint64_t* written);
+int gsnfs_container_unpack(const uint8_t* buf /* host */, uint64_t bytes, gsnfs_frame_desc* desc,
+                           gsnfs_section* sections /* out, max_sections entries */, int max_sections, int* n_sections);
+
 /* ---- whole-frame calls on HOST buffers (copies inside; used for end-to-end timing) --------------- */
 /* encode = H2D(xyz, attr) -> octree_encode -> voxel_merge -> raht_forward(weights = counts) -> D2H.
  * Host outputs: h_occ[occ_capacity], h_level_sizes[depth+1], h_weights[n] (first N_v valid),

@@ -33,6 +33,21 @@ class GsnfsCounts(ctypes.Structure):
     _fields_ = [("n_voxels", c_uint32), ("occ_bytes", c_uint32), ("status", c_uint32), ("reserved", c_uint32)]
 
 
+class GsnfsFrameDesc(ctypes.Structure):
+    _fields_ = [("depth", c_uint32), ("channels", c_uint32), ("n_voxels", c_uint32), ("occ_bytes", c_uint32),
+                ("rlgr_block", c_uint32), ("flags", c_uint32), ("bbox_min", c_float * 3), ("bbox_max", c_float * 3),
+                ("dz_round", c_float), ("recon_bias", c_float)]
+
+
+class GsnfsSection(ctypes.Structure):
+    _fields_ = [("id", c_uint32), ("reserved", c_uint32), ("data", c_void_p), ("bytes", c_uint64)]
+
+
+SEC_LEVEL_SIZES, SEC_QSTEP, SEC_KLT, SEC_OCC_RAW, SEC_OCC_FREQ, SEC_OCC_NWORDS, SEC_OCC_PAYLOAD, SEC_WEIGHTS, SEC_COEF_BITS, \
+    SEC_COEF_STREAM = range(1, 11)
+GSNFS_MAX_SECTIONS = 16
+
+
 class GsnfsError(RuntimeError):
     def __init__(self, status: int, where: str, detail: str = ""):
         self.status = status
@@ -79,6 +94,11 @@ _SIGNATURES = {
     "gsnfs_rans_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p, c_void_p, c_void_p, c_uint64,
                                   c_void_p]),
     "gsnfs_rans_decode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p]),
+    "gsnfs_container_size": (c_uint64, [POINTER(GsnfsSection), c_int]),
+    "gsnfs_container_pack": (c_int, [POINTER(GsnfsFrameDesc), POINTER(GsnfsSection), c_int, c_void_p, c_uint64,
+                                     POINTER(c_uint64)]),
+    "gsnfs_container_unpack": (c_int, [c_void_p, c_uint64, POINTER(GsnfsFrameDesc), POINTER(GsnfsSection), c_int,
+                                       POINTER(c_int)]),
     "gsnfs_frame_encode_host": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_uint64, c_int, POINTER(c_float),
                                         POINTER(c_float), c_int, POINTER(c_float), POINTER(GsnfsQuant), c_void_p,
                                         c_uint64, c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -382,6 +402,37 @@ def gsnfs_rans_decode(ctx: Context, d_payload, payload_bytes, d_freq, d_nwords, 
         _dptr(d_freq, torch.int16, "d_freq"), _dptr(d_nwords, torch.int16, "d_nwords"), int(n),
         _dptr(d_out, torch.uint8, "d_out"), _dptr(d_info, torch.int64, "d_info"))
     ctx._check(rc, "gsnfs_rans_decode")
+
+
+def container_pack(desc: GsnfsFrameDesc, sections: dict) -> np.ndarray:
+    """{section id: contiguous numpy array} -> one uint8 buffer (host only; marshalling of gsnfs_container_pack)."""
+    arrs = {k: np.ascontiguousarray(v) for k, v in sections.items()}
+    secs = (GsnfsSection * len(arrs))()
+    for i, (k, a) in enumerate(arrs.items()):
+        secs[i] = GsnfsSection(int(k), 0, a.ctypes.data if a.nbytes else None, a.nbytes)
+    size = int(lib().gsnfs_container_size(secs, len(arrs)))
+    out = np.zeros(size, dtype=np.uint8)
+    written = c_uint64(0)
+    rc = lib().gsnfs_container_pack(ctypes.byref(desc), secs, len(arrs), out.ctypes.data, size, ctypes.byref(written))
+    if rc != GSNFS_OK:
+        raise GsnfsError(rc, "gsnfs_container_pack")
+    return out[:written.value]
+
+
+def container_unpack(buf: np.ndarray):
+    """uint8 buffer -> (GsnfsFrameDesc, {section id: uint8 view into buf}); raises GsnfsError on a damaged buffer."""
+    buf = np.ascontiguousarray(buf, dtype=np.uint8)
+    desc = GsnfsFrameDesc()
+    secs = (GsnfsSection * GSNFS_MAX_SECTIONS)()
+    n = c_int(0)
+    rc = lib().gsnfs_container_unpack(buf.ctypes.data, buf.nbytes, ctypes.byref(desc), secs, GSNFS_MAX_SECTIONS, ctypes.byref(n))
+    if rc != GSNFS_OK:
+        raise GsnfsError(rc, "gsnfs_container_unpack")
+    out = {}
+    for i in range(n.value):
+        off = (secs[i].data - buf.ctypes.data) if secs[i].bytes else 0
+        out[int(secs[i].id)] = buf[off:off + secs[i].bytes]
+    return desc, out
 
 
 def gsnfs_frame_encode_host(ctx: Context, h_xyz, h_attr, n, channels, bbox_min, bbox_max, depth, qstep, quant,

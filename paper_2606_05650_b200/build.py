@@ -15,7 +15,7 @@ ROOT = os.path.dirname(PKG_DIR)
 CSRC = os.path.join(PKG_DIR, "csrc")
 OBJ_DIR = os.path.join(PKG_DIR, "build")
 LIB_PATH = os.path.join(PKG_DIR, "libgsnfs.so")
-SOURCES = ["api.cu", "octree_encode.cu", "merge.cu", "octree_decode.cu", "raht_schedule.cu", "raht.cu", "rlgr.cu", "color.cu", "rans.cu"]
+SOURCES = ["api.cu", "octree_encode.cu", "merge.cu", "octree_decode.cu", "raht_schedule.cu", "raht.cu", "rlgr.cu", "color.cu", "rans.cu", "container.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
     "--fmad=true",                      # IEEE sqrt/div kept (no -use_fast_math): [R11]

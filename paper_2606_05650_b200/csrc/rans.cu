@@ -1,6 +1,6 @@
 // Entropy coding of the octree occupancy bytes: static order-0 range-ANS (rANS), in place of the closed nvCOMP ANS the
 // paper calls ("runs a GPU-based entropy encoder, ANS"; L283; L801 "adds only ~0.3 ms but roughly halves
-// the compressed size").  Rules = reading [R17] of DESIGN.md (the same as oracle/rans_oracle.c states them): one 12-bit
+// the compressed size").  Rules = reading [R17] of DESIGN.md: one 12-bit
 // frequency table per frame, independent blocks of 1024 bytes, 32-bit state with lower bound 2^16 and 16-bit
 // renormalisation words, a block = final state + words in decoder order.
 //

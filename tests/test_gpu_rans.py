@@ -123,3 +123,67 @@ def test_capacity_and_corruption(B, ctx):
     B.gsnfs_rans_decode(ctx, d_p, nbytes, d_f, d_nw, len(x), d_out, d_info)
     torch.cuda.synchronize()
     assert B.rlgr_info(d_info)[2] == 0 and np.array_equal(d_out.cpu().numpy(), x)
+
+
+def test_whole_frame_through_the_container(B):
+    """A frame coded on the device (octree -> rANS, merge + RAHT + quantiser -> RLGR), framed by gsnfs_container_pack,
+    parsed back, decoded on the device: voxels bit-exact, attributes as the raw-coefficient path gives them."""
+    fr = synth.make_frame(2)
+    n, C, J, blk = fr.n, fr.channels, fr.depth, 2048
+    ctx = B.Context(max_points=n, max_channels=C, max_depth=J)
+    try:
+        buf = B.FrameBuffers(n, C, J, DEV)
+        d_xyz, d_attr = torch.from_numpy(fr.xyz).to(DEV), torch.from_numpy(fr.attr).to(DEV)
+        B.encode_frame(ctx, buf, d_xyz, d_attr, fr.bbox_min, fr.bbox_max, fr.qstep)
+        cap = buf.occ.numel()
+        d_f = torch.zeros(256, dtype=torch.int16, device=DEV)
+        d_nw = torch.zeros(B.gsnfs_rans_blocks(cap), dtype=torch.int16, device=DEV)
+        d_p = torch.zeros(B.gsnfs_rans_capacity(cap), dtype=torch.uint8, device=DEV)
+        d_ri = torch.zeros(2, dtype=torch.int64, device=DEV)
+        B.gsnfs_rans_encode(ctx, buf.occ, cap, buf.counts, d_f, d_nw, d_p, d_ri)
+        d_bits = torch.zeros(B.gsnfs_rlgr_blocks(n, C, blk), dtype=torch.int32, device=DEV)
+        d_stream = torch.zeros(B.gsnfs_rlgr_capacity(n, C, blk), dtype=torch.uint8, device=DEV)
+        d_li = torch.zeros(2, dtype=torch.int64, device=DEV)
+        B.gsnfs_rlgr_encode(ctx, buf.qcoeff, n, buf.counts, C, blk, d_bits, d_stream, d_li)
+        torch.cuda.synchronize()
+        cnt = buf.counts.cpu().numpy()
+        nv, ob = int(cnt[0]), int(cnt[1])
+        pbytes, pblocks, _ = B.rlgr_info(d_ri)
+        sbytes, sblocks, _ = B.rlgr_info(d_li)
+        desc = B.GsnfsFrameDesc()
+        desc.depth, desc.channels, desc.n_voxels, desc.occ_bytes, desc.rlgr_block, desc.flags = J, C, nv, ob, blk, 0
+        desc.bbox_min[:] = fr.bbox_min.tolist(); desc.bbox_max[:] = fr.bbox_max.tolist()
+        desc.dz_round, desc.recon_bias = 1.0 / 3.0, 0.0
+        file = B.container_pack(desc, {
+            B.SEC_LEVEL_SIZES: buf.level_sizes.cpu().numpy(), B.SEC_QSTEP: fr.qstep,
+            B.SEC_OCC_FREQ: d_f.cpu().numpy(), B.SEC_OCC_NWORDS: d_nw[:pblocks].cpu().numpy(), B.SEC_OCC_PAYLOAD: d_p[:pbytes].cpu().numpy(),
+            B.SEC_WEIGHTS: buf.weights[:nv].cpu().numpy(),
+            B.SEC_COEF_BITS: d_bits[:B.gsnfs_rlgr_blocks(nv, C, blk)].cpu().numpy(), B.SEC_COEF_STREAM: d_stream[:sbytes].cpu().numpy()})
+        raw = n * 12 + n * C * 4
+        print(f"container: {file.size} bytes for a {raw}-byte frame ({raw / file.size:.2f}x; occupancy {ob} -> {pbytes})")
+        # ---- receiver
+        d2, sec = B.container_unpack(file)
+        J2, C2, nv2, ob2, blk2 = d2.depth, d2.channels, d2.n_voxels, d2.occ_bytes, d2.rlgr_block
+        levels = sec[B.SEC_LEVEL_SIZES].view(np.uint32)
+        qstep = sec[B.SEC_QSTEP].view(np.float32)
+        dev = lambda a, dt: torch.from_numpy(np.ascontiguousarray(a).view(dt).copy()).to(DEV)
+        r_occ = torch.zeros(max(ob2, 4), dtype=torch.uint8, device=DEV)
+        info = torch.zeros(2, dtype=torch.int64, device=DEV)
+        B.gsnfs_rans_decode(ctx, dev(sec[B.SEC_OCC_PAYLOAD], np.uint8), sec[B.SEC_OCC_PAYLOAD].size, dev(sec[B.SEC_OCC_FREQ], np.int16),
+                            dev(sec[B.SEC_OCC_NWORDS], np.int16), ob2, r_occ, info)
+        rbuf = B.FrameBuffers(nv2, C2, J2, DEV)
+        B.gsnfs_octree_decode(ctx, r_occ, ob2, levels, J2, rbuf.dec_xyz, rbuf.dec_keys, rbuf.dec_counts)
+        info2 = torch.zeros(2, dtype=torch.int64, device=DEV)
+        B.gsnfs_rlgr_decode(ctx, dev(sec[B.SEC_COEF_STREAM], np.uint8), sec[B.SEC_COEF_STREAM].size,
+                            dev(sec[B.SEC_COEF_BITS], np.int32), nv2, C2, blk2, rbuf.qcoeff, info2)
+        B.gsnfs_raht_inverse(ctx, rbuf.dec_keys, dev(sec[B.SEC_WEIGHTS], np.int32), nv2, rbuf.dec_counts, J2, rbuf.qcoeff, None, C2,
+                             qstep, (d2.dz_round, d2.recon_bias), rbuf.dec_attr)
+        torch.cuda.synchronize()
+        assert B.rlgr_info(info)[2] == 0 and B.rlgr_info(info2)[2] == 0 and int(rbuf.dec_counts.cpu()[2]) == 0
+        assert torch.equal(r_occ[:ob2], buf.occ[:ob]) and torch.equal(rbuf.qcoeff[:nv2], buf.qcoeff[:nv])
+        assert torch.equal(rbuf.dec_keys[:nv2], buf.voxel_keys[:nv])
+        B.decode_frame(ctx, buf, buf.level_sizes.cpu().numpy(), ob, fr.qstep)
+        torch.cuda.synchronize()
+        assert torch.equal(rbuf.dec_attr[:nv2], buf.dec_attr[:nv]) and torch.equal(rbuf.dec_xyz[:nv2], buf.dec_xyz[:nv])
+    finally:
+        ctx.close()
