@@ -304,7 +304,7 @@ def run_ours(args, rank, world, local_rank):
     sort_frac = (ab["_sort_total"] / (sort_ms * 1e-3) / 1e9 / peak) if sort_ms else None
 
     # ---- end to end through the host-buffer ABI calls (pinned host memory, copies inside the timed region)
-    RLGR_BLOCK = 2048                      # PAPER.md L257 "blocks (e.g., 2K or 4K successive coefficients)"
+    RLGR_BLOCK = 512                       # Table A.5's fastest block size (here too: profiles/r2_rlgr_blocks.md)
     e2e = e2e_raw = entropy = None
     if rank == 0 or world > 1:
         cap = B.gsnfs_occ_capacity(n, J)
@@ -349,6 +349,55 @@ def run_ours(args, rank, world, local_rank):
                "d2h_bytes_per_step": 16 + 4 * (J + 1) + 16 + side + 16 + 16 + nv_e * 12 + nv_e * C * 4, "steps": ks,
                "api": "gsnfs_frame_encode_host_packed + gsnfs_frame_decode_host_packed (coefficients as RLGR bytes, "
                       f"block {RLGR_BLOCK})", "coefficient_stream_bytes": sb}
+        # the same packed calls as a two-stage pipeline: a second context decodes frame t on its own stream (a second host
+        # thread) while this one encodes frame t + 1, so the two PCIe directions are busy at the same time -- the
+        # back-to-back streaming use-case; encoder and decoder share nothing but the host buffers
+        if world == 1:
+            import queue
+            ctx2 = B.Context(max_points=n, max_channels=C, max_depth=J, device=local_rank)
+            s_enc, s_dec = torch.cuda.Stream(), torch.cuda.Stream()
+            sets = []
+            for _ in range(2):
+                sets.append(dict(occ=pin(cap, dt=torch.uint8), lev=pin(J + 1, dt=torch.int32), w=pin(n, dt=torch.int32),
+                                 bits=pin(B.gsnfs_rlgr_blocks(n, C, RLGR_BLOCK), dt=torch.int32),
+                                 stream=pin(n * C * 4, dt=torch.uint8), cnt=pin(4, dt=torch.int32), info=pin(2, dt=torch.int64)))
+            h_out2, h_vx2, h_cnt3 = pin(n, C, dt=torch.float32), pin(n, 3, dt=torch.int32), pin(4, dt=torch.int32)
+            ready, free = queue.Queue(), queue.Queue()
+            kp = max(4, min(args.steps, 12))
+
+            def producer():
+                for i in range(kp + 2):
+                    b = free.get()
+                    B.gsnfs_frame_encode_host_packed(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None,
+                                                     RLGR_BLOCK, b["occ"], b["lev"], b["w"], b["bits"], b["stream"],
+                                                     b["cnt"], b["info"], stream=s_enc)
+                    ready.put(b)
+
+            def consumer(times):
+                for i in range(kp + 2):
+                    b = ready.get()
+                    if i == 2:
+                        times.append(time.perf_counter())          # two frames of warm-up, then kp timed frames
+                    B.gsnfs_frame_decode_host_packed(ctx2, b["occ"], int(b["cnt"][1]), b["lev"].numpy(), J, b["w"], b["bits"],
+                                                     b["stream"], int(b["info"][0]), RLGR_BLOCK, C, fr.qstep, None, h_vx2,
+                                                     h_out2, h_cnt3, stream=s_dec)
+                    free.put(b)
+                times.append(time.perf_counter())
+
+            for b in sets:
+                free.put(b)
+            times = []
+            ta, tb = threading.Thread(target=producer), threading.Thread(target=consumer, args=(times,))
+            torch.cuda.synchronize()
+            ta.start(); tb.start(); ta.join(); tb.join()
+            torch.cuda.synchronize()
+            ms_pp = (times[1] - times[0]) * 1e3 / kp
+            ok_pp = bool(torch.equal(h_out2[:nv_e], h_out[:nv_e]))
+            e2e["pipelined"] = {"value": round(n / (ms_pp * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_pp, 4),
+                                "frames": kp, "same_output_as_serial": ok_pp,
+                                "how": "encoder thread + decoder thread, one context and stream each, double-buffered pinned "
+                                       "host buffers; host wall clock over the timed frames (all calls are blocking)"}
+            ctx2.close()
         ms_r, ks = time_e2e(raw_step)
         e2e_raw = {"value": round(world * n / (ms_r * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_r, 4),
                    "h2d_bytes_per_step": n * 12 + n * C * 4 + ob_e + nv_e * 4 + nv_e * C * 4,

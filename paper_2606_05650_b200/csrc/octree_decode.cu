@@ -55,8 +55,9 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
                                                             uint32_t* __restrict__ tile_sums, uint32_t* __restrict__ PD,
                                                             uint64_t* __restrict__ Kmid,
                                                             uint32_t* __restrict__ xyz, uint64_t* __restrict__ keys_out,
-                                                            gsnfs_counts* __restrict__ counts) {
+                                                            gsnfs_counts* __restrict__ counts, RahtPlan* __restrict__ tl) {
   cg::grid_group grid = cg::this_grid();
+  GSNFS_TSTAMP(tl, 0);
   __shared__ uint32_t s_w[9];
   __shared__ uint16_t s_stage[8 * kScanTile];   // a tile's (node-in-tile << 3 | digit) entries on their way out
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -90,7 +91,9 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
     }
     __syncthreads();
   }
+  GSNFS_TSTAMP(tl, 1);
   grid.sync();
+  GSNFS_TSTAMP(tl, 2);
   // ---- 2. down-sweep: (parent << 3 | digit) of every child.  The children of a tile are one contiguous id range:
   // staged in shared memory as 16-bit (node-in-tile << 3 | digit), written out coalesced.  The tile's base (number of
   // children before it) is carried from the CTA's previous tile by summing the tile sums in between.
@@ -148,7 +151,9 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
       __syncthreads();
     }
   }
+  GSNFS_TSTAMP(tl, 3);
   grid.sync();
+  GSNFS_TSTAMP(tl, 4);
   // ---- header vs stream, level by level [O12]: with the node count right and no childless node, level e + 1 starts
   // at the header's offset iff its first node is the first child of level e's first node and the node before it is
   // the last child of the node before that
@@ -197,7 +202,9 @@ __global__ void __launch_bounds__(256) octree_decode_kernel(const uint8_t* __res
         }
       }
     }
+    GSNFS_TSTAMP(tl, 5 + 2 * stage);
     if (stage == 0) grid.sync();
+    GSNFS_TSTAMP(tl, 6 + 2 * stage);
   }
 }
 
@@ -264,7 +271,8 @@ int run_octree_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_occ, uin
   if (grid > want) grid = want;
   if (grid < 1) grid = 1;
   void* args[] = {(void*)&d_occ, (void*)&S, (void*)&lv, (void*)&ctx->scan_sums,
-                  (void*)&ctx->dec_parent, (void*)&ctx->dec_kmid, (void*)&d_voxel_xyz, (void*)&d_voxel_keys, (void*)&d_counts};
+                  (void*)&ctx->dec_parent, (void*)&ctx->dec_kmid, (void*)&d_voxel_xyz, (void*)&d_voxel_keys, (void*)&d_counts,
+                  (void*)&ctx->raht_plan};
   GSNFS_KERNEL(ctx, st, "octree_decode");
   GSNFS_CUDA_OK(ctx, cudaLaunchCooperativeKernel((void*)octree_decode_kernel, dim3(grid), dim3(256), args, 0, st));
   GSNFS_LAUNCH_CHECK(ctx, st);
