@@ -426,10 +426,70 @@ def run_ours(args, rank, world, local_rank):
                 enc_t.append(ev3[0].elapsed_time(ev3[1]))
                 dec_t.append(ev3[1].elapsed_time(ev3[2]))
         ok = bool(torch.equal(d_back[:nv], buf.qcoeff[:nv])) and B.rlgr_info(d_info)[2] == 0
+        sweep = None
+        if args.rlgr_sweep:                                   # Table A.5's axis: block size vs latency and size
+            sweep = []
+            for blk in (256, 512, 1024, 2048, 4096, 8192):
+                sb_bits = torch.empty(B.gsnfs_rlgr_blocks(n, C, blk), dtype=torch.int32, device=dev)
+                te, td = [], []
+                for it in range(6):
+                    ev3[0].record(stream)
+                    B.gsnfs_rlgr_encode(ctx, buf.qcoeff, n, buf.counts, C, blk, sb_bits, d_stream, d_info)
+                    ev3[1].record(stream)
+                    torch.cuda.synchronize()
+                    sb_bytes = B.rlgr_info(d_info)[0]
+                    B.gsnfs_rlgr_decode(ctx, d_stream, sb_bytes, sb_bits, nv, C, blk, d_back, d_info)
+                    ev3[2].record(stream)
+                    torch.cuda.synchronize()
+                    if it >= 2:
+                        te.append(ev3[0].elapsed_time(ev3[1])); td.append(ev3[1].elapsed_time(ev3[2]))
+                sweep.append({"block": blk, "encode_ms": round(float(np.median(te)), 4), "decode_ms": round(float(np.median(td)), 4),
+                              "stream_bytes": sb_bytes})
+        # the other stages around the path: occupancy bytes through rANS (NEXT-3), colour decorrelation (NEXT-2)
+        cap_o = buf.occ.numel()
+        a_f = torch.zeros(256, dtype=torch.int16, device=dev)
+        a_nw = torch.zeros(B.gsnfs_rans_blocks(cap_o), dtype=torch.int16, device=dev)
+        a_p = torch.zeros(B.gsnfs_rans_capacity(cap_o), dtype=torch.uint8, device=dev)
+        a_back = torch.zeros(cap_o, dtype=torch.uint8, device=dev)
+        others = {}
+        t_a, t_b = [], []
+        for it in range(6):
+            ev3[0].record(stream)
+            B.gsnfs_rans_encode(ctx, buf.occ, cap_o, buf.counts, a_f, a_nw, a_p, d_info)
+            ev3[1].record(stream)
+            torch.cuda.synchronize()
+            pb = B.rlgr_info(d_info)[0]
+            B.gsnfs_rans_decode(ctx, a_p, pb, a_f, a_nw, s_occ, a_back, d_info)
+            ev3[2].record(stream)
+            torch.cuda.synchronize()
+            if it >= 2:
+                t_a.append(ev3[0].elapsed_time(ev3[1])); t_b.append(ev3[1].elapsed_time(ev3[2]))
+        others["occupancy_rans"] = {"encode_ms": round(float(np.median(t_a)), 4), "decode_ms": round(float(np.median(t_b)), 4),
+                                    "bytes_in": s_occ, "bytes_out": pb, "ratio": round(s_occ / max(pb, 1), 3),
+                                    "roundtrip_exact": bool(torch.equal(a_back[:s_occ], buf.occ[:s_occ]))}
+        if B.gsnfs_klt_floats(C):
+            d_klt = torch.zeros(B.gsnfs_klt_floats(C), dtype=torch.float32, device=dev)
+            t_a, t_b, t_c = [], [], []
+            ev4 = [torch.cuda.Event(enable_timing=True) for _ in range(4)]
+            for it in range(6):
+                ev4[0].record(stream)
+                B.gsnfs_klt_fit(ctx, d_attr, n, None, C, d_klt)
+                ev4[1].record(stream)
+                B.gsnfs_color_forward(ctx, d_attr, n, None, C, d_klt, buf.merged)
+                ev4[2].record(stream)
+                B.gsnfs_color_inverse(ctx, buf.merged, n, None, C, d_klt, buf.merged)
+                ev4[3].record(stream)
+                torch.cuda.synchronize()
+                if it >= 2:
+                    t_a.append(ev4[0].elapsed_time(ev4[1])); t_b.append(ev4[1].elapsed_time(ev4[2])); t_c.append(ev4[2].elapsed_time(ev4[3]))
+            others["colour_decorrelation"] = {"klt_fit_ms": round(float(np.median(t_a)), 4), "forward_ms": round(float(np.median(t_b)), 4),
+                                              "inverse_ms": round(float(np.median(t_c)), 4),
+                                              "max_abs_roundtrip_error": float((buf.merged[:n] - d_attr).abs().max())}
         entropy = {"coder": f"block-parallel RLGR, block {RLGR_BLOCK} (PAPER.md L257, L803)", "encode_ms": round(float(np.median(enc_t)), 4),
                    "decode_ms": round(float(np.median(dec_t)), 4), "stream_bytes": sbytes, "raw_bytes": nv * C * 4,
                    "ratio": round(nv * C * 4 / max(sbytes, 1), 3), "roundtrip_exact": ok,
-                   "note": "synthetic attributes are i.i.d. (SURVEY 8(d)): the ratio is not a compression claim"}
+                   "note": "synthetic attributes are i.i.d. (SURVEY 8(d)): the ratio is not a compression claim",
+                   "block_sweep": sweep, "other_stages": others}
 
     ladder = None
     if rank == 0 and world == 1 and args.ladder_frames > 0 and args.config == "3" and args.n_override is None:
@@ -542,6 +602,7 @@ def main():
                     help="BASELINE.json config (1-based); 3 = headline 1M frame; pc = point-cloud shaped frame (NEXT-4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--rlgr-sweep", action="store_true", help="also time the RLGR coder at Table A.5's block sizes")
     ap.add_argument("--n-override", type=int, default=None,
                     help="same recipe with another N (e.g. 16000000: key arrays no longer fit the 126 MB L2); not the headline")
     ap.add_argument("--ladder-frames", type=int, default=300,

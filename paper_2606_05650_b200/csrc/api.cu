@@ -134,7 +134,8 @@ static int create_impl(gsnfs_ctx* c) {
   c->color_parts_cap = (uint32_t)c->num_sms * 2u;
   const size_t o_colp = b.take((size_t)c->color_parts_cap * 3 * 135 * sizeof(double));
   c->rlgr_off_cap = (N / GSNFS_RLGR_MIN_BLOCK + 1) * (uint64_t)C + 1;
-  const size_t o_rlo = b.take(c->rlgr_off_cap * 8);
+  c->rlgr_rows_cap = N / GSNFS_RLGR_MIN_BLOCK + 2;
+  const size_t o_rlo = b.take(c->rlgr_rows_cap * 8), o_rls = b.take((c->rlgr_rows_cap / 256 + 2) * 8);
   const size_t o_dpar = b.take((c->occ_cap + N + 2) * 4), o_dkm = b.take((N + 1) * 8);
   c->pool_bytes = b.off;
   GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->pool, c->pool_bytes));
@@ -150,7 +151,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
   c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);
-  c->rlgr_off = (uint64_t*)(p + o_rlo);
+  c->rlgr_rowsum = (uint64_t*)(p + o_rlo); c->rlgr_supersum = (uint64_t*)(p + o_rls);
   c->color_partial = (double*)(p + o_colp);
   c->rans_hist = (uint32_t*)(p + o_rah); c->rans_scratch = (uint16_t*)(p + o_ras);
   c->rans_states = (uint32_t*)(p + o_rast); c->rans_off = (uint64_t*)(p + o_rao);

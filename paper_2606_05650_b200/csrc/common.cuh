@@ -124,9 +124,11 @@ struct gsnfs_ctx {
   uint64_t* rans_off;
   uint64_t rans_blocks_cap;
 
-  // RLGR: byte offset of every block stream (exclusive scan of the block sizes)
-  uint64_t* rlgr_off;
-  uint64_t rlgr_off_cap;
+  // RLGR: bytes of every block row and of every 256 block rows (stream offsets without a scan pass)
+  uint64_t* rlgr_rowsum;
+  uint64_t* rlgr_supersum;
+  uint64_t rlgr_rows_cap;
+  uint64_t rlgr_off_cap;   // entries of a block header at the smallest block size (staging of the *_host_packed calls)
 
   // decode
   uint64_t* dec_kmid;      // Morton codes of the decoder's middle level (max_points + 1 entries)

@@ -71,25 +71,83 @@ __device__ __forceinline__ void gr_put(BitSink<WRITE>& s, uint32_t u, int& kRP) 
 }
 
 // One CTA = the blocks (b, c) of one block of rows b, thread c = channel c.
+// Offsets without a scan pass: the count pass leaves, per block row b, the bytes of its C streams (rowsum[b]) and, per
+// 256 block rows, their sum (supersum).  Row b then starts at sum(supersum[0 .. b/256)) + sum(rowsum[256 (b/256) .. b)), and
+// channel c inside the row at the exclusive prefix of the row's block sizes -- a few hundred cached loads per CTA.
+constexpr uint32_t kRowGroup = 256;
+
+struct RowOffsets { uint64_t row_start, total; };
+// all threads of the CTA call it; nrows = block rows of the tensor (host upper bound)
+__device__ RowOffsets rlgr_row_offsets(const uint64_t* __restrict__ rowsum, const uint64_t* __restrict__ supersum,
+                                       uint32_t b, uint32_t nrows, uint64_t* s_red /* 2 */) {
+  const uint32_t ng = (nrows + kRowGroup - 1) / kRowGroup, g = b / kRowGroup;
+  uint64_t before = 0, total = 0;
+  for (uint32_t i = threadIdx.x; i < ng; i += blockDim.x) { const uint64_t v = supersum[i]; total += v; if (i < g) before += v; }
+  for (uint32_t i = g * kRowGroup + threadIdx.x; i < b; i += blockDim.x) before += rowsum[i];
+  if (threadIdx.x == 0) { s_red[0] = 0; s_red[1] = 0; }
+  __syncthreads();
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    before += __shfl_xor_sync(0xffffffffu, before, o);
+    total += __shfl_xor_sync(0xffffffffu, total, o);
+  }
+  if ((threadIdx.x & 31) == 0) { atomicAdd((unsigned long long*)&s_red[0], before); atomicAdd((unsigned long long*)&s_red[1], total); }
+  __syncthreads();
+  RowOffsets r;
+  r.row_start = s_red[0];
+  r.total = s_red[1];
+  return r;
+}
+// exclusive prefix over the threads of the CTA (blockDim.x <= 256) of one 32-bit value each; returns the CTA total too
+__device__ __forceinline__ uint32_t cta_excl_scan(uint32_t v, uint32_t* s_w /* 9 */, uint32_t* total) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nw = (blockDim.x + 31) >> 5;
+  uint32_t inc = v;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t t = __shfl_up_sync(0xffffffffu, inc, o); if (lane >= o) inc += t; }
+  if (lane == 31) s_w[warp] = inc;
+  __syncthreads();
+  uint32_t before = 0, tot = 0;
+  for (int w = 0; w < nw; ++w) { const uint32_t x = s_w[w]; if (w < warp) before += x; tot += x; }
+  *total = tot;
+  return before + inc - v;
+}
+
 template <bool WRITE>
 __global__ void __launch_bounds__(256) rlgr_encode_kernel(const int32_t* __restrict__ q, uint32_t n_host,
                                                           const uint32_t* __restrict__ n_dev, int C, uint32_t B,
-                                                          uint32_t* __restrict__ block_bits,
-                                                          const uint64_t* __restrict__ block_off,
-                                                          uint8_t* __restrict__ stream, const gsnfs_rlgr_info* __restrict__ info) {
+                                                          uint32_t* __restrict__ block_bits, uint64_t* __restrict__ rowsum,
+                                                          uint64_t* __restrict__ supersum, uint64_t capacity,
+                                                          uint8_t* __restrict__ stream, gsnfs_rlgr_info* __restrict__ info) {
+  __shared__ uint64_t s_red[2];
+  __shared__ uint32_t s_w[9];
   const uint32_t n = n_dev ? min(*n_dev, n_host) : n_host;
   const uint32_t b = blockIdx.x;
   const int c = threadIdx.x;
   const uint64_t r0 = (uint64_t)b * B;
-  if (c >= C) return;
-  if (r0 >= n) {                         // block row beyond the actual N_v (n_host was an upper bound)
-    if (!WRITE) block_bits[(size_t)b * C + c] = 0u;
+  const bool active = c < C && r0 < n;
+  if (!WRITE && r0 >= n) {               // block row beyond the actual N_v (n_host was an upper bound)
+    if (c < C) block_bits[(size_t)b * C + c] = 0u;
+    if (c == 0) rowsum[b] = 0ull;
     return;
   }
-  if (WRITE && info->status) return;     // the stream does not fit the caller's buffer: nothing is written
-  const uint32_t cnt = (uint32_t)min((uint64_t)B, (uint64_t)n - r0);
+  uint64_t my_off = 0;
+  if (WRITE) {
+    if (r0 >= n) return;
+    const RowOffsets ro = rlgr_row_offsets(rowsum, supersum, b, gridDim.x, s_red);
+    uint32_t rtot;
+    const uint32_t ex = cta_excl_scan(c < C ? block_bits[(size_t)b * C + c] >> 3 : 0u, s_w, &rtot);
+    my_off = ro.row_start + ex;
+    if (b == 0 && c == 0) {
+      info->stream_bytes = ro.total;
+      info->n_blocks = gridDim.x * (uint32_t)C;
+      info->status = ro.total > capacity ? 2u : 0u;
+    }
+    if (ro.total > capacity) return;     // the stream does not fit the caller's buffer: nothing is written
+  }
+  if (!active && WRITE) return;
+  const uint32_t cnt = active ? (uint32_t)min((uint64_t)B, (uint64_t)n - r0) : 0u;
   BitSink<WRITE> s;
-  if (WRITE) s.out = reinterpret_cast<uint32_t*>(stream + block_off[(size_t)b * C + c]);
+  if (WRITE) s.out = reinterpret_cast<uint32_t*>(stream + my_off);
   const int32_t* src = q + r0 * C + c;
   int kP = 0, kRP = 8;
   uint32_t run = 0;
@@ -118,48 +176,28 @@ __global__ void __launch_bounds__(256) rlgr_encode_kernel(const int32_t* __restr
   }
   if (run > 0) s.put(0u, 1u);
   s.finish();
-  if (!WRITE) block_bits[(size_t)b * C + c] = (uint32_t)s.total;
+  if (!WRITE) {
+    if (active) block_bits[(size_t)b * C + c] = (uint32_t)s.total;
+    uint32_t rtot;
+    (void)cta_excl_scan(active ? (uint32_t)(s.total >> 3) : 0u, s_w, &rtot);
+    if (c == 0) {
+      rowsum[b] = rtot;
+      atomicAdd((unsigned long long*)&supersum[b / kRowGroup], (unsigned long long)rtot);
+    }
+  }
 }
 
-// one CTA: exclusive scan of the block sizes (bytes) -> offsets; total, block count, overflow status
-__global__ void __launch_bounds__(1024) rlgr_scan_kernel(const uint32_t* __restrict__ block_bits, uint64_t nent,
-                                                         uint64_t* __restrict__ block_off, uint64_t capacity,
-                                                         gsnfs_rlgr_info* __restrict__ info) {
-  __shared__ uint64_t s_warp[33];
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  uint64_t carry = 0;
-  for (uint64_t base = 0; base < nent; base += 1024) {
-    const uint64_t i = base + tid;
-    const uint64_t v = i < nent ? (uint64_t)(block_bits[i] >> 3) : 0ull;
-    uint64_t inc = v;
-#pragma unroll
-    for (int o = 1; o < 32; o <<= 1) {
-      const uint64_t t = __shfl_up_sync(0xffffffffu, inc, o);
-      if (lane >= o) inc += t;
-    }
-    if (lane == 31) s_warp[warp] = inc;
-    __syncthreads();
-    if (warp == 0) {
-      const uint64_t w = s_warp[lane];
-      uint64_t winc = w;
-#pragma unroll
-      for (int o = 1; o < 32; o <<= 1) {
-        const uint64_t t = __shfl_up_sync(0xffffffffu, winc, o);
-        if (lane >= o) winc += t;
-      }
-      s_warp[lane] = winc - w;
-      if (lane == 31) s_warp[32] = winc;
-    }
-    __syncthreads();
-    if (i < nent) block_off[i] = carry + s_warp[warp] + inc - v;
-    carry += s_warp[32];
-    __syncthreads();
-  }
-  if (tid == 0) {
-    block_off[nent] = carry;
-    info->stream_bytes = carry;
-    info->n_blocks = (uint32_t)nent;
-    info->status = carry > capacity ? 2u : 0u;
+// decoder side: the same two sums from the stream header
+__global__ void __launch_bounds__(256) rlgr_rowsum_kernel(const uint32_t* __restrict__ block_bits, int C,
+                                                          uint64_t* __restrict__ rowsum, uint64_t* __restrict__ supersum) {
+  __shared__ uint32_t s_w[9];
+  const uint32_t b = blockIdx.x;
+  const int c = threadIdx.x;
+  uint32_t rtot;
+  (void)cta_excl_scan(c < C ? block_bits[(size_t)b * C + c] >> 3 : 0u, s_w, &rtot);
+  if (c == 0) {
+    rowsum[b] = rtot;
+    atomicAdd((unsigned long long*)&supersum[b / kRowGroup], (unsigned long long)rtot);
   }
 }
 
@@ -217,15 +255,22 @@ __device__ __forceinline__ uint32_t gr_get(BitSource& s, int& kRP) {
 
 __global__ void __launch_bounds__(256) rlgr_decode_kernel(const uint8_t* __restrict__ stream, uint64_t stream_bytes,
                                                           const uint32_t* __restrict__ block_bits,
-                                                          const uint64_t* __restrict__ block_off, uint32_t n, int C, uint32_t B,
+                                                          const uint64_t* __restrict__ rowsum,
+                                                          const uint64_t* __restrict__ supersum, uint32_t n, int C, uint32_t B,
                                                           int32_t* __restrict__ q, gsnfs_rlgr_info* __restrict__ info) {
+  __shared__ uint64_t s_red[2];
+  __shared__ uint32_t s_w[9];
   const uint32_t b = blockIdx.x;
   const int c = threadIdx.x;
   const uint64_t r0 = (uint64_t)b * B;
+  const RowOffsets ro = rlgr_row_offsets(rowsum, supersum, b, gridDim.x, s_red);
+  uint32_t rtot;
+  const uint32_t ex = cta_excl_scan(c < C ? block_bits[(size_t)b * C + c] >> 3 : 0u, s_w, &rtot);
+  if (b == 0 && c == 0) { info->stream_bytes = ro.total; info->n_blocks = gridDim.x * (uint32_t)C; }
   if (c >= C || r0 >= n) return;
   const uint32_t cnt = (uint32_t)min((uint64_t)B, (uint64_t)n - r0);
   const size_t e = (size_t)b * C + c;
-  const uint64_t off = block_off[e], bytes = block_bits[e] >> 3;
+  const uint64_t off = ro.row_start + ex, bytes = block_bits[e] >> 3;
   int32_t* dst = q + r0 * C + c;
   if ((block_bits[e] & 31u) || off + bytes > stream_bytes) {      // header inconsistent with the stream
     atomicOr(&info->status, 1u);
@@ -275,8 +320,7 @@ int run_rlgr_encode(gsnfs_ctx* ctx, cudaStream_t st, const int32_t* d_q, uint32_
                     int channels, uint32_t block, uint32_t* d_block_bits, uint8_t* d_stream, uint64_t capacity,
                     gsnfs_rlgr_info* d_info) {
   const uint32_t nblk = (n + block - 1) / block;
-  const uint64_t nent = (uint64_t)nblk * (uint64_t)channels;
-  if (nent + 1 > ctx->rlgr_off_cap) return GSNFS_E_CAPACITY;
+  if (nblk + 1 > ctx->rlgr_rows_cap) return GSNFS_E_CAPACITY;
   if (n == 0) {
     GSNFS_KERNEL(ctx, st, "rlgr_info");
     rlgr_info_kernel<<<1, 1, 0, st>>>(d_info, 0ull, 0u, 0u);
@@ -285,14 +329,14 @@ int run_rlgr_encode(gsnfs_ctx* ctx, cudaStream_t st, const int32_t* d_q, uint32_
   }
   const uint32_t* n_dev = d_counts ? &d_counts->n_voxels : nullptr;
   const int threads = (channels + 31) & ~31;
+  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->rlgr_supersum, 0, sizeof(uint64_t) * (nblk / kRowGroup + 1), st));
   GSNFS_KERNEL(ctx, st, "rlgr_count");
-  rlgr_encode_kernel<false><<<nblk, threads, 0, st>>>(d_q, n, n_dev, channels, block, d_block_bits, nullptr, nullptr, nullptr);
-  GSNFS_LAUNCH_CHECK(ctx, st);
-  GSNFS_KERNEL(ctx, st, "rlgr_scan");
-  rlgr_scan_kernel<<<1, 1024, 0, st>>>(d_block_bits, nent, ctx->rlgr_off, capacity, d_info);
+  rlgr_encode_kernel<false><<<nblk, threads, 0, st>>>(d_q, n, n_dev, channels, block, d_block_bits, ctx->rlgr_rowsum,
+                                                      ctx->rlgr_supersum, 0ull, nullptr, nullptr);
   GSNFS_LAUNCH_CHECK(ctx, st);
   GSNFS_KERNEL(ctx, st, "rlgr_write");
-  rlgr_encode_kernel<true><<<nblk, threads, 0, st>>>(d_q, n, n_dev, channels, block, d_block_bits, ctx->rlgr_off, d_stream, d_info);
+  rlgr_encode_kernel<true><<<nblk, threads, 0, st>>>(d_q, n, n_dev, channels, block, d_block_bits, ctx->rlgr_rowsum,
+                                                     ctx->rlgr_supersum, capacity, d_stream, d_info);
   GSNFS_LAUNCH_CHECK(ctx, st);
   return GSNFS_OK;
 }
@@ -301,20 +345,19 @@ int run_rlgr_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_stream, ui
                     const uint32_t* d_block_bits, uint32_t n, int channels, uint32_t block, int32_t* d_q,
                     gsnfs_rlgr_info* d_info) {
   const uint32_t nblk = (n + block - 1) / block;
-  const uint64_t nent = (uint64_t)nblk * (uint64_t)channels;
-  if (nent + 1 > ctx->rlgr_off_cap) return GSNFS_E_CAPACITY;
-  if (n == 0) {
-    GSNFS_KERNEL(ctx, st, "rlgr_info");
-    rlgr_info_kernel<<<1, 1, 0, st>>>(d_info, 0ull, 0u, stream_bytes ? 1u : 0u);
-    GSNFS_LAUNCH_CHECK(ctx, st);
-    return GSNFS_OK;
-  }
-  GSNFS_KERNEL(ctx, st, "rlgr_scan");
-  rlgr_scan_kernel<<<1, 1024, 0, st>>>(d_block_bits, nent, ctx->rlgr_off, ~0ull, d_info);      // offsets from the header
+  if (nblk + 1 > ctx->rlgr_rows_cap) return GSNFS_E_CAPACITY;
+  GSNFS_KERNEL(ctx, st, "rlgr_info");
+  rlgr_info_kernel<<<1, 1, 0, st>>>(d_info, 0ull, 0u, (n == 0 && stream_bytes) ? 1u : 0u);
   GSNFS_LAUNCH_CHECK(ctx, st);
+  if (n == 0) return GSNFS_OK;
   const int threads = (channels + 31) & ~31;
+  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->rlgr_supersum, 0, sizeof(uint64_t) * (nblk / kRowGroup + 1), st));
+  GSNFS_KERNEL(ctx, st, "rlgr_rowsum");
+  rlgr_rowsum_kernel<<<nblk, threads, 0, st>>>(d_block_bits, channels, ctx->rlgr_rowsum, ctx->rlgr_supersum);
+  GSNFS_LAUNCH_CHECK(ctx, st);
   GSNFS_KERNEL(ctx, st, "rlgr_decode");
-  rlgr_decode_kernel<<<nblk, threads, 0, st>>>(d_stream, stream_bytes, d_block_bits, ctx->rlgr_off, n, channels, block, d_q, d_info);
+  rlgr_decode_kernel<<<nblk, threads, 0, st>>>(d_stream, stream_bytes, d_block_bits, ctx->rlgr_rowsum, ctx->rlgr_supersum, n,
+                                               channels, block, d_q, d_info);
   GSNFS_LAUNCH_CHECK(ctx, st);
   return GSNFS_OK;
 }
