@@ -123,6 +123,7 @@ static int create_impl(gsnfs_ctx* c) {
   const size_t o_rpend = b.take(c->raht_hdr_cap * 128 * sizeof(uint4));
   const size_t o_rbs = b.take((size_t)c->raht_bsum_cap * 4);
   const size_t o_rgs = b.take(N * 4);
+  const size_t o_mpart = b.take(2 * (N / 256 + 2) * (size_t)C * 8);
   const size_t o_rrec = b.take(c->raht_rec_cap * sizeof(uint4));
   const size_t o_rhdr = b.take(c->raht_hdr_cap * sizeof(RahtTileHdr));
   const size_t o_rtp = b.take(c->raht_hdr_cap * 4);
@@ -148,6 +149,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->scan_sums = (uint32_t*)(p + o_ssums);
   c->raht_pend = (uint4*)(p + o_rpend); c->raht_bsum = (uint32_t*)(p + o_rbs);
   c->raht_rec = (uint4*)(p + o_rrec); c->raht_gsrc = (uint32_t*)(p + o_rgs);
+  c->merge_partial = (double*)(p + o_mpart);
   c->raht_hdr = (RahtTileHdr*)(p + o_rhdr); c->raht_tile_pend = (uint32_t*)(p + o_rtp);
   c->raht_plan = (RahtPlan*)(p + o_rplan); c->raht_rows = (float*)(p + o_rrows);
   c->dec_parent = (uint32_t*)(p + o_dpar); c->dec_kmid = (uint64_t*)(p + o_dkm);

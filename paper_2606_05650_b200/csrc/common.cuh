@@ -40,6 +40,7 @@ struct RahtPlan {
   uint32_t nphases;
   uint32_t overflow;                  // the schedule did not fit the scratch, or `invalid`: the transform kernels write nothing
   uint32_t invalid;                   // voxel codes not sorted and unique, or a zero leaf weight
+  uint32_t has_long;                  // fused merge: some voxel holds >= kLongRun Gaussians (merge_long.cuh)
   uint32_t M[kRahtMaxPhases + 2];     // active entries of phase p (1-based); M[1] = N_v
   uint32_t poff[kRahtMaxPhases + 2];  // row offset of phase p (p >= 2) in the idx / pending-row pools
   uint32_t toff[kRahtMaxPhases + 2];  // tile-header offset of phase p (records start at toff * kRahtTile)
@@ -96,6 +97,7 @@ struct gsnfs_ctx {
   uint4* raht_pend;        // pending entries {code, first voxel, node weight}, tile strided (raht_hdr_cap x 128)
   uint32_t* raht_bsum;     // pending counts summed per 256 tiles
   uint32_t* raht_gsrc;     // fused merge: first Gaussian of every voxel
+  double* merge_partial;   // long-run merge: 2 x ceil(max_points / 256) x max_channels chunk partial sums (merge_long.cuh)
   uint32_t raht_bsum_cap;
   uint4* raht_rec;         // merge records
   gsnfs::RahtTileHdr* raht_hdr;

@@ -4,9 +4,22 @@
 // is a straight 16-byte-vector row copy, so the kernel is a 2 x 4C bytes/voxel HBM stream.
 #include <type_traits>
 
-#include "common.cuh"
+#include "merge_long.cuh"
 
 namespace gsnfs {
+
+// Pre-pass of the long runs (merge_long.cuh): one 16-lane group per chunk of sorted positions.  Without long runs (every
+// frame of the timed configs) a chunk costs two binary searches.
+template <int VEC>
+__global__ void __launch_bounds__(256) merge_long_kernel(const float* __restrict__ attr, int C, const uint32_t* __restrict__ perm,
+                                                         const uint32_t* __restrict__ vstart,
+                                                         const gsnfs_counts* __restrict__ counts, uint32_t nchunks,
+                                                         double* __restrict__ partial) {
+  const uint32_t nv = counts->n_voxels;
+  if (nv == 0) return;
+  for (uint32_t chunk = blockIdx.x * 16 + threadIdx.y; chunk < nchunks; chunk += gridDim.x * 16)
+    long_chunk_partials<VEC>(attr, C, perm, vstart, nv, chunk, partial, (int)threadIdx.x, 16);
+}
 
 // VEC = 4: channels % 4 == 0, rows moved as float4 (rows are then 16-byte aligned);  VEC = 1: any C.
 // Layout: threadIdx.x = vector lane inside a row (16 lanes), threadIdx.y = row slot; each thread keeps
@@ -16,6 +29,7 @@ __global__ void __launch_bounds__(256) merge_kernel(const float* __restrict__ at
                                                     const uint32_t* __restrict__ perm,
                                                     const uint32_t* __restrict__ vstart,
                                                     const gsnfs_counts* __restrict__ counts,
+                                                    const double* __restrict__ partial,
                                                     float* __restrict__ merged, uint32_t* __restrict__ weights) {
   using VecT = typename std::conditional<VEC == 4, float4, float>::type;
   const uint32_t nv = counts->n_voxels;
@@ -42,7 +56,13 @@ __global__ void __launch_bounds__(256) merge_kernel(const float* __restrict__ at
         const uint32_t v = r0 + threadIdx.y + 16 * k;
         if (e[k] <= s[k]) continue;
         const uint32_t cnt = e[k] - s[k];
-        if (cnt > 1) {                           // rare: fp64 accumulation in sorted order, then mean
+        if (cnt >= kLongRun) {                   // long run: chunk partials left by merge_long_kernel, in chunk order
+          double a[VEC];
+          long_run_sum<VEC>(partial, C, s[k], e[k], c, a);
+          const double inv = (double)cnt;
+          if constexpr (VEC == 4) x[k] = make_float4((float)(a[0] / inv), (float)(a[1] / inv), (float)(a[2] / inv), (float)(a[3] / inv));
+          else x[k] = (float)(a[0] / inv);
+        } else if (cnt > 1) {                    // rare: fp64 accumulation in sorted order, then mean
           if constexpr (VEC == 4) {
             double a0 = x[k].x, a1 = x[k].y, a2 = x[k].z, a3 = x[k].w;
             uint32_t q = s[k] + 1;
@@ -90,11 +110,21 @@ int run_voxel_merge(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, int ch
   const uint32_t blocks_needed = (n + 16 * ROWS - 1) / (16 * ROWS);
   const uint32_t gcap = (uint32_t)ctx->num_sms * 32u;
   const int grid = (int)(blocks_needed < gcap ? blocks_needed : gcap);
+  const uint32_t nchunks = (n + kLongChunk - 1) / kLongChunk;
+  const int lgrid = (int)min((nchunks + 15u) / 16u, (uint32_t)ctx->num_sms * 8u);
+  GSNFS_KERNEL(ctx, st, "merge_long");
+  if (channels % 4 == 0)
+    merge_long_kernel<4><<<lgrid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, nchunks, ctx->merge_partial);
+  else
+    merge_long_kernel<1><<<lgrid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, nchunks, ctx->merge_partial);
+  GSNFS_LAUNCH_CHECK(ctx, st);
   GSNFS_KERNEL(ctx, st, "merge");
   if (channels % 4 == 0)
-    merge_kernel<4, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, d_merged, d_weights);
+    merge_kernel<4, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, ctx->merge_partial, d_merged,
+                                                  d_weights);
   else
-    merge_kernel<1, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, d_merged, d_weights);
+    merge_kernel<1, ROWS><<<grid, block, 0, st>>>(d_attr, channels, d_perm, d_voxel_start, d_counts, ctx->merge_partial, d_merged,
+                                                  d_weights);
   GSNFS_LAUNCH_CHECK(ctx, st);
   return GSNFS_OK;
 }

@@ -17,6 +17,7 @@
 // cooperative kernel -- the paper's "prelude" -- and is shared by the forward and the inverse transform.
 #include <cooperative_groups.h>
 
+#include "merge_long.cuh"
 #include "raht_math.cuh"
 
 namespace cg = cooperative_groups;
@@ -69,6 +70,7 @@ struct GatherArgs {          // fused merge: rows of phase 1 are gathered throug
   const uint32_t* gsrc;      // NULL => rows are contiguous
   const uint32_t* perm;
   const uint32_t* vstart;
+  double* partial;           // chunk partial sums of the long runs (merge_long.cuh)
 };
 
 template <int VEC>
@@ -104,6 +106,14 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
   if (!has_q) out_q = nullptr;
   const uint32_t nph = plan->nphases;
   if (plan->overflow) return;                                           // uniform: no grid.sync mismatch
+  if (ga.gsrc && plan->has_long) {       // fused merge with long duplicate runs: chunk partial sums by the whole grid first
+    const uint32_t nv = plan->M[1];
+    const uint32_t nchunks = (ga.vstart[nv] + kLongChunk - 1) / kLongChunk;
+    for (uint32_t chunk = blockIdx.x * nhw + hw; chunk < nchunks; chunk += gridDim.x * nhw)
+      long_chunk_partials<VEC>(attr_in, C, ga.perm, ga.vstart, nv, chunk, ga.partial, l16, lpr);
+    __threadfence();
+    grid.sync();
+  }
   for (uint32_t p = 1; p <= nph; ++p) {
     const uint32_t M = plan->M[p], Mnext = plan->M[p + 1];
     const uint32_t ntiles = (M + T - 1) / T, toff = plan->toff[p];
@@ -165,7 +175,13 @@ __global__ void __launch_bounds__(kXT, 3) raht_forward_kernel(
             if (gsrc) {      // duplicate voxel: mean of its Gaussians, fp64 accumulation in sorted order [O9]
               const uint32_t s0 = ga.vstart[ks + k];
               for (int c = l16; c < cv; c += lpr) {
-                if constexpr (VEC == 4) {
+                if (w >= kLongRun) {
+                  double a[VEC];
+                  long_run_sum<VEC>(ga.partial, C, s0, s0 + w, c, a);
+                  const double dw = (double)w;
+                  if constexpr (VEC == 4) r[c] = make_float4((float)(a[0] / dw), (float)(a[1] / dw), (float)(a[2] / dw), (float)(a[3] / dw));
+                  else r[c] = (float)(a[0] / dw);
+                } else if constexpr (VEC == 4) {
                   const float4 x = r[c];
                   double a0 = x.x, a1 = x.y, a2 = x.z, a3 = x.w;
                   uint32_t q = 1;
@@ -490,7 +506,7 @@ int run_raht(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const uint64_t* d_ke
   sp.perm = d_perm; sp.vstart = d_vstart; sp.gsrc = ctx->raht_gsrc; sp.weights_out = d_weights_out;
   if (fused) d_weights = d_weights_out;        // the transform kernels read the run lengths the schedule writes
   GatherArgs ga;
-  ga.gsrc = fused ? ctx->raht_gsrc : nullptr; ga.perm = d_perm; ga.vstart = d_vstart;
+  ga.gsrc = fused ? ctx->raht_gsrc : nullptr; ga.perm = d_perm; ga.vstart = d_vstart; ga.partial = ctx->merge_partial;
   if (d_keys) {                                  // NULL: the schedule of the previous call on this context is reused
     int rc = launch_raht_schedule(ctx, st, d_keys, d_weights, n_voxels, d_counts, sp);
     if (rc != GSNFS_OK) return rc;

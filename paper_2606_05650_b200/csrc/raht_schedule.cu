@@ -24,6 +24,7 @@
 #include <cooperative_groups.h>
 #include <cstddef>
 
+#include "merge_long.cuh"
 #include "raht.cuh"
 
 namespace cg = cooperative_groups;
@@ -162,6 +163,7 @@ __global__ void __launch_bounds__(256) raht_schedule_kernel(
           mk = pf_key;
           if (sp.perm) {
             went = pf_b - pf_a;
+            if (went >= kLongRun) plan->has_long = 1u;        // the forward kernel runs the chunk pre-pass first
             sp.gsrc[vidx] = sp.perm[pf_a];
             sp.weights_out[vidx] = went;
           } else {
@@ -428,7 +430,7 @@ int launch_raht_schedule(gsnfs_ctx* ctx, cudaStream_t st, const uint64_t* d_keys
                          uint32_t n_voxels, gsnfs_counts* d_counts, const SchedPools& sp_in) {
   SchedPools sp = sp_in;
   GSNFS_CUDA_OK(ctx, cudaMemsetAsync(ctx->raht_bsum, 0, sizeof(uint32_t) * ctx->raht_bsum_cap, st));
-  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(&ctx->raht_plan->overflow, 0, 2 * sizeof(uint32_t), st));   // overflow, invalid
+  GSNFS_CUDA_OK(ctx, cudaMemsetAsync(&ctx->raht_plan->overflow, 0, 3 * sizeof(uint32_t), st));   // overflow, invalid, has_long
   int per_sm = ctx->occ_cache[0];
   if (per_sm == 0) {
     GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, raht_schedule_kernel, 256, 0));

@@ -80,16 +80,19 @@ def rel_l2(got, ref):
     return num / den
 
 
-def check_quantised(q_gpu, q_ref):
+def check_quantised(q_gpu, q_ref, allow=0):
+    """>= 99.99 % identical, the rest off by exactly one.  `allow`: absolute number of +-1 differences tolerated when the
+    tensor is too small for the fraction to mean anything (frames of <= 512 voxels holding thousands of Gaussians each:
+    |q| reaches 5e4 bins there, where one fp32 ulp of the coefficient is already 0.003 bins)."""
     diff = q_gpu.astype(np.int64) - q_ref
     nz = diff != 0
     frac = nz.mean() if diff.size else 0.0
-    assert frac <= 1e-4, f"{frac:.3e} of quantised coefficients differ"
+    assert frac <= 1e-4 or nz.sum() <= allow, f"{frac:.3e} of quantised coefficients differ"
     assert np.all(np.abs(diff[nz]) == 1)
     return frac
 
 
-def full_pipeline_check(B, ctx, fr, dz=None, check_decode=True):
+def full_pipeline_check(B, ctx, fr, dz=None, check_decode=True, allow=0):
     ref = orc.encode_frame(fr.xyz, fr.attr, fr.bbox_min, fr.bbox_max, fr.depth, fr.qstep,
                            dz_round=orc.DZ_ROUND_DEFAULT if dz is None else float(np.float32(dz)))
     buf, got = gpu_position_encode(B, ctx, fr)
@@ -114,7 +117,7 @@ def full_pipeline_check(B, ctx, fr, dz=None, check_decode=True):
     q = buf.qcoeff[:nv].cpu().numpy()
     err = rel_l2(Y, ref["coeff"])
     assert err.max() <= 1e-5, f"coefficient rel L2 {err.max():.3e}"
-    frac = check_quantised(q, ref["qcoeff"])
+    frac = check_quantised(q, ref["qcoeff"], allow)
     if not check_decode:
         return frac
     # decode: position stream from the GPU encoder (bit-exact to the oracle's), coefficients = the ORACLE's
@@ -150,6 +153,13 @@ def test_config2_full_pipeline(B, ctx_small):
 def test_dense_duplicates(B, ctx_small, n, depth, channels):
     # heavy duplicate merging, weights up to hundreds, vector (C%4==0) and scalar channel paths
     full_pipeline_check(B, ctx_small, synth.make_dense_frame(n=n, depth=depth, channels=channels, seed=n))
+
+
+@pytest.mark.parametrize("n,depth,channels", [(40_000, 2, 56), (30_000, 1, 7), (60_000, 3, 12), (10_000, 1, 3), (100_000, 4, 56)])
+def test_long_duplicate_runs(B, ctx_small, n, depth, channels):
+    # hundreds to thousands of Gaussians per voxel: the chunk-wise sums of merge_long.cuh (runs that cross many chunks of
+    # 256 sorted positions, shorter runs that start and end inside a chunk next to them), vector and scalar channel paths
+    full_pipeline_check(B, ctx_small, synth.make_dense_frame(n=n, depth=depth, channels=channels, seed=n), allow=3)
 
 
 @pytest.mark.parametrize("dz", [0.0, 0.5])
@@ -231,9 +241,11 @@ def test_unit_weights_paper_mode(B, ctx_small):
     assert np.all(np.abs(back.cpu().numpy() - ref["merged"]) <= 1e-4 * rng_c)     # perfect reconstruction
 
 
-@pytest.mark.parametrize("maker", ["config1", "dense56", "dense7", "dense12"])
+@pytest.mark.parametrize("maker", ["config1", "dense56", "dense7", "dense12", "long56", "long7"])
 def test_fused_merge_forward_equals_separate_calls(B, ctx_small, maker):
     fr = {"config1": lambda: synth.make_frame(1),
+          "long56": lambda: synth.make_dense_frame(n=40_000, depth=2, channels=56, seed=6),      # runs of >= 256 rows:
+          "long7": lambda: synth.make_dense_frame(n=30_000, depth=1, channels=7, seed=7),        # chunk-wise sums
           "dense56": lambda: synth.make_dense_frame(n=20_000, depth=5, channels=56, seed=3),
           "dense7": lambda: synth.make_dense_frame(n=3_000, depth=4, channels=7, seed=4),
           "dense12": lambda: synth.make_dense_frame(n=30_000, depth=6, channels=12, seed=5)}[maker]()

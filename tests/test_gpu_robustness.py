@@ -67,10 +67,11 @@ def run_all(B, ctx, fr, g):
     return nv, ob, sb, pb
 
 
-@pytest.mark.parametrize("maker", ["config1", "dense", "pointcloud_small"])
+@pytest.mark.parametrize("maker", ["config1", "dense", "pointcloud_small", "long_runs"])
 def test_repeatable_and_in_bounds(B, maker):
     fr = {"config1": lambda: synth.make_frame(1), "dense": lambda: synth.make_dense_frame(20_000, 5, 56, seed=9),
-          "pointcloud_small": lambda: synth.make_pointcloud_frame(n=60_000, depth=8)}[maker]()
+          "pointcloud_small": lambda: synth.make_pointcloud_frame(n=60_000, depth=8),
+          "long_runs": lambda: synth.make_dense_frame(50_000, 2, 56, seed=11)}[maker]()     # chunk-wise merge pre-pass
     n, C, J = fr.n, fr.channels, fr.depth
     ctx = B.Context(max_points=n, max_channels=max(C, 4), max_depth=J)
     try:
