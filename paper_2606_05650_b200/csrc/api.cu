@@ -132,7 +132,7 @@ static int create_impl(gsnfs_ctx* c) {
   c->rans_blocks_cap = c->occ_cap / GSNFS_RANS_BLOCK + 64;
   const size_t o_rah = b.take(256 * 4), o_ras = b.take(c->rans_blocks_cap * GSNFS_RANS_BLOCK * 2);
   const size_t o_rast = b.take(c->rans_blocks_cap * 4), o_rao = b.take((c->rans_blocks_cap + 1) * 8);
-  c->color_parts_cap = (uint32_t)c->num_sms * 2u;
+  c->color_parts_cap = (uint32_t)c->num_sms * 4u;
   const size_t o_colp = b.take((size_t)c->color_parts_cap * 3 * 135 * sizeof(double));
   c->rlgr_off_cap = (N / GSNFS_RLGR_MIN_BLOCK + 1) * (uint64_t)C + 1;
   c->rlgr_rows_cap = N / GSNFS_RLGR_MIN_BLOCK + 2;

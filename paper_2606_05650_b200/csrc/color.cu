@@ -5,10 +5,11 @@
 // component positive; y = (x - mu) E).
 //
 // The paper does this with PyTorch matmuls.  Here: one streaming pass accumulates the 3 x (K + K(K+1)/2) first and second
-// moments in fp64 (one thread per moment, rows staged through shared memory, per-CTA partials reduced in a fixed order so
-// the fit is deterministic); one warp per YUV channel then diagonalises its K x K covariance with cyclic Jacobi
-// rotations in fp64; the transform itself is one streaming pass (a row tile in shared memory, one thread per output
-// element, K multiply-adds each).
+// moments in fp64 (one thread per moment, rows staged through shared memory with cp.async, two tiles in flight, per-CTA
+// partials reduced in a fixed order so the fit is deterministic); one warp per YUV channel then diagonalises its K x K
+// covariance with cyclic Jacobi rotations in fp64; the transform itself is one streaming pass (row tiles double buffered
+// in shared memory; one thread per (row, YUV channel) keeps the K inputs in registers and reads the basis as broadcast
+// 16-byte vectors: K + K*K/4 shared-memory loads for K*K multiply-adds, where one thread per output element needed 3 K*K).
 #include "common.cuh"
 
 namespace gsnfs {
@@ -39,19 +40,40 @@ __device__ __forceinline__ void mat3(float* r, int i0, int i1, int i2, const flo
   r[i2] = fmaf(m[6], a, fmaf(m[7], b, m[8] * c));
 }
 
-// Stage `cnt` rows (C floats each) of a row-major tensor into shared memory, coalesced.
-__device__ __forceinline__ void stage_rows(float* s, const float* g, uint32_t cnt, int C) {
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(a), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async16(void* smem_dst, const void* gmem_src) {
+  const unsigned a = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(a), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
+
+// Stage `cnt` rows (C floats each, contiguous in global memory) into shared memory with row pitch `pitch` floats,
+// asynchronously.  pitch == C and a 16-byte aligned source: 16-byte copies; otherwise element-wise.
+__device__ __forceinline__ void stage_rows_async(float* s, int pitch, const float* g, uint32_t cnt, int C) {
   const uint32_t tot = cnt * (uint32_t)C;
-  for (uint32_t i = threadIdx.x; i < tot; i += blockDim.x) s[i] = g[i];
+  if (pitch == C && ((tot | (uint32_t)C) & 3u) == 0u && (reinterpret_cast<uintptr_t>(g) & 15u) == 0u) {
+    for (uint32_t i = threadIdx.x; i < tot / 4; i += blockDim.x) cp_async16(s + 4 * i, g + 4 * i);
+  } else {
+    for (uint32_t i = threadIdx.x; i < tot; i += blockDim.x) {
+      const uint32_t r = i / (uint32_t)C, c = i - r * (uint32_t)C;
+      cp_async4(s + (size_t)r * pitch + c, g + i);
+    }
+  }
 }
 
 // ---- 1. moments of the YUV-converted SH AC coefficients -------------------------------------------------------------
 __global__ void __launch_bounds__(448) color_stats_kernel(const float* __restrict__ attr, uint32_t n_host,
                                                           const uint32_t* __restrict__ n_dev, int C,
                                                           double* __restrict__ partial /* gridDim.x x 3 x kMomMax */) {
-  extern __shared__ float s_rows[];                      // kColRows x C
+  extern __shared__ __align__(16) float s_rows[];        // 2 x kColRows x C floats, then kColRows x 3K doubles (YUV AC)
   const uint32_t n = n_dev ? min(*n_dev, n_host) : n_host;
   const int K = (C - 11) / 3;
+  const int W = 3 * K;
+  double* s_d = reinterpret_cast<double*>(s_rows + 2 * kColRows * C);
   const int nmom = K + K * (K + 1) / 2;
   // thread -> (YUV channel c, moment m): m < K: sum of component m; else the pair (i, j), i <= j
   const int t = threadIdx.x;
@@ -65,46 +87,92 @@ __global__ void __launch_bounds__(448) color_stats_kernel(const float* __restric
   } else if (c < 3) {
     pi = m;
   }
-  const int base = 11 + K * c;
   double acc = 0.0;
-  for (uint32_t r0 = blockIdx.x * kColRows; r0 < n; r0 += gridDim.x * kColRows) {
+  const uint32_t stride = gridDim.x * kColRows;
+  uint32_t r0 = blockIdx.x * kColRows;
+  int cur = 0;
+  if (r0 < n) stage_rows_async(s_rows, C, attr + (size_t)r0 * C, min((uint32_t)kColRows, n - r0), C);
+  cp_async_commit();
+  for (; r0 < n; r0 += stride) {
     const uint32_t cnt = min((uint32_t)kColRows, n - r0);
-    __syncthreads();
-    stage_rows(s_rows, attr + (size_t)r0 * C, cnt, C);
-    __syncthreads();
-    for (uint32_t i = t; i < cnt * (uint32_t)K; i += blockDim.x) {      // AC triples -> YUV
+    const float* rows = s_rows + (size_t)cur * kColRows * C;
+    const uint32_t rn = r0 + stride;
+    if (rn < n) stage_rows_async(s_rows + (size_t)(cur ^ 1) * kColRows * C, C, attr + (size_t)rn * C, min((uint32_t)kColRows, n - rn), C);
+    cp_async_commit();
+    cp_async_wait<1>();
+    __syncthreads();                                      // rows(cur) landed; the previous tile's moments are done with s_d
+    // AC triples -> YUV, widened to fp64 once.  Rows are stored in pairs, s_d[(r / 2) * W + col] = {row r, row r + 1}, so
+    // that the moment loop below fetches two rows per 16-byte load (it is bound by shared-memory wavefronts)
+    const uint32_t cnt2 = (cnt + 1u) & ~1u;
+    for (uint32_t i = t; i < cnt2 * (uint32_t)K; i += blockDim.x) {
       const uint32_t r = i / K, j = i - r * K;
-      mat3(s_rows + (size_t)r * C, 11 + j, 11 + K + j, 11 + 2 * K + j, c_yuv);
+      double y = 0.0, u = 0.0, v = 0.0;
+      if (r < cnt) {
+        const float* row = rows + (size_t)r * C + 11 + j;
+        const float a = row[0], b = row[K], g = row[2 * K];
+        y = (double)fmaf(c_yuv[0], a, fmaf(c_yuv[1], b, c_yuv[2] * g));
+        u = (double)fmaf(c_yuv[3], a, fmaf(c_yuv[4], b, c_yuv[5] * g));
+        v = (double)fmaf(c_yuv[6], a, fmaf(c_yuv[7], b, c_yuv[8] * g));
+      }
+      double* d = s_d + ((size_t)(r >> 1) * W + j) * 2 + (r & 1u);
+      d[0] = y; d[2 * K] = u; d[4 * K] = v;
     }
     __syncthreads();
     if (c < 3) {
-      if (pj < 0) for (uint32_t r = 0; r < cnt; ++r) acc += (double)s_rows[(size_t)r * C + base + pi];
-      else for (uint32_t r = 0; r < cnt; ++r) acc += (double)s_rows[(size_t)r * C + base + pi] * (double)s_rows[(size_t)r * C + base + pj];
+      const double2* a = reinterpret_cast<const double2*>(s_d) + K * c + pi;
+      if (pj < 0) {
+#pragma unroll 8
+        for (uint32_t r = 0; r < cnt2 / 2; ++r) { const double2 x = a[(size_t)r * W]; acc += x.x; acc += x.y; }
+      } else {
+        const double2* b = reinterpret_cast<const double2*>(s_d) + K * c + pj;
+#pragma unroll 8
+        for (uint32_t r = 0; r < cnt2 / 2; ++r) {
+          const double2 x = a[(size_t)r * W], y = b[(size_t)r * W];
+          acc = fma(x.x, y.x, acc);
+          acc = fma(x.y, y.y, acc);
+        }
+      }
     }
+    cur ^= 1;
   }
+  cp_async_wait<0>();
   if (c < 3) partial[((size_t)blockIdx.x * 3 + c) * kMomMax + m] = acc;
 }
 
 // ---- 2. three K x K eigen-decompositions (cyclic Jacobi, fp64), one warp each ----------------------------------------
-__global__ void __launch_bounds__(96) klt_eig_kernel(const double* __restrict__ partial, int nparts, uint32_t n_host,
-                                                     const uint32_t* __restrict__ n_dev, int C, float* __restrict__ klt) {
-  __shared__ double s_S[3][kKMax][kKMax + 1];
-  __shared__ double s_V[3][kKMax][kKMax + 1];
+// The partials are reduced by one thread per moment in a fixed order.  A sweep applies its K(K-1)/2 rotations in K - 1
+// (K even) or K (K odd) rounds of disjoint pairs (round-robin pairing: the rotations of a round commute, so they are
+// computed together -- one lane per pair -- and applied together, lanes = rows, then lanes = columns): 15 dependent
+// steps per sweep at K = 15 instead of 105.
+constexpr int kEigThreads = 416;             // >= 3 * kMomMax
+
+__global__ void __launch_bounds__(kEigThreads) klt_eig_kernel(const double* __restrict__ partial, int nparts, uint32_t n_host,
+                                                              const uint32_t* __restrict__ n_dev, int C, float* __restrict__ klt) {
+  __shared__ double s_S[3][kKMax][kKMax + 2];             // row pitch 17 doubles: a column walk hits 16 different banks
+  __shared__ double s_V[3][kKMax][kKMax + 2];
   __shared__ double s_mom[3][kMomMax];
-  __shared__ double s_cs[3][2];
+  __shared__ double s_rot[3][(kKMax + 1) / 2][2];         // (cos, sin) of the round's rotations
+  __shared__ int s_pq[3][(kKMax + 1) / 2][2];
   __shared__ int s_ord[3][kKMax];
   const uint32_t n = n_dev ? min(*n_dev, n_host) : n_host;
   const KltLayout L = klt_layout(C);
   const int K = L.K, nmom = K + K * (K + 1) / 2;
-  const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  float* out = klt + (size_t)c * L.stride;
   if (K == 0) return;
-  for (int m = lane; m < nmom; m += 32) {                 // fixed-order reduction of the per-CTA partials
-    double a = 0.0;
-    for (int p = 0; p < nparts; ++p) a += partial[((size_t)p * 3 + c) * kMomMax + m];
-    s_mom[c][m] = a;
+  {
+    const int t = threadIdx.x;
+    if (t < 3 * nmom) {                                    // fixed-order reduction of the per-CTA partials
+      const int cc = t / nmom, m = t - cc * nmom;
+      const double* src = partial + (size_t)cc * kMomMax + m;
+      double a = 0.0;
+#pragma unroll 16
+      for (int p = 0; p < nparts; ++p) a += __ldg(src + (size_t)p * 3 * kMomMax);
+      s_mom[cc][m] = a;
+    }
   }
-  __syncwarp();
+  __syncthreads();
+  const int c = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  if (c >= 3) return;
+  float* out = klt + (size_t)c * L.stride;
   const double inv_n = n ? 1.0 / (double)n : 0.0;
   {
     int m = K;
@@ -117,6 +185,7 @@ __global__ void __launch_bounds__(96) klt_eig_kernel(const double* __restrict__ 
     for (int i = lane; i < K * K; i += 32) s_V[c][i / K][i % K] = (i / K == i % K) ? 1.0 : 0.0;
   }
   __syncwarp();
+  const int Kp = K + (K & 1), ring = Kp - 1, npair = Kp / 2;          // players 0 .. Kp-1 (player K is a bye when K is odd)
   for (int sweep = 0; sweep < 30; ++sweep) {
     double off = 0.0, dia = 0.0;
     for (int i = lane; i < K * K; i += 32) {
@@ -126,41 +195,55 @@ __global__ void __launch_bounds__(96) klt_eig_kernel(const double* __restrict__ 
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) { off += __shfl_xor_sync(0xffffffffu, off, o); dia += __shfl_xor_sync(0xffffffffu, dia, o); }
     if (off <= 1e-30 * dia || off == 0.0) break;
-    for (int p = 0; p < K - 1; ++p) {
-      for (int q = p + 1; q < K; ++q) {
-        if (lane == 0) {
+    for (int round = 0; round < ring; ++round) {
+      if (lane < npair) {                     // its pair of this round and the rotation that zeroes S[p][q]
+        const int a = lane == 0 ? Kp - 1 : (round + lane) % ring;
+        const int b = lane == 0 ? round : (round - lane + ring) % ring;
+        const int p = min(a, b), q = max(a, b);
+        double cs = 1.0, sn = 0.0;
+        if (q < K) {
           const double apq = s_S[c][p][q];
-          double cs = 1.0, sn = 0.0;
           if (apq != 0.0) {
             const double theta = (s_S[c][q][q] - s_S[c][p][p]) / (2.0 * apq);
             const double tt = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
             cs = 1.0 / sqrt(tt * tt + 1.0);
             sn = tt * cs;
           }
-          s_cs[c][0] = cs; s_cs[c][1] = sn;
         }
-        __syncwarp();
-        const double cs = s_cs[c][0], sn = s_cs[c][1];
-        if (sn != 0.0) {
-          if (lane < K) {                      // columns p, q of S and V:  [x_p, x_q] <- [c x_p - s x_q, s x_p + c x_q]
-            const double sp = s_S[c][lane][p], sq = s_S[c][lane][q];
-            s_S[c][lane][p] = cs * sp - sn * sq;
-            s_S[c][lane][q] = sn * sp + cs * sq;
-            const double vp = s_V[c][lane][p], vq = s_V[c][lane][q];
-            s_V[c][lane][p] = cs * vp - sn * vq;
-            s_V[c][lane][q] = sn * vp + cs * vq;
-          }
-          __syncwarp();
-          if (lane < K) {                      // rows p, q of S
-            const double sp = s_S[c][p][lane], sq = s_S[c][q][lane];
-            s_S[c][p][lane] = cs * sp - sn * sq;
-            s_S[c][q][lane] = sn * sp + cs * sq;
-          }
-          __syncwarp();
-          if (lane == 0) { s_S[c][p][q] = 0.0; s_S[c][q][p] = 0.0; }
-        }
-        __syncwarp();
+        s_pq[c][lane][0] = p; s_pq[c][lane][1] = q;
+        s_rot[c][lane][0] = cs; s_rot[c][lane][1] = sn;
       }
+      __syncwarp();
+      for (int idx = lane; idx < K * npair; idx += 32) {    // columns p, q of S and V:  [x_p, x_q] <- [c x_p - s x_q, s x_p + c x_q]
+        const int k = idx / K, i = idx - k * K;
+        const double ck = s_rot[c][k][0], sk = s_rot[c][k][1];
+        if (sk != 0.0) {
+          const int pk = s_pq[c][k][0], qk = s_pq[c][k][1];
+          const double sp = s_S[c][i][pk], sq = s_S[c][i][qk];
+          s_S[c][i][pk] = ck * sp - sk * sq;
+          s_S[c][i][qk] = sk * sp + ck * sq;
+          const double vp = s_V[c][i][pk], vq = s_V[c][i][qk];
+          s_V[c][i][pk] = ck * vp - sk * vq;
+          s_V[c][i][qk] = sk * vp + ck * vq;
+        }
+      }
+      __syncwarp();
+      for (int idx = lane; idx < K * npair; idx += 32) {    // rows p, q of S
+        const int k = idx / K, j = idx - k * K;
+        const double ck = s_rot[c][k][0], sk = s_rot[c][k][1];
+        if (sk != 0.0) {
+          const int pk = s_pq[c][k][0], qk = s_pq[c][k][1];
+          const double sp = s_S[c][pk][j], sq = s_S[c][qk][j];
+          s_S[c][pk][j] = ck * sp - sk * sq;
+          s_S[c][qk][j] = sk * sp + ck * sq;
+        }
+      }
+      __syncwarp();
+      if (lane < npair && s_rot[c][lane][1] != 0.0) {
+        const int p = s_pq[c][lane][0], q = s_pq[c][lane][1];
+        s_S[c][p][q] = 0.0; s_S[c][q][p] = 0.0;
+      }
+      __syncwarp();
     }
   }
   if (lane == 0) {                             // eigenvalues in descending order (stable selection)
@@ -187,15 +270,20 @@ __global__ void __launch_bounds__(96) klt_eig_kernel(const double* __restrict__ 
 }
 
 // ---- 3. the transform: RGB -> YUV on every SH function, (x - mu) E on the AC coefficients (or the inverse) -------------
+// Shared memory: two row tiles (filled by cp.async, transformed in place, copied out coalesced), odd row pitch, the
+// basis as [c][q][16] floats (row q of E_c, or of E_c^T for the inverse, padded to four 16-byte vectors) and the means.
+constexpr int kEP = 16;                      // padded basis row
+
 template <bool INV>
 __global__ void __launch_bounds__(256) color_apply_kernel(const float* __restrict__ in, uint32_t n_host,
                                                           const uint32_t* __restrict__ n_dev, int C,
                                                           const float* __restrict__ klt /* NULL: YUV only */,
                                                           float* __restrict__ out) {
-  extern __shared__ float s_dyn[];
-  float* s_rows = s_dyn;                                   // kColRows x C
-  float* s_tmp = s_rows + kColRows * C;                    // kColRows x C (transformed)
-  float* s_klt = s_tmp + kColRows * C;                     // 3 x stride
+  extern __shared__ __align__(16) float s_dyn[];
+  const int P = C | 1;                                     // odd row pitch: a warp's 32 rows fall into 32 different banks
+  float* s_in = s_dyn;                                     // 2 x kColRows x P; a tile is transformed in place
+  float* s_E = s_in + 2 * kColRows * P;                    // 3 x kKMax x kEP (16-byte aligned: kColRows % 4 == 0)
+  float* s_mu = s_E + 3 * kKMax * kEP;                     // 3 x kEP
   __shared__ float s_m[9];
   const uint32_t n = n_dev ? min(*n_dev, n_host) : n_host;
   const KltLayout L = klt_layout(C);
@@ -212,48 +300,83 @@ __global__ void __launch_bounds__(256) color_apply_kernel(const float* __restric
       s_m[t] = (float)((m[r1 * 3 + c1] * m[r2 * 3 + c2] - m[r1 * 3 + c2] * m[r2 * 3 + c1]) / det);
     }
   }
-  if (klt) for (int i = t; i < 3 * L.stride; i += blockDim.x) s_klt[i] = klt[i];
-  for (uint32_t r0 = blockIdx.x * kColRows; r0 < n; r0 += gridDim.x * kColRows) {
+  for (int i = t; i < 3 * kKMax * kEP + 3 * kEP; i += blockDim.x) s_E[i] = 0.f;      // s_E and s_mu are contiguous
+  __syncthreads();
+  if (klt) {
+    // forward: y_j = sum_q (x_q - mu_q) E[q][j]  -> row q holds E[q][.];  inverse: x_j = sum_q y_q E[j][q] + mu_j -> E^T
+    for (int i = t; i < 3 * K * K; i += blockDim.x) {
+      const int c = i / (K * K), rem = i - c * K * K, q = rem / K, j = rem - q * K;
+      const float* kc = klt + (size_t)c * L.stride + 2 * K;
+      s_E[(c * kKMax + q) * kEP + j] = INV ? kc[j * K + q] : kc[q * K + j];
+    }
+    for (int i = t; i < 3 * K; i += blockDim.x) s_mu[(i / K) * kEP + (i % K)] = klt[(size_t)(i / K) * L.stride + (i % K)];
+  }
+  const uint32_t stride = gridDim.x * kColRows;
+  uint32_t r0 = blockIdx.x * kColRows;
+  int cur = 0;
+  if (r0 < n) stage_rows_async(s_in, P, in + (size_t)r0 * C, min((uint32_t)kColRows, n - r0), C);
+  cp_async_commit();
+  for (; r0 < n; r0 += stride) {
     const uint32_t cnt = min((uint32_t)kColRows, n - r0);
-    __syncthreads();
-    stage_rows(s_rows, in + (size_t)r0 * C, cnt, C);
-    __syncthreads();
+    float* rows = s_in + (size_t)cur * kColRows * P;
+    const uint32_t rn = r0 + stride;
+    if (rn < n) stage_rows_async(s_in + (size_t)(cur ^ 1) * kColRows * P, P, in + (size_t)rn * C, min((uint32_t)kColRows, n - rn), C);
+    cp_async_commit();
+    cp_async_wait<1>();
+    __syncthreads();                                       // rows(cur) landed; the previous tile's copy-out is complete
     if (!INV) {
       for (uint32_t i = t; i < cnt * (uint32_t)(K + 1); i += blockDim.x) {       // every SH function -> YUV
-        const uint32_t r = i / (K + 1), j = i - r * (K + 1);
-        float* row = s_rows + (size_t)r * C;
+        const uint32_t r = (K == 15) ? (i >> 4) : i / (K + 1), j = i - r * (K + 1);
+        float* row = rows + (size_t)r * P;
         if (j == 0) mat3(row, 8, 9, 10, s_m); else mat3(row, 11 + (j - 1), 11 + K + (j - 1), 11 + 2 * K + (j - 1), s_m);
       }
       __syncthreads();
     }
-    // one thread per output element; AC element (c, j): sum_i (x_i - mu_i) E[i][j]  (inverse: sum_i y_i E[j][i] + mu_j)
-    for (uint32_t i = t; i < cnt * (uint32_t)C; i += blockDim.x) {
-      const uint32_t r = i / C, ch = i - r * C;
-      const float* row = s_rows + (size_t)r * C;
-      float v = row[ch];
-      if (klt && ch >= 11) {
-        const int c = (int)(ch - 11) / K, j = (int)(ch - 11) - c * K;
-        const float* kc = s_klt + c * L.stride;
-        const float* x = row + 11 + c * K;
-        float acc = 0.f;
-        if (!INV) for (int q = 0; q < K; ++q) acc = fmaf(x[q] - kc[q], kc[2 * K + q * K + j], acc);
-        else { for (int q = 0; q < K; ++q) acc = fmaf(x[q], kc[2 * K + j * K + q], acc); acc += kc[j]; }
-        v = acc;
+    // one thread per (row, YUV channel); the threads of a warp share the channel, so the basis loads are broadcasts
+    if (klt) {
+      for (uint32_t i = t; i < 3u * kColRows; i += blockDim.x) {
+        const uint32_t c = i / kColRows, r = i - c * kColRows;
+        if (r >= cnt) continue;
+        const float* x = rows + (size_t)r * P + 11 + c * K;
+        float* y = rows + (size_t)r * P + 11 + c * K;         // in place: this thread has read all of x by then
+        const float* E = s_E + c * kKMax * kEP;
+        const float* mu = s_mu + c * kEP;
+        float acc[kEP];
+#pragma unroll
+        for (int j = 0; j < kEP; ++j) acc[j] = 0.f;
+#pragma unroll
+        for (int q = 0; q < kKMax; ++q) {
+          if (q < K) {
+            const float xv = INV ? x[q] : x[q] - mu[q];
+            const float4* e4 = reinterpret_cast<const float4*>(E + q * kEP);
+#pragma unroll
+            for (int v = 0; v < kEP / 4; ++v) {
+              const float4 e = e4[v];
+              acc[4 * v + 0] = fmaf(xv, e.x, acc[4 * v + 0]); acc[4 * v + 1] = fmaf(xv, e.y, acc[4 * v + 1]);
+              acc[4 * v + 2] = fmaf(xv, e.z, acc[4 * v + 2]); acc[4 * v + 3] = fmaf(xv, e.w, acc[4 * v + 3]);
+            }
+          }
+        }
+#pragma unroll
+        for (int j = 0; j < kKMax; ++j) if (j < K) y[j] = INV ? acc[j] + mu[j] : acc[j];
       }
-      s_tmp[i] = v;
     }
     __syncthreads();
     if (INV) {
       for (uint32_t i = t; i < cnt * (uint32_t)(K + 1); i += blockDim.x) {       // every SH function back to RGB
-        const uint32_t r = i / (K + 1), j = i - r * (K + 1);
-        float* row = s_tmp + (size_t)r * C;
+        const uint32_t r = (K == 15) ? (i >> 4) : i / (K + 1), j = i - r * (K + 1);
+        float* row = rows + (size_t)r * P;
         if (j == 0) mat3(row, 8, 9, 10, s_m); else mat3(row, 11 + (j - 1), 11 + K + (j - 1), 11 + 2 * K + (j - 1), s_m);
       }
       __syncthreads();
     }
     float* g = out + (size_t)r0 * C;
-    for (uint32_t i = t; i < cnt * (uint32_t)C; i += blockDim.x) g[i] = s_tmp[i];
+    for (uint32_t r = t >> 5; r < cnt; r += blockDim.x >> 5)                      // a warp per row: coalesced, no division
+      for (int ch = t & 31; ch < C; ch += 32) g[(size_t)r * C + ch] = rows[(size_t)r * P + ch];
+    __syncthreads();                                       // the next iteration's prefetch refills this buffer
+    cur ^= 1;
   }
+  cp_async_wait<0>();
 }
 
 }  // namespace
@@ -267,12 +390,12 @@ int run_klt_fit(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, uint32_t n
   const int threads = (3 * nmom + 31) & ~31;
   const int grid = (int)min((uint32_t)ctx->color_parts_cap, (n + kColRows - 1) / kColRows);
   if (grid < 1) return GSNFS_OK;
-  const size_t smem = sizeof(float) * kColRows * channels;
+  const size_t smem = sizeof(float) * 2 * kColRows * channels + sizeof(double) * kColRows * 3 * K;
   GSNFS_KERNEL(ctx, st, "color_stats");
   color_stats_kernel<<<grid, threads, smem, st>>>(d_attr, n, n_dev, channels, ctx->color_partial);
   GSNFS_LAUNCH_CHECK(ctx, st);
   GSNFS_KERNEL(ctx, st, "klt_eig");
-  klt_eig_kernel<<<1, 96, 0, st>>>(ctx->color_partial, grid, n, n_dev, channels, d_klt);
+  klt_eig_kernel<<<1, kEigThreads, 0, st>>>(ctx->color_partial, grid, n, n_dev, channels, d_klt);
   GSNFS_LAUNCH_CHECK(ctx, st);
   return GSNFS_OK;
 }
@@ -282,8 +405,9 @@ int run_color_apply(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const float* 
   if (n == 0) return GSNFS_OK;
   const uint32_t* n_dev = d_counts ? &d_counts->n_voxels : nullptr;
   const KltLayout L = klt_layout(channels);
-  const size_t smem = sizeof(float) * (2 * kColRows * channels + 3 * L.stride);
-  const int grid = (int)min((uint32_t)ctx->num_sms * 4u, (n + kColRows - 1) / kColRows);
+  (void)L;
+  const size_t smem = sizeof(float) * (2 * kColRows * (channels | 1) + 3 * kKMax * kEP + 3 * kEP);
+  const int grid = (int)min((uint32_t)ctx->num_sms * 6u, (n + kColRows - 1) / kColRows);
   GSNFS_KERNEL(ctx, st, inverse ? "color_inverse" : "color_forward");
   if (inverse) color_apply_kernel<true><<<grid, 256, smem, st>>>(d_in, n, n_dev, channels, d_klt, d_out);
   else color_apply_kernel<false><<<grid, 256, smem, st>>>(d_in, n, n_dev, channels, d_klt, d_out);
@@ -292,7 +416,9 @@ int run_color_apply(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const float* 
 }
 
 int color_setup(gsnfs_ctx* ctx) {
-  const int smem = (int)(sizeof(float) * (2 * kColRows * 56 + 3 * (30 + 225)));
+  const int smem = (int)(sizeof(float) * (2 * kColRows * 57 + 3 * kKMax * kEP + 3 * kEP));
+  GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(color_stats_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                          (int)(sizeof(float) * 2 * kColRows * 56 + sizeof(double) * kColRows * 3 * kKMax)));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(color_apply_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(color_apply_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   return GSNFS_OK;
