@@ -7,7 +7,9 @@ A "step" is one pass of the whole hot path over one frame: gsnfs_octree_encode -
 merge fused into the forward transform + quantiser) on the encoder side, the decoder's header read-back, then
 gsnfs_octree_decode -> gsnfs_raht_inverse.  `value` is whole-job Mgaussians/s with inputs resident in HBM; `e2e` is the
 same metric through the *_host_packed ABI calls with pinned host buffers (H2D/D2H inside the timed region; the
-coefficients cross PCIe as RLGR bytes), `e2e_raw` through the *_host calls (raw int32 coefficients).  `entropy` times
+coefficients cross PCIe as RLGR bytes) on a back-to-back frame stream (an encoder thread and a decoder thread, one context
+each; `e2e.serial`: one frame at a time on one context), `e2e_raw` through the *_host calls (raw int32 coefficients,
+one frame at a time).  `entropy` times
 the RLGR coder on the frame's quantised coefficients, outside the step.  `--config pc` is the
 point-cloud shaped workload (NEXT-4: 1M points, depth 10, 3 colour channels).
 Multi-GPU: frames are independent (intra-only codec) => replicas only, one frame stream per
@@ -393,10 +395,16 @@ def run_ours(args, rank, world, local_rank):
             torch.cuda.synchronize()
             ms_pp = (times[1] - times[0]) * 1e3 / kp
             ok_pp = bool(torch.equal(h_out2[:nv_e], h_out[:nv_e]))
-            e2e["pipelined"] = {"value": round(n / (ms_pp * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_pp, 4),
-                                "frames": kp, "same_output_as_serial": ok_pp,
-                                "how": "encoder thread + decoder thread, one context and stream each, three sets of pinned "
-                                       "host buffers in rotation; host wall clock over the timed frames (all calls are blocking)"}
+            # the headline end-to-end figure is the back-to-back frame stream (the codec's use-case, config 5 / PAPER.md
+            # L45-49); the one-frame-at-a-time loop above is kept beside it as "serial"
+            serial = {k: e2e[k] for k in ("value", "ms_per_step", "steps", "api")}
+            serial["how"] = "encode then decode of one frame at a time on one context: the two PCIe directions never overlap"
+            e2e.update({"value": round(n / (ms_pp * 1e-3) / 1e6, 3), "ms_per_step": round(ms_pp, 4), "steps": kp,
+                        "same_output_as_serial": ok_pp, "serial": serial,
+                        "how": "back-to-back frames: an encoder thread and a decoder thread, one context and stream each, "
+                               "three sets of pinned host buffers in rotation, every frame's inputs copied host -> device "
+                               "and its results device -> host inside the timed region; host wall clock over the timed "
+                               "frames (all calls are blocking)"})
             ctx2.close()
         ms_r, ks = time_e2e(raw_step)
         e2e_raw = {"value": round(world * n / (ms_r * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_r, 4),
