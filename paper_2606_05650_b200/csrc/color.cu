@@ -66,28 +66,33 @@ __device__ __forceinline__ void stage_rows_async(float* s, int pitch, const floa
 }
 
 // ---- 1. moments of the YUV-converted SH AC coefficients -------------------------------------------------------------
-__global__ void __launch_bounds__(448) color_stats_kernel(const float* __restrict__ attr, uint32_t n_host,
-                                                          const uint32_t* __restrict__ n_dev, int C,
-                                                          double* __restrict__ partial /* gridDim.x x 3 x kMomMax */) {
-  extern __shared__ __align__(16) float s_rows[];        // 2 x kColRows x C floats, then kColRows x 3K doubles (YUV AC)
+// Second moments as 4 x 4 outer-product blocks: the K <= 15 components of a YUV channel are padded to 16 = four blocks of
+// four; a thread owns one of the ten block pairs (bi <= bj) of one channel and one of eight row groups, and keeps the 16
+// products (+ the 4 sums, on diagonal blocks) in registers: 8 shared-memory loads feed 32 fp64 FMAs per pair of rows,
+// where one thread per moment needed 32 loads for them (that version kept the shared-memory pipe 92 % busy).  The row
+// groups' accumulators are combined in a fixed order at the end, so the fit stays deterministic.
+constexpr int kStatThreads = 256;            // 240 used: 3 channels x 10 block pairs x 8 row groups
+constexpr int kStatW = 49;                   // double2 per row pair (3 x 16 columns + 1: odd pitch, conflict-free row groups)
+constexpr int kStatAcc = 20;                 // 16 products + 4 sums
+
+__global__ void __launch_bounds__(kStatThreads) color_stats_kernel(const float* __restrict__ attr, uint32_t n_host,
+                                                                   const uint32_t* __restrict__ n_dev, int C,
+                                                                   double* __restrict__ partial /* gridDim.x x 3 x kMomMax */) {
+  extern __shared__ __align__(16) float s_rows[];        // 2 x kColRows x C floats, then (kColRows / 2) x kStatW double2
   const uint32_t n = n_dev ? min(*n_dev, n_host) : n_host;
   const int K = (C - 11) / 3;
-  const int W = 3 * K;
-  double* s_d = reinterpret_cast<double*>(s_rows + 2 * kColRows * C);
-  const int nmom = K + K * (K + 1) / 2;
-  // thread -> (YUV channel c, moment m): m < K: sum of component m; else the pair (i, j), i <= j
+  double2* s_d = reinterpret_cast<double2*>(s_rows + 2 * kColRows * C);       // [row pair][column] = {row 2rp, row 2rp + 1}
   const int t = threadIdx.x;
-  const int c = t / nmom, m = t - c * nmom;
-  int pi = 0, pj = -1;
-  if (c < 3 && m >= K) {
-    int r = m - K;
-    pi = 0;
-    while (r >= K - pi) { r -= K - pi; ++pi; }
-    pj = pi + r;
-  } else if (c < 3) {
-    pi = m;
-  }
-  double acc = 0.0;
+  const int g = t & 7, task = t >> 3;          // row group, (channel, block pair)
+  const int c = task / 10, pidx = task - c * 10;
+  // block pairs in the order (0,0) (0,1) (0,2) (0,3) (1,1) (1,2) (1,3) (2,2) (2,3) (3,3)
+  const int bi = pidx < 4 ? 0 : pidx < 7 ? 1 : pidx < 9 ? 2 : 3;
+  const int bj = pidx < 4 ? pidx : pidx < 7 ? pidx - 3 : pidx < 9 ? pidx - 5 : 3;
+  const bool active = task < 30, diag = bi == bj;
+  double acc[kStatAcc];
+#pragma unroll
+  for (int i = 0; i < kStatAcc; ++i) acc[i] = 0.0;
+  for (int i = t; i < (kColRows / 2) * kStatW; i += kStatThreads) s_d[i] = make_double2(0.0, 0.0);   // padding columns stay zero
   const uint32_t stride = gridDim.x * kColRows;
   uint32_t r0 = blockIdx.x * kColRows;
   int cur = 0;
@@ -101,42 +106,75 @@ __global__ void __launch_bounds__(448) color_stats_kernel(const float* __restric
     cp_async_commit();
     cp_async_wait<1>();
     __syncthreads();                                      // rows(cur) landed; the previous tile's moments are done with s_d
-    // AC triples -> YUV, widened to fp64 once.  Rows are stored in pairs, s_d[(r / 2) * W + col] = {row r, row r + 1}, so
-    // that the moment loop below fetches two rows per 16-byte load (it is bound by shared-memory wavefronts)
-    const uint32_t cnt2 = (cnt + 1u) & ~1u;
-    for (uint32_t i = t; i < cnt2 * (uint32_t)K; i += blockDim.x) {
-      const uint32_t r = i / K, j = i - r * K;
-      double y = 0.0, u = 0.0, v = 0.0;
-      if (r < cnt) {
-        const float* row = rows + (size_t)r * C + 11 + j;
-        const float a = row[0], b = row[K], g = row[2 * K];
-        y = (double)fmaf(c_yuv[0], a, fmaf(c_yuv[1], b, c_yuv[2] * g));
-        u = (double)fmaf(c_yuv[3], a, fmaf(c_yuv[4], b, c_yuv[5] * g));
-        v = (double)fmaf(c_yuv[6], a, fmaf(c_yuv[7], b, c_yuv[8] * g));
+    // AC triples of two rows -> YUV, widened to fp64 once (rows beyond the tile's count are zeros)
+    for (uint32_t i = t; i < (uint32_t)(kColRows / 2) * (uint32_t)K; i += kStatThreads) {
+      const uint32_t rp = (K == 15) ? (i / 15u) : i / (uint32_t)K, j = i - rp * (uint32_t)K;
+      double2 y = make_double2(0.0, 0.0), u = y, v = y;
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        const uint32_t r = 2 * rp + h;
+        if (r < cnt) {
+          const float* row = rows + (size_t)r * C + 11 + j;
+          const float a = row[0], b = row[K], gg = row[2 * K];
+          const double yy = (double)fmaf(c_yuv[0], a, fmaf(c_yuv[1], b, c_yuv[2] * gg));
+          const double uu = (double)fmaf(c_yuv[3], a, fmaf(c_yuv[4], b, c_yuv[5] * gg));
+          const double vv = (double)fmaf(c_yuv[6], a, fmaf(c_yuv[7], b, c_yuv[8] * gg));
+          if (h == 0) { y.x = yy; u.x = uu; v.x = vv; } else { y.y = yy; u.y = uu; v.y = vv; }
+        }
       }
-      double* d = s_d + ((size_t)(r >> 1) * W + j) * 2 + (r & 1u);
-      d[0] = y; d[2 * K] = u; d[4 * K] = v;
+      double2* d = s_d + (size_t)rp * kStatW + j;
+      d[0] = y; d[16] = u; d[32] = v;
     }
     __syncthreads();
-    if (c < 3) {
-      const double2* a = reinterpret_cast<const double2*>(s_d) + K * c + pi;
-      if (pj < 0) {
-#pragma unroll 8
-        for (uint32_t r = 0; r < cnt2 / 2; ++r) { const double2 x = a[(size_t)r * W]; acc += x.x; acc += x.y; }
-      } else {
-        const double2* b = reinterpret_cast<const double2*>(s_d) + K * c + pj;
-#pragma unroll 8
-        for (uint32_t r = 0; r < cnt2 / 2; ++r) {
-          const double2 x = a[(size_t)r * W], y = b[(size_t)r * W];
-          acc = fma(x.x, y.x, acc);
-          acc = fma(x.y, y.y, acc);
+    if (active) {
+      const double2* pa = s_d + 16 * c + 4 * bi;
+      const double2* pb = s_d + 16 * c + 4 * bj;
+#pragma unroll
+      for (int q = 0; q < kColRows / 16; ++q) {             // this group's row pairs: g, g + 8, ...
+        const int rp = g + 8 * q;
+        double2 a[4], b[4];
+#pragma unroll
+        for (int u = 0; u < 4; ++u) { a[u] = pa[(size_t)rp * kStatW + u]; b[u] = pb[(size_t)rp * kStatW + u]; }
+#pragma unroll
+        for (int u = 0; u < 4; ++u)
+#pragma unroll
+          for (int v = 0; v < 4; ++v) acc[4 * u + v] = fma(a[u].y, b[v].y, fma(a[u].x, b[v].x, acc[4 * u + v]));
+        if (diag) {
+#pragma unroll
+          for (int u = 0; u < 4; ++u) acc[16 + u] += a[u].x + a[u].y;
         }
       }
     }
     cur ^= 1;
   }
   cp_async_wait<0>();
-  if (c < 3) partial[((size_t)blockIdx.x * 3 + c) * kMomMax + m] = acc;
+  __syncthreads();
+  // combine the eight row groups in a fixed order: one thread per moment
+  double* s_red = reinterpret_cast<double*>(s_rows);        // [task][group][kStatAcc]
+  if (active) {
+#pragma unroll
+    for (int i = 0; i < kStatAcc; ++i) s_red[((size_t)task * 8 + g) * kStatAcc + i] = acc[i];
+  }
+  __syncthreads();
+  const int nmom = K + K * (K + 1) / 2;
+  for (int m3 = t; m3 < 3 * nmom; m3 += kStatThreads) {
+    const int cc = m3 / nmom, m = m3 - cc * nmom;
+    int pi = m, pj = -1;
+    if (m >= K) {                                           // the pair (pi, pj), pi <= pj, in row-major upper-triangle order
+      int r = m - K;
+      pi = 0;
+      while (r >= K - pi) { r -= K - pi; ++pi; }
+      pj = pi + r;
+    }
+    const int ti = pi >> 2, tj = (pj < 0 ? pi : pj) >> 2;
+    const int pidx2 = ti == 0 ? tj : ti == 1 ? 3 + tj : ti == 2 ? 5 + tj : 9;      // inverse of the block-pair order above
+    const int slot = pj < 0 ? 16 + (pi & 3) : 4 * (pi & 3) + (pj & 3);
+    const double* src = s_red + (size_t)(cc * 10 + pidx2) * 8 * kStatAcc + slot;
+    double a = 0.0;
+#pragma unroll
+    for (int gg = 0; gg < 8; ++gg) a += src[gg * kStatAcc];
+    partial[((size_t)blockIdx.x * 3 + cc) * kMomMax + m] = a;
+  }
 }
 
 // ---- 2. three K x K eigen-decompositions (cyclic Jacobi, fp64), one warp each ----------------------------------------
@@ -186,6 +224,14 @@ __global__ void __launch_bounds__(kEigThreads) klt_eig_kernel(const double* __re
   }
   __syncwarp();
   const int Kp = K + (K & 1), ring = Kp - 1, npair = Kp / 2;          // players 0 .. Kp-1 (player K is a bye when K is odd)
+  constexpr int kItems = (kKMax * ((kKMax + 1) / 2) + 31) / 32;       // (pair, row) items per lane and round
+  int it_k[kItems], it_i[kItems];                                    // pair and row / column of this lane's items (-1: none)
+#pragma unroll
+  for (int it = 0; it < kItems; ++it) {
+    const int idx = lane + 32 * it;
+    it_k[it] = idx < K * npair ? idx / K : -1;
+    it_i[it] = idx < K * npair ? idx % K : 0;
+  }
   for (int sweep = 0; sweep < 30; ++sweep) {
     double off = 0.0, dia = 0.0;
     for (int i = lane; i < K * K; i += 32) {
@@ -204,9 +250,19 @@ __global__ void __launch_bounds__(kEigThreads) klt_eig_kernel(const double* __re
         if (q < K) {
           const double apq = s_S[c][p][q];
           if (apq != 0.0) {
-            const double theta = (s_S[c][q][q] - s_S[c][p][p]) / (2.0 * apq);
-            const double tt = (theta >= 0.0 ? 1.0 : -1.0) / (fabs(theta) + sqrt(theta * theta + 1.0));
-            cs = 1.0 / sqrt(tt * tt + 1.0);
+            // tan of the rotation angle: the smaller root of t^2 + 2 theta t - 1 = 0.  Reciprocal and reciprocal square
+            // root instead of division and square root (this lane's chain is the critical path of the round)
+            const double theta = (s_S[c][q][q] - s_S[c][p][p]) * __drcp_rn(2.0 * apq);
+            const double at = fabs(theta);
+            double tt;
+            if (at < 1e100) {
+              const double w = theta * theta + 1.0;
+              tt = __drcp_rn(at + w * rsqrt(w));
+            } else {
+              tt = 0.5 * __drcp_rn(at);                   // theta^2 would overflow
+            }
+            if (theta < 0.0) tt = -tt;
+            cs = rsqrt(tt * tt + 1.0);
             sn = tt * cs;
           }
         }
@@ -214,28 +270,50 @@ __global__ void __launch_bounds__(kEigThreads) klt_eig_kernel(const double* __re
         s_rot[c][lane][0] = cs; s_rot[c][lane][1] = sn;
       }
       __syncwarp();
-      for (int idx = lane; idx < K * npair; idx += 32) {    // columns p, q of S and V:  [x_p, x_q] <- [c x_p - s x_q, s x_p + c x_q]
-        const int k = idx / K, i = idx - k * K;
-        const double ck = s_rot[c][k][0], sk = s_rot[c][k][1];
-        if (sk != 0.0) {
-          const int pk = s_pq[c][k][0], qk = s_pq[c][k][1];
-          const double sp = s_S[c][i][pk], sq = s_S[c][i][qk];
-          s_S[c][i][pk] = ck * sp - sk * sq;
-          s_S[c][i][qk] = sk * sp + ck * sq;
-          const double vp = s_V[c][i][pk], vq = s_V[c][i][qk];
-          s_V[c][i][pk] = ck * vp - sk * vq;
-          s_V[c][i][qk] = sk * vp + ck * vq;
+      // columns p, q of S and V:  [x_p, x_q] <- [c x_p - s x_q, s x_p + c x_q].  The (pair, row) items of a lane are
+      // independent: all operands are loaded before the first store (one warp per matrix: nothing else hides the latency)
+      {
+        double ck[kItems], sk[kItems], sp[kItems], sq[kItems], vp[kItems], vq[kItems];
+        int pk[kItems], qk[kItems];
+#pragma unroll
+        for (int it = 0; it < kItems; ++it) {
+          sk[it] = 0.0;
+          if (it_k[it] >= 0) {
+            ck[it] = s_rot[c][it_k[it]][0]; sk[it] = s_rot[c][it_k[it]][1];
+            pk[it] = s_pq[c][it_k[it]][0]; qk[it] = s_pq[c][it_k[it]][1];
+            sp[it] = s_S[c][it_i[it]][pk[it]]; sq[it] = s_S[c][it_i[it]][qk[it]];
+            vp[it] = s_V[c][it_i[it]][pk[it]]; vq[it] = s_V[c][it_i[it]][qk[it]];
+          }
+        }
+#pragma unroll
+        for (int it = 0; it < kItems; ++it) {
+          if (sk[it] != 0.0) {
+            s_S[c][it_i[it]][pk[it]] = ck[it] * sp[it] - sk[it] * sq[it];
+            s_S[c][it_i[it]][qk[it]] = sk[it] * sp[it] + ck[it] * sq[it];
+            s_V[c][it_i[it]][pk[it]] = ck[it] * vp[it] - sk[it] * vq[it];
+            s_V[c][it_i[it]][qk[it]] = sk[it] * vp[it] + ck[it] * vq[it];
+          }
         }
       }
       __syncwarp();
-      for (int idx = lane; idx < K * npair; idx += 32) {    // rows p, q of S
-        const int k = idx / K, j = idx - k * K;
-        const double ck = s_rot[c][k][0], sk = s_rot[c][k][1];
-        if (sk != 0.0) {
-          const int pk = s_pq[c][k][0], qk = s_pq[c][k][1];
-          const double sp = s_S[c][pk][j], sq = s_S[c][qk][j];
-          s_S[c][pk][j] = ck * sp - sk * sq;
-          s_S[c][qk][j] = sk * sp + ck * sq;
+      {   // rows p, q of S
+        double ck[kItems], sk[kItems], sp[kItems], sq[kItems];
+        int pk[kItems], qk[kItems];
+#pragma unroll
+        for (int it = 0; it < kItems; ++it) {
+          sk[it] = 0.0;
+          if (it_k[it] >= 0) {
+            ck[it] = s_rot[c][it_k[it]][0]; sk[it] = s_rot[c][it_k[it]][1];
+            pk[it] = s_pq[c][it_k[it]][0]; qk[it] = s_pq[c][it_k[it]][1];
+            sp[it] = s_S[c][pk[it]][it_i[it]]; sq[it] = s_S[c][qk[it]][it_i[it]];
+          }
+        }
+#pragma unroll
+        for (int it = 0; it < kItems; ++it) {
+          if (sk[it] != 0.0) {
+            s_S[c][pk[it]][it_i[it]] = ck[it] * sp[it] - sk[it] * sq[it];
+            s_S[c][qk[it]][it_i[it]] = sk[it] * sp[it] + ck[it] * sq[it];
+          }
         }
       }
       __syncwarp();
@@ -386,13 +464,20 @@ int run_klt_fit(gsnfs_ctx* ctx, cudaStream_t st, const float* d_attr, uint32_t n
   const uint32_t* n_dev = d_counts ? &d_counts->n_voxels : nullptr;
   const int K = (channels - 11) / 3;
   if (K == 0) return GSNFS_OK;
-  const int nmom = K + K * (K + 1) / 2;
-  const int threads = (3 * nmom + 31) & ~31;
-  const int grid = (int)min((uint32_t)ctx->color_parts_cap, (n + kColRows - 1) / kColRows);
+  // row tiles + the fp64 copy; the final combine reuses the buffer as [30 tasks][8 groups][kStatAcc] doubles
+  const size_t smem = max(sizeof(float) * 2 * kColRows * channels + sizeof(double2) * (kColRows / 2) * kStatW,
+                          sizeof(double) * 30 * 8 * kStatAcc);
+  int per_sm = ctx->occ_cache[8];
+  if (per_sm == 0 || ctx->occ_cache_smem[8] != smem) {
+    GSNFS_CUDA_OK(ctx, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, color_stats_kernel, kStatThreads, smem));
+    ctx->occ_cache[8] = per_sm;
+    ctx->occ_cache_smem[8] = smem;
+  }
+  const uint32_t want = (n + kColRows - 1) / kColRows;
+  const int grid = (int)min(min((uint32_t)ctx->color_parts_cap, (uint32_t)max(per_sm, 1) * (uint32_t)ctx->num_sms), want);
   if (grid < 1) return GSNFS_OK;
-  const size_t smem = sizeof(float) * 2 * kColRows * channels + sizeof(double) * kColRows * 3 * K;
   GSNFS_KERNEL(ctx, st, "color_stats");
-  color_stats_kernel<<<grid, threads, smem, st>>>(d_attr, n, n_dev, channels, ctx->color_partial);
+  color_stats_kernel<<<grid, kStatThreads, smem, st>>>(d_attr, n, n_dev, channels, ctx->color_partial);
   GSNFS_LAUNCH_CHECK(ctx, st);
   GSNFS_KERNEL(ctx, st, "klt_eig");
   klt_eig_kernel<<<1, kEigThreads, 0, st>>>(ctx->color_partial, grid, n, n_dev, channels, d_klt);
@@ -418,7 +503,7 @@ int run_color_apply(gsnfs_ctx* ctx, cudaStream_t st, bool inverse, const float* 
 int color_setup(gsnfs_ctx* ctx) {
   const int smem = (int)(sizeof(float) * (2 * kColRows * 57 + 3 * kKMax * kEP + 3 * kEP));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(color_stats_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)(sizeof(float) * 2 * kColRows * 56 + sizeof(double) * kColRows * 3 * kKMax)));
+                                          (int)(sizeof(float) * 2 * kColRows * 56 + sizeof(double2) * (kColRows / 2) * kStatW)));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(color_apply_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(color_apply_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   return GSNFS_OK;
