@@ -57,6 +57,14 @@ __device__ __forceinline__ void stage_rows_async(float* s, int pitch, const floa
   const uint32_t tot = cnt * (uint32_t)C;
   if (pitch == C && ((tot | (uint32_t)C) & 3u) == 0u && (reinterpret_cast<uintptr_t>(g) & 15u) == 0u) {
     for (uint32_t i = threadIdx.x; i < tot / 4; i += blockDim.x) cp_async16(s + 4 * i, g + 4 * i);
+  } else if ((C & 7) == 0 && (blockDim.x & 7u) == 0u) {
+    // 8 lanes per row (one 32-byte sector each), C / 8 independent copies per thread and row pass, no index division
+    const uint32_t c0 = threadIdx.x & 7u, rstep = blockDim.x >> 3;
+    for (uint32_t r = threadIdx.x >> 3; r < cnt; r += rstep) {
+      float* sr = s + (size_t)r * pitch + c0;
+      const float* gr = g + (size_t)r * C + c0;
+      for (int q = 0; q < C; q += 8) cp_async4(sr + q, gr + q);
+    }
   } else {
     for (uint32_t i = threadIdx.x; i < tot; i += blockDim.x) {
       const uint32_t r = i / (uint32_t)C, c = i - r * (uint32_t)C;
@@ -449,8 +457,16 @@ __global__ void __launch_bounds__(256) color_apply_kernel(const float* __restric
       __syncthreads();
     }
     float* g = out + (size_t)r0 * C;
-    for (uint32_t r = t >> 5; r < cnt; r += blockDim.x >> 5)                      // a warp per row: coalesced, no division
-      for (int ch = t & 31; ch < C; ch += 32) g[(size_t)r * C + ch] = rows[(size_t)r * P + ch];
+    if ((C & 7) == 0) {                                    // 8 lanes per row: full 32-byte sectors, no index division
+      for (uint32_t r = t >> 3; r < cnt; r += blockDim.x >> 3) {
+        const float* sr = rows + (size_t)r * P + (t & 7);
+        float* gr = g + (size_t)r * C + (t & 7);
+        for (int q = 0; q < C; q += 8) gr[q] = sr[q];
+      }
+    } else {
+      for (uint32_t r = t >> 5; r < cnt; r += blockDim.x >> 5)                    // a warp per row: coalesced
+        for (int ch = t & 31; ch < C; ch += 32) g[(size_t)r * C + ch] = rows[(size_t)r * P + ch];
+    }
     __syncthreads();                                       // the next iteration's prefetch refills this buffer
     cur ^= 1;
   }
