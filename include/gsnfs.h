@@ -284,6 +284,35 @@ int gsnfs_rans_decode(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* d_payl
                       const uint16_t* d_freq, const uint16_t* d_nwords, uint64_t n, uint8_t* d_out,
                       gsnfs_rans_info* d_info);
 
+/* gsnfs_rans_decode for callers that may not allocate device memory.
+ * Who needs it: a player or renderer that decodes occupancy streams from a thread or a phase of its frame loop where
+ * device allocation is off limits -- the application has handed the whole GPU to its own pool (a tensor framework's
+ * caching allocator, an engine's arena) so a library cudaMalloc can fail or fragment it; or it runs under a memory
+ * budget that is frozen after start-up; or it cannot afford the device-wide synchronisation and the unbounded latency
+ * a cudaMalloc/cudaFree brings into a real-time loop.  Every other call of this header needs a gsnfs_ctx, and
+ * gsnfs_create() is one cudaMalloc.  This call takes NO context and calls no cudaMalloc, cudaFree or any library
+ * routine that allocates: its only working memory (the table of block-stream offsets, 8 bytes per 1024-byte block,
+ * which gsnfs_rans_decode keeps in the context scratch) is a fixed 256 KB array that is part of the library image, so
+ * every GPU that loads libgsnfs.so holds those 256 KB from load until the process exits, used or not.
+ * Same arguments, same result (d_out and d_info, bit for bit) and same device-side corruption report as
+ * gsnfs_rans_decode; inputs and outputs are still the caller's device buffers.
+ * Limit: n <= GSNFS_RANS_STATIC_MAX_BYTES (32 MiB of occupancy bytes: the 16M-Gaussian frame at depth 16 needs about
+ * 19 MB); a larger n returns GSNFS_E_CAPACITY before anything is enqueued -- use gsnfs_rans_decode with a context then.
+ * Device: the work goes to the CURRENT device of the calling thread, which must be the device `stream` belongs to.
+ * First call on each device: it looks up the device address of the built-in table (and sets one kernel attribute),
+ * once, under a lock; that lookup is ordinary host-side set-up work, so make this first call before any stream capture
+ * is started on that device.  Later calls only enqueue two kernels on `stream` and return without synchronising.
+ * Sharing: all calls on one device use the same table.  Calls on one stream are ordered and safe back to back; two
+ * calls that can overlap on the GPU (different streams, no event between them) race on the table and decode
+ * garbage -- serialise them.  The table keeps the previous call's offsets between calls; nothing in it has to start at
+ * zero, every call rewrites the entries it reads (and d_info in full) before it reads them.
+ * Errors: INVALID_ARGUMENT (NULL pointer, n >= 2^32), CAPACITY (n beyond the limit above), CUDA (no current device,
+ * more than 64 devices, a failed launch; cudaGetLastError() still holds the runtime's code). */
+#define GSNFS_RANS_STATIC_MAX_BYTES (32ull << 20)
+int gsnfs_rans_decode_static(gsnfs_stream stream, const uint8_t* d_payload, uint64_t payload_bytes,
+                             const uint16_t* d_freq, const uint16_t* d_nwords, uint64_t n, uint8_t* d_out,
+                             gsnfs_rans_info* d_info);
+
 /* ---- bitstream container (host only) -----------------------------------------------------------------
  * PAPER.md:L176 ("J ... and the number of occupied nodes n_d at each level ... is encoded in the bitstream as
  * metadata"), L526 ("The header stores the number of levels and the node count of each level"), L255 (per-attribute

@@ -94,6 +94,7 @@ _SIGNATURES = {
     "gsnfs_rans_encode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p, c_void_p, c_void_p, c_uint64,
                                   c_void_p]),
     "gsnfs_rans_decode": (c_int, [c_void_p, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p]),
+    "gsnfs_rans_decode_static": (c_int, [c_void_p, c_void_p, c_uint64, c_void_p, c_void_p, c_uint64, c_void_p, c_void_p]),
     "gsnfs_container_size": (c_uint64, [POINTER(GsnfsSection), c_int]),
     "gsnfs_container_pack": (c_int, [POINTER(GsnfsFrameDesc), POINTER(GsnfsSection), c_int, c_void_p, c_uint64,
                                      POINTER(c_uint64)]),
@@ -402,6 +403,24 @@ def gsnfs_rans_decode(ctx: Context, d_payload, payload_bytes, d_freq, d_nwords, 
         _dptr(d_freq, torch.int16, "d_freq"), _dptr(d_nwords, torch.int16, "d_nwords"), int(n),
         _dptr(d_out, torch.uint8, "d_out"), _dptr(d_info, torch.int64, "d_info"))
     ctx._check(rc, "gsnfs_rans_decode")
+
+
+GSNFS_RANS_STATIC_MAX_BYTES = 32 << 20
+
+
+def gsnfs_rans_decode_static(d_payload, payload_bytes, d_freq, d_nwords, n, d_out, d_info, stream=None):
+    """gsnfs_rans_decode for callers that may not allocate device memory (their own pool owns the GPU, a frozen memory
+    budget, or a frame loop that cannot take cudaMalloc's device-wide synchronisation): no Context, no allocation; the
+    block-offset table is a fixed 256 KB array inside the library.  n <= GSNFS_RANS_STATIC_MAX_BYTES, else GsnfsError
+    (GSNFS_E_CAPACITY).  Runs on the current device; calls that overlap on the GPU race on the shared table; the first
+    call on a device does a one-off address lookup and belongs before any stream capture (include/gsnfs.h)."""
+    rc = lib().gsnfs_rans_decode_static(
+        _stream(stream), _dptr(d_payload, torch.uint8, "d_payload"), int(payload_bytes),
+        _dptr(d_freq, torch.int16, "d_freq"), _dptr(d_nwords, torch.int16, "d_nwords"), int(n),
+        _dptr(d_out, torch.uint8, "d_out"), _dptr(d_info, torch.int64, "d_info"))
+    if rc != GSNFS_OK:
+        raise GsnfsError(rc, "gsnfs_rans_decode_static",
+                         f"(n = {int(n)}, limit {GSNFS_RANS_STATIC_MAX_BYTES} bytes)" if rc == -2 else "")
 
 
 def container_pack(desc: GsnfsFrameDesc, sections: dict) -> np.ndarray:

@@ -8,6 +8,8 @@
 // encodes backwards from a padded shared-memory copy of its 1024 bytes into a strided scratch -> scan of the word counts
 // -> compaction into the caller's payload.  Decoding is one launch: a 4096-entry slot -> symbol table in shared
 // memory, one thread per block, output staged in shared memory and written coalesced.
+#include <mutex>
+
 #include "common.cuh"
 
 namespace gsnfs {
@@ -302,3 +304,70 @@ int rans_setup(gsnfs_ctx* ctx) {
 }
 
 }  // namespace gsnfs
+
+// ---- gsnfs_rans_decode_static: the decoder without a context and without any allocation ---------------------------
+// For callers that must not allocate device memory (see gsnfs.h: the GPU belongs to the application's own pool, the
+// memory budget is frozen, or a cudaMalloc's device-wide synchronisation has no place in their frame loop).  The one
+// piece of working memory the decoder needs -- the byte offset of every block stream, which run_rans_decode() keeps in
+// the context scratch -- lives here in a file-scope device array that ships inside the library image.  The kernels are
+// the ones above; only where `off` points differs.
+
+namespace gsnfs {
+namespace {
+
+constexpr uint64_t kStaticMaxBlocks = GSNFS_RANS_STATIC_MAX_BYTES / kRansBlock;      // 32768 blocks
+static_assert(GSNFS_RANS_STATIC_MAX_BYTES % kRansBlock == 0, "limit is a whole number of blocks");
+
+// 256 KB + 8 on every GPU that loads the library, until the process exits.  In HOST code this name is only a handle
+// for cudaGetSymbolAddress(): it is not a device address and must never be handed to a kernel as one.
+static __device__ __align__(256) uint64_t g_static_off[kStaticMaxBlocks + 1];
+
+constexpr int kStaticMaxDevices = 64;
+std::mutex g_static_mu;
+uint64_t* g_static_off_dev[kStaticMaxDevices];     // device address of g_static_off on device i; nullptr = not set up
+
+// Once per device, with that device current: resolve the array's device address (every device has its own copy of
+// the array at its own address) and raise the decoder's dynamic shared memory limit as rans_setup() does per context.
+int static_off_for_current_device(uint64_t** out) {
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kStaticMaxDevices) return GSNFS_E_CUDA;
+  std::lock_guard<std::mutex> lock(g_static_mu);
+  if (!g_static_off_dev[dev]) {
+    uint64_t* p = nullptr;
+    if (cudaGetSymbolAddress((void**)&p, g_static_off) != cudaSuccess || !p) return GSNFS_E_CUDA;
+    if (cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)(kRansCta * kRansPitch + kRansM)) != cudaSuccess)
+      return GSNFS_E_CUDA;
+    g_static_off_dev[dev] = p;
+  }
+  *out = g_static_off_dev[dev];
+  return GSNFS_OK;
+}
+
+}  // namespace
+}  // namespace gsnfs
+
+int gsnfs_rans_decode_static(gsnfs_stream stream, const uint8_t* d_payload, uint64_t payload_bytes,
+                             const uint16_t* d_freq, const uint16_t* d_nwords, uint64_t n, uint8_t* d_out,
+                             gsnfs_rans_info* d_info) {
+  using namespace gsnfs;
+  if (!d_freq || !d_info || (n && (!d_payload || !d_nwords || !d_out))) return GSNFS_E_INVALID_ARGUMENT;
+  if (n >= (1ull << 32)) return GSNFS_E_INVALID_ARGUMENT;
+  if (n > GSNFS_RANS_STATIC_MAX_BYTES) return GSNFS_E_CAPACITY;      // the built-in table has no room: nothing is enqueued
+  uint64_t* off = nullptr;
+  const int rc = static_off_for_current_device(&off);
+  if (rc != GSNFS_OK) return rc;
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint64_t nblk = (n + kRansBlock - 1) / kRansBlock;           // <= kStaticMaxBlocks; the scan writes off[0 .. nblk]
+  // The scan rewrites every offset this call's decoder reads, and all of d_info, so the previous call's leftovers in
+  // the table are never seen and nothing needs a memset.
+  rans_scan_kernel<<<1, 1024, 0, st>>>(d_nwords, n, nullptr, nblk, off, ~0ull, d_info);
+  if (cudaPeekAtLastError() != cudaSuccess) return GSNFS_E_CUDA;
+  const int grid = (int)((nblk + kRansCta - 1) / kRansCta);
+  if (grid > 0) {
+    rans_decode_kernel<<<grid, kRansCta, kRansCta * kRansPitch + kRansM, st>>>(d_payload, payload_bytes, d_freq, d_nwords, off,
+                                                                              n, d_out, d_info);
+    if (cudaPeekAtLastError() != cudaSuccess) return GSNFS_E_CUDA;
+  }
+  return GSNFS_OK;
+}
