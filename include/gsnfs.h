@@ -55,7 +55,8 @@ typedef struct gsnfs_counts {
  *   q = sign(y) * floor(|y| * (1/qstep_c) + dz_round),   y^ = sign(q) * (|q| + recon_bias*[q != 0]) * qstep_c.
  * Arithmetic of the integer decision (normative, the CPU oracle evaluates the same): y is the fp32 coefficient
  * widened to fp64; 1/qstep_c is the fp64 reciprocal of the fp32 step (one rounding); the product and the sum are
- * each rounded once in fp64 (no fused multiply-add); floor; saturation to int32.
+ * each rounded once in fp64 (no fused multiply-add); floor; saturation to int32; sign(+-0) = 0, so an exactly zero
+ * coefficient gives q = 0 even at dz_round = 1.
  * NULL => { 1/3, 0 }.  Required: 0 <= dz_round <= 1, 0 <= recon_bias < 1, both finite (else INVALID_ARGUMENT). */
 typedef struct gsnfs_quant {
   float dz_round;
@@ -140,8 +141,8 @@ int gsnfs_octree_decode(gsnfs_ctx* ctx, gsnfs_stream stream,
  * index, high = -b*y0 + a*y1 goes to the right index (A.6 l.16-17) [R6].  The signal transformed is
  * x_i = sqrt(w_i) * attr_i [R2]; d_weights == NULL means unit leaf weights (the paper's case).
  * Output order ("canonical order", [R8]): row i of the Morton-sorted voxel list, row 0 = DC.
- *   qstep (host, `channels` entries) != NULL: d_qcoeff[i][c] = sign(y) floor(|y|/qstep_c + dz_round),
- *   saturated to int32, evaluated in fp64 from the fp32 coefficient.  d_coeff (unquantised fp32) and
+ *   qstep (host, `channels` entries) != NULL: d_qcoeff[i][c] = sign(y) floor(|y| * (1/qstep_c) + dz_round),
+ *   saturated to int32, in the arithmetic gsnfs_quant states (fp64, from the fp32 coefficient).  d_coeff (unquantised fp32) and
  *   d_qcoeff may each be NULL, not both; d_qcoeff requires qstep.
  * n_voxels is the row count; if d_counts != NULL the actual N_v is read on the device from it and
  * n_voxels is only an upper bound (rows beyond N_v are untouched); a d_counts whose status is already non-zero
@@ -163,7 +164,7 @@ int gsnfs_raht_forward(gsnfs_ctx* ctx, gsnfs_stream stream,
                        int32_t* d_qcoeff, float* d_coeff);
 
 /* One more quantisation of an unquantised coefficient tensor (d_coeff of gsnfs_raht_forward, N_v x channels,
- * canonical order): d_qcoeff[i][c] = sign(y) floor(|y|/qstep_c + dz_round), the same rule and arithmetic as the
+ * canonical order): d_qcoeff[i][c] = sign(y) floor(|y| * (1/qstep_c) + dz_round), the same rule and arithmetic as the
  * quantiser fused into gsnfs_raht_forward [R10], so a bitrate ladder (one step per
  * attribute and rung) can share one sort/octree/transform and pay only this pass per rung.  qstep: host,
  * `channels` entries, all > 0 and finite; quant may be NULL (dz_round = 1/3).  n_rows is the row count; if

@@ -491,9 +491,24 @@ static int frame_pool(gsnfs_ctx* c) {
   const size_t o_occ = b.take(c->occ_cap), o_lev = b.take(256), o_perm = b.take(N * 4), o_vk = b.take(N * 8);
   const size_t o_vs = b.take((N + 1) * 4), o_w = b.take(N * 4), o_vx = b.take(N * 12), o_cnt = b.take(256);
   const size_t o_bits = b.take(c->rlgr_off_cap * 4), o_info = b.take(256);
+  // create everything first and publish it last: a context whose pool, copy stream or events could not be created keeps
+  // fpool == NULL, so the next call tries again instead of running on a null stream
+  char* p = nullptr;
+  cudaStream_t cs = nullptr;
+  cudaEvent_t ea = nullptr, eb = nullptr;
+  cudaError_t e = cudaMalloc((void**)&p, b.off);
+  if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&cs, cudaStreamNonBlocking);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ea, cudaEventDisableTiming);
+  if (e == cudaSuccess) e = cudaEventCreateWithFlags(&eb, cudaEventDisableTiming);
+  if (e != cudaSuccess) {
+    if (eb) cudaEventDestroy(eb);
+    if (ea) cudaEventDestroy(ea);
+    if (cs) cudaStreamDestroy(cs);
+    if (p) cudaFree(p);
+    snprintf(c->err, sizeof(c->err), "host-frame staging (%zu bytes, copy stream, events): %s", b.off, cudaGetErrorString(e));
+    return GSNFS_E_CUDA;
+  }
   c->fpool_bytes = b.off;
-  GSNFS_CUDA_OK(c, cudaMalloc((void**)&c->fpool, c->fpool_bytes));
-  char* p = c->fpool;
   c->f_xyz = (float*)(p + o_xyz); c->f_attr = (float*)(p + o_attr); c->f_merged = (float*)(p + o_mrg);
   c->f_q = (int32_t*)(p + o_q); c->f_occ = (uint8_t*)(p + o_occ); c->f_levels = (uint32_t*)(p + o_lev);
   c->f_perm = (uint32_t*)(p + o_perm); c->f_vkeys = (uint64_t*)(p + o_vk); c->f_vstart = (uint32_t*)(p + o_vs);
@@ -501,13 +516,12 @@ static int frame_pool(gsnfs_ctx* c) {
   c->f_bits = (uint32_t*)(p + o_bits); c->f_info = (gsnfs_rlgr_info*)(p + o_info);
   c->f_stream = (uint8_t*)c->f_merged;                 // the fused encoder never materialises the merged tensor
   c->f_stream_cap = N * C * 4;
-  GSNFS_CUDA_OK(c, cudaStreamCreateWithFlags(&c->copy_stream, cudaStreamNonBlocking));
-  GSNFS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_a, cudaEventDisableTiming));
-  GSNFS_CUDA_OK(c, cudaEventCreateWithFlags(&c->ev_b, cudaEventDisableTiming));
+  c->copy_stream = cs; c->ev_a = ea; c->ev_b = eb;
+  c->fpool = p;
   return GSNFS_OK;
 }
 
-int gsnfs_frame_encode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
+static int frame_encode_host_impl(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
                             int channels, const float bbox_min[3], const float bbox_max[3], int depth,
                             const float* qstep, const gsnfs_quant* quant, uint8_t* h_occ, uint64_t occ_capacity,
                             uint32_t* h_level_sizes, uint32_t* h_weights, int32_t* h_qcoeff, gsnfs_counts* h_counts) {
@@ -545,7 +559,7 @@ int gsnfs_frame_encode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_
   return GSNFS_OK;
 }
 
-int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
+static int frame_decode_host_impl(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
                             const uint32_t* level_sizes, int depth, const uint32_t* h_weights, const int32_t* h_qcoeff,
                             int channels, const float* qstep, const gsnfs_quant* quant, uint32_t* h_voxel_xyz,
                             float* h_attr, gsnfs_counts* h_counts) {
@@ -590,7 +604,7 @@ int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* 
 }
 
 // ---- the same two frame calls with the coefficients entropy coded (RLGR) before they leave the device ----------
-int gsnfs_frame_encode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
+static int frame_encode_host_packed_impl(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
                                    int channels, const float bbox_min[3], const float bbox_max[3], int depth,
                                    const float* qstep, const gsnfs_quant* quant, int rlgr_block, uint8_t* h_occ,
                                    uint64_t occ_capacity, uint32_t* h_level_sizes, uint32_t* h_weights,
@@ -645,7 +659,7 @@ int gsnfs_frame_encode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const fl
   return take_sticky(ctx);
 }
 
-int gsnfs_frame_decode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
+static int frame_decode_host_packed_impl(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
                                    const uint32_t* level_sizes, int depth, const uint32_t* h_weights,
                                    const uint32_t* h_block_bits, const uint8_t* h_stream, uint64_t stream_bytes,
                                    int rlgr_block, int channels, const float* qstep, const gsnfs_quant* quant,
@@ -697,6 +711,56 @@ int gsnfs_frame_decode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const ui
   GSNFS_CUDA_OK(ctx, cudaStreamSynchronize(st));
   if (info.status) h_counts->status |= 1u;                                 // a corrupt coefficient stream is a corrupt frame
   return take_sticky(ctx);
+}
+
+// A frame call that fails after its first cudaMemcpyAsync (a bad bbox found by gsnfs_octree_encode, a capacity error of
+// a later stage, a CUDA error) must not hand the caller's pinned buffers back while a DMA still reads or writes them:
+// every failing return drains both streams first.  Successful returns have synchronised already.
+static int frame_done(gsnfs_ctx* ctx, gsnfs_stream stream, int rc) {
+  if (rc != GSNFS_OK && ctx) {
+    cudaStreamSynchronize((cudaStream_t)stream);
+    if (ctx->fpool && ctx->copy_stream) cudaStreamSynchronize(ctx->copy_stream);
+  }
+  return rc;
+}
+
+int gsnfs_frame_encode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
+                            int channels, const float bbox_min[3], const float bbox_max[3], int depth,
+                            const float* qstep, const gsnfs_quant* quant, uint8_t* h_occ, uint64_t occ_capacity,
+                            uint32_t* h_level_sizes, uint32_t* h_weights, int32_t* h_qcoeff, gsnfs_counts* h_counts) {
+  return frame_done(ctx, stream,
+                    frame_encode_host_impl(ctx, stream, h_xyz, h_attr, n, channels, bbox_min, bbox_max, depth, qstep, quant, h_occ,
+                                           occ_capacity, h_level_sizes, h_weights, h_qcoeff, h_counts));
+}
+
+int gsnfs_frame_decode_host(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
+                            const uint32_t* level_sizes, int depth, const uint32_t* h_weights, const int32_t* h_qcoeff,
+                            int channels, const float* qstep, const gsnfs_quant* quant, uint32_t* h_voxel_xyz,
+                            float* h_attr, gsnfs_counts* h_counts) {
+  return frame_done(ctx, stream,
+                    frame_decode_host_impl(ctx, stream, h_occ, occ_bytes, level_sizes, depth, h_weights, h_qcoeff, channels, qstep, quant,
+                                           h_voxel_xyz, h_attr, h_counts));
+}
+
+int gsnfs_frame_encode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const float* h_xyz, const float* h_attr, uint64_t n,
+                                   int channels, const float bbox_min[3], const float bbox_max[3], int depth,
+                                   const float* qstep, const gsnfs_quant* quant, int rlgr_block, uint8_t* h_occ,
+                                   uint64_t occ_capacity, uint32_t* h_level_sizes, uint32_t* h_weights,
+                                   uint32_t* h_block_bits, uint8_t* h_stream, uint64_t stream_capacity,
+                                   gsnfs_counts* h_counts, gsnfs_rlgr_info* h_info) {
+  return frame_done(ctx, stream,
+                    frame_encode_host_packed_impl(ctx, stream, h_xyz, h_attr, n, channels, bbox_min, bbox_max, depth, qstep, quant, rlgr_block, h_occ,
+                                                  occ_capacity, h_level_sizes, h_weights, h_block_bits, h_stream, stream_capacity, h_counts, h_info));
+}
+
+int gsnfs_frame_decode_host_packed(gsnfs_ctx* ctx, gsnfs_stream stream, const uint8_t* h_occ, uint64_t occ_bytes,
+                                   const uint32_t* level_sizes, int depth, const uint32_t* h_weights,
+                                   const uint32_t* h_block_bits, const uint8_t* h_stream, uint64_t stream_bytes,
+                                   int rlgr_block, int channels, const float* qstep, const gsnfs_quant* quant,
+                                   uint32_t* h_voxel_xyz, float* h_attr, gsnfs_counts* h_counts) {
+  return frame_done(ctx, stream,
+                    frame_decode_host_packed_impl(ctx, stream, h_occ, occ_bytes, level_sizes, depth, h_weights, h_block_bits, h_stream, stream_bytes,
+                                                  rlgr_block, channels, qstep, quant, h_voxel_xyz, h_attr, h_counts));
 }
 
 }  // extern "C"

@@ -274,7 +274,7 @@ __global__ void __launch_bounds__(kEigThreads) klt_eig_kernel(const double* __re
             sn = tt * cs;
           }
         }
-        s_pq[c][lane][0] = p; s_pq[c][lane][1] = q;
+        s_pq[c][lane][0] = p; s_pq[c][lane][1] = q < K ? q : p;     // the bye pair (q == K, odd K) is the identity: its operand loads stay inside the K x K matrix
         s_rot[c][lane][0] = cs; s_rot[c][lane][1] = sn;
       }
       __syncwarp();

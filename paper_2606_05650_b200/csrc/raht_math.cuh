@@ -98,7 +98,7 @@ __device__ __forceinline__ int quant_exact(float y, double inv, double f) {
   double m = floor(__dadd_rn(__dmul_rn(fabs((double)y), inv), f));      // product and sum rounded once each, no FMA (gsnfs.h)
   m = fmin(m, 2147483647.0);
   const int q = (int)m;
-  return y < 0.f ? -q : q;
+  return y < 0.f ? -q : (y > 0.f ? q : 0);      // sign(+-0) = 0: with dz_round == 1 the floor is 1 for y == 0, q is not
 }
 __device__ __forceinline__ bool quant_fast2(float y0, float y1, float i0, float i1, float fm, int& q0, int& q1) {
   const float s0 = __uint_as_float(__float_as_uint(fm) ^ (__float_as_uint(y0) & 0x80000000u));

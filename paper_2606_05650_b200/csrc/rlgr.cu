@@ -132,7 +132,10 @@ __global__ void __launch_bounds__(256) rlgr_encode_kernel(const int32_t* __restr
   }
   uint64_t my_off = 0;
   if (WRITE) {
-    if (r0 >= n) return;
+    if (r0 >= n) {                       // block 0 gets here only if the device-side N_v is 0: an empty stream, reported as such
+      if (b == 0 && c == 0) { info->stream_bytes = 0ull; info->n_blocks = gridDim.x * (uint32_t)C; info->status = 0u; }
+      return;
+    }
     const RowOffsets ro = rlgr_row_offsets(rowsum, supersum, b, gridDim.x, s_red);
     uint32_t rtot;
     const uint32_t ex = cta_excl_scan(c < C ? block_bits[(size_t)b * C + c] >> 3 : 0u, s_w, &rtot);
@@ -272,7 +275,9 @@ __global__ void __launch_bounds__(256) rlgr_decode_kernel(const uint8_t* __restr
   const size_t e = (size_t)b * C + c;
   const uint64_t off = ro.row_start + ex, bytes = block_bits[e] >> 3;
   int32_t* dst = q + r0 * C + c;
-  if ((block_bits[e] & 31u) || off + bytes > stream_bytes) {      // header inconsistent with the stream
+  // header inconsistent with the stream: a length that is not whole words, a block that therefore starts off a word
+  // boundary (some EARLIER entry was damaged: the word loads below would fault), or bytes beyond the stream
+  if ((block_bits[e] & 31u) || (off & 3ull) || off + bytes > stream_bytes) {
     atomicOr(&info->status, 1u);
     for (uint32_t i = 0; i < cnt; ++i) dst[(size_t)i * C] = 0;
     return;

@@ -126,3 +126,33 @@ def test_energy_compaction_and_pipeline(B):
         ctx.close()
     for bad in (57, 10, 11 + 3 * 16):
         assert B.gsnfs_klt_floats(bad) == 0
+
+
+def test_device_yuv_constants_against_the_bt601_definition(B):
+    """The nine device constants pinned to [R15]'s definition (U = 0.492 (B - Y), V = 0.877 (R - Y) from the luma weights),
+    not to the oracle's table: unit primaries through gsnfs_color_forward (YUV only), on the DC triple and on every AC
+    triple, read back entry by entry to the five printed digits (+ one fp32 rounding)."""
+    w = np.array([0.299, 0.587, 0.114])
+    D = np.stack([w, 0.436 / (1 - w[2]) * (np.array([0, 0, 1.0]) - w), 0.615 / (1 - w[0]) * (np.array([1.0, 0, 0]) - w)])
+    C, K = 56, 15
+    ctx = B.Context(max_points=64, max_channels=C, max_depth=4)
+    try:
+        trips = [[8, 9, 10]] + [[11 + j, 11 + K + j, 11 + 2 * K + j] for j in range(K)]
+        a = np.zeros((3 * len(trips), C), np.float32)
+        for t, trip in enumerate(trips):
+            for prim in range(3):
+                a[3 * t + prim, trip[prim]] = 1.0
+        a[:, :8] = 0.25                                                  # geometry channels must pass through
+        d_a = torch.from_numpy(a).to(DEV)
+        d_y = torch.empty_like(d_a)
+        B.gsnfs_color_forward(ctx, d_a, a.shape[0], None, C, None, d_y)
+        torch.cuda.synchronize()
+        y = d_y.cpu().numpy().astype(np.float64)
+        for t, trip in enumerate(trips):
+            for prim in range(3):
+                assert np.abs(y[3 * t + prim, trip] - D[:, prim]).max() < 1e-5 + 6e-8, (t, prim)
+                other = np.setdiff1d(np.arange(8, C), trip)
+                assert np.all(y[3 * t + prim, other] == 0.0)
+        assert np.all(y[:, :8] == 0.25)
+    finally:
+        ctx.close()

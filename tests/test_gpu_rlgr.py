@@ -34,7 +34,7 @@ def gpu_encode(B, ctx, q, block, capacity=None, counts=None, n_rows=None):
     cap = B.gsnfs_rlgr_capacity(n_rows, C, block) if capacity is None else capacity
     bits = torch.full((max(nb, 1),), -1, dtype=torch.int32, device=DEV)
     stream = torch.zeros(max(cap, 4), dtype=torch.uint8, device=DEV)
-    info = torch.zeros(2, dtype=torch.int64, device=DEV)
+    info = torch.full((2,), -1, dtype=torch.int64, device=DEV)
     B.gsnfs_rlgr_encode(ctx, d_q if n else torch.zeros((1, C), dtype=torch.int32, device=DEV), n_rows, counts, C, block, bits,
                         stream, info)
     torch.cuda.synchronize()
@@ -98,11 +98,13 @@ def test_real_coefficients_all_table_a5_block_sizes(B, ctx):
     assert sizes[512] <= 1.05 * sizes[8192]
 
 
-def test_config3_full_size_sampled_blocks_and_roundtrip(B, ctx):
-    """BASELINE.json configs[2] at full size in bench.py's launch configuration (block 2048): header compared in full
-    with the oracle, decode(encode(q)) = q on the device, 200 sampled block streams compared byte for byte."""
+@pytest.mark.parametrize("block", [512, 2048])
+def test_config3_full_size_sampled_blocks_and_roundtrip(B, ctx, block):
+    """BASELINE.json configs[2] at full size, at the block size bench.py times (RLGR_BLOCK = 512: 1954 CTAs) and at 2048
+    (489 CTAs, a different occupancy regime): header compared in full with the oracle, decode(encode(q)) = q on the device,
+    200 sampled block streams compared byte for byte."""
     rng = np.random.default_rng(11)
-    n, C, block = 1_000_000, 56, 2048
+    n, C = 1_000_000, 56
     scale = np.concatenate([np.full(3, 60.0), np.full(4, 40.0), [30.0], np.full(3, 25.0), np.full(45, 6.0)])
     q = np.rint(rng.laplace(0, 1, (n, C)) * scale[None, :]).astype(np.int32)
     bits, stream, nbytes, nblocks, status, d_q = gpu_encode(B, ctx, q, block)
@@ -146,8 +148,20 @@ def test_device_counts_chain_capacity_and_corruption(B, ctx):
     bad_bits[5] -= 32                                     # a block shorter than what its coefficients need
     back, (_, _, st) = gpu_decode(B, ctx, stream, nbytes, bad_bits, n, C, block)
     assert st & 1
+    # an entry damaged by a part of a word moves every later block of its row off a 4-byte boundary: flagged (status
+    # bit 0), no misaligned load, the context stays usable
+    for k, delta in ((5, 8), (5, 16), (0, 24), (C + 3, 8)):
+        bad_bits = bits.copy()
+        bad_bits[k] -= delta
+        back, (_, _, st) = gpu_decode(B, ctx, stream, nbytes, bad_bits, n, C, block)
+        assert st & 1, (k, delta)
     back, (_, _, st) = gpu_decode(B, ctx, stream, nbytes, bits, n, C, block)
     assert st == 0 and np.array_equal(back, q)
+    # device-side N_v = 0 with a host bound > 0 (an empty frame, or one the decoder flagged): an empty stream, and the
+    # info record is written (not left stale)
+    zero = torch.zeros(4, dtype=torch.int32, device=DEV)
+    ebits, _, nbytes0, nblocks0, status0, _ = gpu_encode(B, ctx, q, block, counts=zero)
+    assert (nbytes0, status0) == (0, 0) and nblocks0 == ebits.size and np.all(ebits == 0)
     for bad_block in (32, 100_000):
         with pytest.raises(B.GsnfsError):
             gpu_encode(B, ctx, q, bad_block, capacity=1 << 20)
@@ -170,6 +184,15 @@ def test_packed_host_frame_calls(B):
         for _ in range(2):      # twice: the second call reuses the staging pool and the copy stream
             B.gsnfs_frame_encode_host_packed(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None, blk,
                                              h_occ, h_lev, h_w, h_bits, h_stream, h_cnt, h_info)
+        # an argument error that is only found after the attribute copy was queued (an empty bounding box is rejected by
+        # the position coder): the call fails, returns with no DMA in flight on the caller's pinned buffers, and the
+        # context serves the next frame
+        with pytest.raises(B.GsnfsError):
+            B.gsnfs_frame_encode_host_packed(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_min, J, fr.qstep, None, blk,
+                                             h_occ, h_lev, h_w, h_bits, h_stream, h_cnt, h_info)
+        assert torch.cuda.current_stream().query()
+        B.gsnfs_frame_encode_host_packed(ctx, h_xyz, h_attr, n, C, fr.bbox_min, fr.bbox_max, J, fr.qstep, None, blk,
+                                         h_occ, h_lev, h_w, h_bits, h_stream, h_cnt, h_info)
         nv, ob = int(h_cnt[0]), int(h_cnt[1])
         nbytes = int(h_info.numpy().view(np.uint64)[0])
         assert nv == len(ref["voxel_keys"]) and np.array_equal(h_occ[:ob].numpy(), ref["occ"])
@@ -197,5 +220,16 @@ def test_packed_host_frame_calls(B):
         B.gsnfs_frame_decode_host_packed(ctx, h_occ, ob, h_lev.numpy(), J, h_w, bad, h_stream, nbytes, blk, C, fr.qstep,
                                          None, h_vx, h_out, h_cnt2)
         assert int(h_cnt2[2]) & 1
+        # so is a header entry damaged by part of a word (later blocks of the row would start off a 4-byte boundary): the
+        # call reports status bit 0 instead of faulting, and the context still decodes the intact frame afterwards
+        for delta in (8, 16):
+            bad = h_bits.clone().pin_memory()
+            bad[3] -= delta
+            B.gsnfs_frame_decode_host_packed(ctx, h_occ, ob, h_lev.numpy(), J, h_w, bad, h_stream, nbytes, blk, C, fr.qstep,
+                                             None, h_vx, h_out, h_cnt2)
+            assert int(h_cnt2[2]) & 1, delta
+        B.gsnfs_frame_decode_host_packed(ctx, h_occ, ob, h_lev.numpy(), J, h_w, h_bits, h_stream, nbytes, blk, C, fr.qstep,
+                                         None, h_vx, h_out, h_cnt2)
+        assert int(h_cnt2[2]) == 0 and torch.equal(h_out[:nv], h_out2[:nv])
     finally:
         ctx.close()

@@ -40,6 +40,35 @@ def test_yuv_matrix_and_roundtrip():
         orc.sh_layout(57)
 
 
+def bt601_yuv_from_definition():
+    """[R15] by its definition, not by its printed table: luma weights (W_R, W_G, W_B) = (0.299, 0.587, 0.114); U and V are
+    the colour differences B - Y and R - Y scaled to the peak excursions U_max = 0.436 and V_max = 0.615:
+    U = U_max (B - Y) / (1 - W_B) = 0.492 (B - Y),  V = V_max (R - Y) / (1 - W_R) = 0.877 (R - Y)."""
+    w = np.array([0.299, 0.587, 0.114])
+    ku, kv = 0.436 / (1.0 - w[2]), 0.615 / (1.0 - w[0])
+    assert round(ku, 3) == 0.492 and round(kv, 3) == 0.877
+    b_minus_y = np.array([0.0, 0.0, 1.0]) - w
+    r_minus_y = np.array([1.0, 0.0, 0.0]) - w
+    return np.stack([w, ku * b_minus_y, kv * r_minus_y])
+
+
+def test_yuv_matrix_is_bt601_entry_by_entry():
+    """Every one of the nine constants against the definition, to the five decimals they are printed with (cut off, not rounded): a swapped pair of
+    chroma coefficients, a wrong sign or a wrong U / V scale moves an entry by >= 1e-2."""
+    D = bt601_yuv_from_definition()
+    M = orc.YUV_FROM_RGB
+    assert M.shape == (3, 3)
+    assert np.array_equal(M[0], D[0])                                  # the luma weights are exact
+    assert np.abs(M[1:] - D[1:]).max() < 1e-5                         # chroma rows: the table prints 5 decimals, cut off (-0.1471377 -> -0.14713)
+    assert np.all(np.sign(M) == np.sign(D))
+    # and through the transform itself, one unit primary at a time, on the DC triple and on an AC triple
+    dc, ac = orc.sh_layout(56)
+    for k, trip in enumerate((dc, [ac[0][4], ac[1][4], ac[2][4]])):
+        for prim in range(3):
+            e = np.zeros((1, 56)); e[0, trip[prim]] = 1.0
+            assert np.abs(orc.rgb_to_yuv(e)[0, trip] - D[:, prim]).max() < 1e-5, (k, prim)
+
+
 @pytest.mark.parametrize("K", [15, 8, 3])
 def test_klt_is_pca(K):
     a = orc.rgb_to_yuv(_frame(6000, K, K))
