@@ -7,9 +7,9 @@ A "step" is one pass of the whole hot path over one frame: gsnfs_octree_encode -
 merge fused into the forward transform + quantiser) on the encoder side, the decoder's header read-back, then
 gsnfs_octree_decode -> gsnfs_raht_inverse.  `value` is whole-job Mgaussians/s with inputs resident in HBM; `e2e` is the
 same metric through the *_host_packed ABI calls with pinned host buffers (H2D/D2H inside the timed region; the
-coefficients cross PCIe as RLGR bytes) on a back-to-back frame stream (an encoder thread and a decoder thread, one context
-each; `e2e.serial`: one frame at a time on one context), `e2e_raw` through the *_host calls (raw int32 coefficients,
-one frame at a time).  `entropy` times
+coefficients cross PCIe as RLGR bytes), one frame at a time on one context (the round-1 protocol); `e2e_pipelined` is the
+same calls on a back-to-back frame stream (an encoder thread and a decoder thread, one context each: pipeline throughput, not
+frame latency); `e2e_raw` goes through the *_host calls (raw int32 coefficients, one frame at a time).  `entropy` times
 the RLGR coder on the frame's quantised coefficients, outside the step.  `--config pc` is the
 point-cloud shaped workload (NEXT-4: 1M points, depth 10, 3 colour channels).
 Multi-GPU: frames are independent (intra-only codec) => replicas only, one frame stream per
@@ -203,6 +203,53 @@ def run_ladder(B, synth, torch, ctx, buf, dev, n_frames):
                                               "ms_per_frame": round(ms_sh / n_frames, 4)}}
 
 
+def other_config_kernels(B, synth, torch, cfg, dev, device_index, peak, steps=10):
+    """Per-kernel live timings of one more workload (the 3M-Gaussian and point-cloud fractions were
+    builder-run only): the same step as the headline loop, 3 warm-up + `steps` profiled passes, own context and buffers."""
+    fr = synth.make_pointcloud_frame() if cfg == "pc" else synth.make_frame(int(cfg))
+    n, C, J = fr.n, fr.channels, fr.depth
+    ctx = B.Context(max_points=n, max_channels=C, max_depth=J, device=device_index)
+    try:
+        buf = B.FrameBuffers(n, C, J, dev)
+        d_xyz, d_attr = torch.from_numpy(fr.xyz).to(dev), torch.from_numpy(fr.attr).to(dev)
+        B.encode_frame(ctx, buf, d_xyz, d_attr, fr.bbox_min, fr.bbox_max, fr.qstep)
+        torch.cuda.synchronize()
+        levels, cnt = buf.level_sizes.cpu().numpy(), buf.counts.cpu().numpy()
+        nv, s_occ = int(cnt[0]), int(cnt[1])
+
+        def step():
+            B.encode_frame(ctx, buf, d_xyz, d_attr, fr.bbox_min, fr.bbox_max, fr.qstep)
+            B.decode_frame(ctx, buf, levels, s_occ, fr.qstep)
+
+        for _ in range(3):
+            step()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record(torch.cuda.current_stream())
+        for _ in range(steps):
+            step()
+        e1.record(torch.cuda.current_stream())
+        torch.cuda.synchronize()
+        ms_step = e0.elapsed_time(e1) / steps
+        ctx.profile_start(4096)
+        for _ in range(steps):
+            step()
+        prof = ctx.profile_stop()
+        ab = algorithmic_bytes(n, nv, s_occ, C, J)
+        ks = {}
+        for name, (c, tot_ms) in prof.items():
+            avg_us = tot_ms / c * 1e3
+            b = ab.get(name)
+            ks[name] = {"avg_us": round(avg_us, 2), "launches_per_step": c / steps,
+                        "frac_of_peak": round(b / (avg_us * 1e-6) / 1e9 / peak, 4) if b else None}
+        return {"workload": f"config {cfg}: N={n}, C={C}, depth {J}", "n_voxels": nv, "occ_bytes": s_occ,
+                "ms_per_step": round(ms_step, 4), "Mgaussians_per_s": round(n / (ms_step * 1e-3) / 1e6, 1), "steps": steps,
+                "note": "header read back once before the loop (no per-step host read); inputs resident in HBM",
+                "kernels": ks}
+    finally:
+        ctx.close()
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -306,8 +353,8 @@ def run_ours(args, rank, world, local_rank):
     sort_frac = (ab["_sort_total"] / (sort_ms * 1e-3) / 1e9 / peak) if sort_ms else None
 
     # ---- end to end through the host-buffer ABI calls (pinned host memory, copies inside the timed region)
-    RLGR_BLOCK = 512                       # Table A.5's fastest block size (here too: profiles/r2_rlgr_blocks.md)
-    e2e = e2e_raw = entropy = None
+    RLGR_BLOCK = 512                       # Table A.5's fastest block size (here too: profiles/r2_stages.md, RLGR block sweep)
+    e2e = e2e_raw = e2e_pipelined = entropy = None
     if rank == 0 or world > 1:
         cap = B.gsnfs_occ_capacity(n, J)
         pin = lambda *s, dt: torch.empty(s, dtype=dt).pin_memory()
@@ -395,16 +442,18 @@ def run_ours(args, rank, world, local_rank):
             torch.cuda.synchronize()
             ms_pp = (times[1] - times[0]) * 1e3 / kp
             ok_pp = bool(torch.equal(h_out2[:nv_e], h_out[:nv_e]))
-            # the headline end-to-end figure is the back-to-back frame stream (the codec's use-case, config 5 / PAPER.md
-            # L45-49); the one-frame-at-a-time loop above is kept beside it as "serial"
-            serial = {k: e2e[k] for k in ("value", "ms_per_step", "steps", "api")}
-            serial["how"] = "encode then decode of one frame at a time on one context: the two PCIe directions never overlap"
-            e2e.update({"value": round(n / (ms_pp * 1e-3) / 1e6, 3), "ms_per_step": round(ms_pp, 4), "steps": kp,
-                        "same_output_as_serial": ok_pp, "serial": serial,
-                        "how": "back-to-back frames: an encoder thread and a decoder thread, one context and stream each, "
-                               "three sets of pinned host buffers in rotation, every frame's inputs copied host -> device "
-                               "and its results device -> host inside the timed region; host wall clock over the timed "
-                               "frames (all calls are blocking)"})
+            # `e2e` stays what it was in round 1: one frame at a time (encode, then decode) through the blocking host calls
+            # on ONE context, timed with CUDA events -- comparable across rounds.  The back-to-back frame stream (the
+            # codec's use-case, config 5 / PAPER.md L45-49) is a different protocol and is reported beside it.
+            e2e["how"] = "encode then decode of one frame at a time on one context: the two PCIe directions never overlap"
+            e2e_pipelined = {
+                "value": round(n / (ms_pp * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_pp, 4), "steps": kp,
+                "h2d_bytes_per_step": e2e["h2d_bytes_per_step"], "d2h_bytes_per_step": e2e["d2h_bytes_per_step"],
+                "same_output_as_serial": ok_pp, "api": e2e["api"],
+                "how": "back-to-back frames: an encoder thread and a decoder thread, one context and stream each, three sets "
+                       "of pinned host buffers in rotation, every frame's inputs copied host -> device and its results "
+                       "device -> host inside the timed region; host wall clock over the timed frames (all calls are "
+                       "blocking).  Throughput of a pipeline, not the latency of a frame"}
             ctx2.close()
         ms_r, ks = time_e2e(raw_step)
         e2e_raw = {"value": round(world * n / (ms_r * 1e-3) / 1e6, 3), "unit": UNIT, "ms_per_step": round(ms_r, 4),
@@ -502,6 +551,11 @@ def run_ours(args, rank, world, local_rank):
     ladder = None
     if rank == 0 and world == 1 and args.ladder_frames > 0 and args.config == "3" and args.n_override is None:
         ladder = run_ladder(B, synth, torch, ctx, buf, dev, args.ladder_frames)
+    others_cfg = None
+    if rank == 0 and world == 1 and args.other_configs and args.config == "3" and args.n_override is None:
+        del d_attr, d_xyz                      # the 3M frame needs the room
+        others_cfg = {c: other_config_kernels(B, synth, torch, c, dev, local_rank, peak)
+                      for c in args.other_configs.split(",") if c}
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         cpu = oracle_time(fr, sample_n=min(fr.n, 1_000_000))
@@ -518,12 +572,12 @@ def run_ours(args, rank, world, local_rank):
                    "replicas": world, "l2_policy": "inputs larger than L2 (236 MB frame vs 126 MB L2); "
                    "intermediates stay wherever the pipeline leaves them"},
         "encode_ms": round(float(np.median(enc_ms)), 4), "decode_ms": round(float(np.median(dec_ms)), 4),
-        "clocks": clocks, "e2e": e2e, "e2e_raw": e2e_raw, "entropy": entropy, "gpu_launches": int(launches),
+        "clocks": clocks, "e2e": e2e, "e2e_pipelined": e2e_pipelined, "e2e_raw": e2e_raw, "entropy": entropy, "gpu_launches": int(launches),
         "gpu_launches_per_step": launches / args.steps,
         "roofline": roofline,
         "sort": {"alg_bytes": ab["_sort_total"], "ms_per_step": sort_ms, "passes": ab["_passes"],
                  "frac_of_peak": round(sort_frac, 4) if sort_frac else None},
-        "kernels": kernels, "ladder": ladder, "cpu_baseline": cpu,
+        "kernels": kernels, "other_configs": others_cfg, "ladder": ladder, "cpu_baseline": cpu,
     }
     print(json.dumps(out))
 
@@ -610,6 +664,8 @@ def main():
                     help="BASELINE.json config (1-based); 3 = headline 1M frame; pc = point-cloud shaped frame (NEXT-4)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--other-configs", default="4,pc",
+                    help="also report per-kernel timings at these workloads (comma list of 4, pc, 1, 2; '' to skip)")
     ap.add_argument("--rlgr-sweep", action="store_true", help="also time the RLGR coder at Table A.5's block sizes")
     ap.add_argument("--n-override", type=int, default=None,
                     help="same recipe with another N (e.g. 16000000: key arrays no longer fit the 126 MB L2); not the headline")
