@@ -6,8 +6,8 @@
 //
 // Five small launches: histogram -> model (one warp quantises the 256 counts to sum 4096) -> one thread per block
 // encodes backwards from a padded shared-memory copy of its 1024 bytes into a strided scratch -> scan of the word counts
-// -> compaction into the caller's payload.  Decoding is one launch: a 4096-entry slot -> symbol table in shared
-// memory, one thread per block, output staged in shared memory and written coalesced.
+// -> compaction into the caller's payload.  Decoding is one launch (+ the offset scan): a 4096-entry packed slot table and
+// the CTA's payload span in shared memory, one thread per block (see rans_decode_kernel).
 #include <mutex>
 
 #include "common.cuh"
@@ -89,24 +89,45 @@ __global__ void __launch_bounds__(kRansCta) rans_encode_kernel(const uint8_t* __
                                                                uint32_t* __restrict__ states, uint16_t* __restrict__ nwords,
                                                                uint64_t nblk_host) {
   extern __shared__ __align__(16) uint8_t s_data[];                 // kRansCta x kRansPitch
-  __shared__ uint16_t s_f[256];
-  __shared__ uint16_t s_cum[256];
+  __shared__ uint2 s_e[256];                                        // symbol -> { floor(2^32 / f), f | cum << 16 }
   const uint64_t n = n_dev ? min((uint64_t)*n_dev, n_host) : n_host;
   const int t = threadIdx.x;
-  for (int s = t; s < 256; s += kRansCta) s_f[s] = freq[s];
-  __syncwarp();
-  if (t == 0) { uint32_t c = 0; for (int s = 0; s < 256; ++s) { s_cum[s] = (uint16_t)c; c += s_f[s]; } }
   const uint64_t b0 = (uint64_t)blockIdx.x * kRansCta;
   const uint64_t base = b0 * kRansBlock;
   if (base >= n) { if (b0 + t < nblk_host) nwords[b0 + t] = 0; return; }
+  // the CTA's 32 blocks into shared memory: asynchronous 4-byte copies (the pitch of 1028 keeps rows 4-byte aligned only),
+  // all in flight while the symbol table is built
   const uint64_t span = min((uint64_t)kRansCta * kRansBlock, n - base);
-  for (uint64_t i = (uint64_t)t * 4u; i < span; i += kRansCta * 4u) {      // coalesced, 4 bytes per lane
-    const uint32_t blk = (uint32_t)(i / kRansBlock), o = (uint32_t)(i % kRansBlock);
-    uint32_t w = 0;
-    if (i + 4 <= span) w = *reinterpret_cast<const uint32_t*>(data + base + i);
-    else for (uint64_t k = i; k < span; ++k) w |= (uint32_t)data[base + k] << (8 * (k - i));
-    *reinterpret_cast<uint32_t*>(s_data + blk * kRansPitch + o) = w;
+  {
+    const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_data);
+    for (uint64_t i = (uint64_t)t * 4u; i < span; i += kRansCta * 4u) {      // coalesced, 4 bytes per lane
+      const uint32_t blk = (uint32_t)(i / kRansBlock), o = (uint32_t)(i % kRansBlock);
+      if (i + 4 <= span) {
+        asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(sbase + blk * kRansPitch + o), "l"(data + base + i) : "memory");
+      } else {
+        uint32_t w = 0;
+        for (uint64_t k = i; k < span; ++k) w |= (uint32_t)data[base + k] << (8 * (k - i));
+        *reinterpret_cast<uint32_t*>(s_data + blk * kRansPitch + o) = w;
+      }
+    }
+    asm volatile("cp.async.commit_group;" ::: "memory");
   }
+  {   // lane t owns symbols 8t .. 8t+7: cumulative frequencies by a warp scan; x / f becomes a multiply by floor(2^32 / f)
+    uint32_t f8[8], lsum = 0;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { f8[j] = freq[8 * t + j]; lsum += f8[j]; }
+    uint32_t inc = lsum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (t >= o) inc += v; }
+    uint32_t c = inc - lsum;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+      const uint32_t f = f8[j];
+      s_e[8 * t + j] = make_uint2(f > 1u ? (uint32_t)((1ull << 32) / f) : 0xffffffffu, f | (c << 16));
+      c += f;
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncwarp();
   const uint64_t myb = b0 + t;
   const uint64_t mybase = myb * kRansBlock;
@@ -115,11 +136,23 @@ __global__ void __launch_bounds__(kRansCta) rans_encode_kernel(const uint8_t* __
   const uint8_t* my = s_data + t * kRansPitch;
   uint16_t* out = scratch + myb * kRansScratchWords + kRansScratchWords;      // filled backwards: decoder order
   uint32_t nw = 0, x = kRansL;
-  for (uint32_t i = cnt; i-- > 0;) {
-    const uint32_t s = my[i], fs = s_f[s];
-    if ((uint64_t)x >= ((uint64_t)fs << 20)) { *--out = (uint16_t)(x & 0xffffu); x >>= 16; ++nw; }
-    const uint32_t q = x / fs;
-    x = q * kRansM + (x - q * fs) + s_cum[s];
+  // one symbol: renormalise if x >= f << 20, then x = (x / f) * 4096 + x % f + cum.  q = x / f: umulhi(x, floor(2^32 / f))
+  // is q or q - 1 (the reciprocal is short by < 1 ulp and x < 2^32), one fix-up makes it exact.
+  auto put = [&](uint2 e) {
+    const uint32_t fs = e.y & 0xffffu;
+    if ((x >> 20) >= fs) { *--out = (uint16_t)(x & 0xffffu); x >>= 16; ++nw; }
+    uint32_t q = __umulhi(x, e.x);
+    uint32_t r = x - q * fs;
+    if (r >= fs) { ++q; r -= fs; }
+    x = q * kRansM + r + (e.y >> 16);
+  };
+  uint32_t i = cnt;
+  while (i & 3u) { --i; put(s_e[my[i]]); }                          // ragged end of the frame's last block
+  while (i) {                                                       // 4 symbols per step: their table entries are loaded
+    i -= 4u;                                                        // before the first of the 4 dependent state updates
+    const uint32_t w4 = *reinterpret_cast<const uint32_t*>(my + i);
+    const uint2 e3 = s_e[w4 >> 24], e2 = s_e[(w4 >> 16) & 0xffu], e1 = s_e[(w4 >> 8) & 0xffu], e0 = s_e[w4 & 0xffu];
+    put(e3); put(e2); put(e1); put(e0);
   }
   states[myb] = x;
   nwords[myb] = (uint16_t)nw;
@@ -186,64 +219,129 @@ __global__ void __launch_bounds__(128) rans_pack_kernel(const uint16_t* __restri
   }
 }
 
+// Decoder: one thread per block, one warp per CTA.  A block is a serial chain of 1024 dependent symbol steps, so the
+// launch is latency bound (6.6 k threads at config 3) and everything on the chain is kept short: ONE shared-memory load
+// per symbol from a 4096-entry slot table that packs {symbol, f - 1, slot - cum} in a word, the CTA's whole payload span
+// (its 32 block streams lie back to back) staged in shared memory by asynchronous 16-byte copies before the first symbol, the
+// next renormalisation word fetched ahead of its use and selected without a branch, 16 decoded bytes stored at a time.
+constexpr uint32_t kRansStageBytes = kRansCta * (4u + 2u * kRansScratchWords);   // the encoder cannot emit more per CTA
+constexpr uint32_t kRansDecodeSmem = kRansM * 4u + kRansStageBytes + 32u;
+
 __global__ void __launch_bounds__(kRansCta) rans_decode_kernel(const uint8_t* __restrict__ payload, uint64_t payload_bytes,
                                                                const uint16_t* __restrict__ freq,
                                                                const uint16_t* __restrict__ nwords,
                                                                const uint64_t* __restrict__ off, uint64_t n,
                                                                uint8_t* __restrict__ out, gsnfs_rlgr_info* __restrict__ info) {
-  extern __shared__ __align__(16) uint8_t s_dyn[];                  // kRansCta x kRansPitch output staging, then the slot table
-  uint8_t* s_out = s_dyn;
-  uint8_t* s_sym = s_dyn + kRansCta * kRansPitch;                   // kRansM
-  __shared__ uint16_t s_f[256];
+  extern __shared__ __align__(16) uint8_t s_dyn[];
+  uint32_t* s_tab = reinterpret_cast<uint32_t*>(s_dyn);             // slot -> symbol | (f - 1) << 8 | (slot - cum) << 20
+  uint8_t* s_pay = s_dyn + kRansM * 4u;                             // payload span of this CTA's blocks (+ slack)
   __shared__ uint16_t s_cum[257];
-  __shared__ uint32_t s_bad;
   const int t = threadIdx.x;
-  for (int s = t; s < 256; s += kRansCta) s_f[s] = freq[s];
-  if (t == 0) s_bad = 0;
-  __syncwarp();
-  if (t == 0) { uint32_t c = 0; for (int s = 0; s < 256; ++s) { s_cum[s] = (uint16_t)min(c, 65535u); c += s_f[s]; } s_cum[256] = (uint16_t)min(c, 65535u); if (c != kRansM) s_bad = 1; }
-  __syncwarp();
-  const bool model_ok = s_bad == 0;
-  if (model_ok)
-    for (int s = t; s < 256; s += kRansCta)
-      for (uint32_t k = 0; k < s_f[s]; ++k) s_sym[s_cum[s] + k] = (uint8_t)s;
-  __syncwarp();
   const uint64_t b0 = (uint64_t)blockIdx.x * kRansCta;
   const uint64_t base = b0 * kRansBlock;
   if (base >= n) return;
-  const uint64_t myb = b0 + t, mybase = myb * kRansBlock;
-  bool bad = !model_ok;
-  if (mybase < n) {
-    const uint32_t cnt = (uint32_t)min((uint64_t)kRansBlock, n - mybase);
-    uint8_t* my = s_out + t * kRansPitch;
-    const uint32_t nw = nwords[myb];
-    const uint64_t o = off[myb];
-    if (bad || o + 4ull + 2ull * nw > payload_bytes) {
-      bad = true;
-      for (uint32_t i = 0; i < cnt; ++i) my[i] = 0;
+  // model: lane t owns symbols 8t .. 8t+7
+  uint32_t f8[8], lsum = 0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) { f8[j] = freq[8 * t + j]; lsum += f8[j]; }
+  uint32_t inc = lsum;
+#pragma unroll
+  for (int o = 1; o < 32; o <<= 1) { const uint32_t v = __shfl_up_sync(0xffffffffu, inc, o); if (t >= o) inc += v; }
+  const uint32_t total = __shfl_sync(0xffffffffu, inc, 31);
+  const bool model_ok = total == kRansM;
+  if (model_ok) {
+    uint32_t c = inc - lsum;
+#pragma unroll
+    for (int j = 0; j < 8; ++j) { s_cum[8 * t + j] = (uint16_t)c; c += f8[j]; }
+    if (t == 31) s_cum[256] = (uint16_t)kRansM;
+  }
+  __syncwarp();
+  // stage the payload span [o0, o1) of the CTA's blocks from the 16-byte boundary at or below its start: asynchronous
+  // 16-byte copies, all in flight while the slot table is built
+  const uint64_t nblk = (n + kRansBlock - 1) / kRansBlock;
+  const uint64_t o0 = off[b0], o1 = min(off[min(b0 + kRansCta, nblk)], payload_bytes);
+  uint32_t sh = 0;
+  if (o0 < o1) {
+    const uint8_t* g = payload + o0;
+    const uint32_t len = (uint32_t)min(o1 - o0, (uint64_t)kRansStageBytes);
+    if (((uintptr_t)payload & 15u) == 0) {
+      sh = (uint32_t)(o0 & 15u);
+      g -= sh;                                                      // 16-byte aligned, still inside the payload
+      const uint32_t tot = len + sh;                                // bytes [0, tot) of g lie inside the payload
+      const uint32_t full = tot & ~15u;
+      const uint32_t sbase = (uint32_t)__cvta_generic_to_shared(s_pay);
+      for (uint32_t i = 16u * t; i < full; i += 16u * kRansCta)
+        asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(sbase + i), "l"(g + i) : "memory");
+      if (t < (int)(tot - full)) s_pay[full + t] = g[full + t];
     } else {
-      const uint8_t* p = payload + o;
-      uint32_t x = (uint32_t)p[0] | ((uint32_t)p[1] << 8) | ((uint32_t)p[2] << 16) | ((uint32_t)p[3] << 24);
-      uint32_t w = 0;
-      for (uint32_t i = 0; i < cnt; ++i) {
-        const uint32_t slot = x & (kRansM - 1u);
-        const uint32_t s = s_sym[slot];
-        my[i] = (uint8_t)s;
-        x = (uint32_t)s_f[s] * (x >> 12) + slot - s_cum[s];
-        if (x < kRansL) {
-          uint32_t nxt = 0;
-          if (w < nw) nxt = (uint32_t)p[4 + 2 * w] | ((uint32_t)p[5 + 2 * w] << 8); else bad = true;
-          ++w;
-          x = (x << 16) | nxt;
-        }
-      }
-      if (w != nw || x != kRansL) bad = true;
+      for (uint32_t i = t; i < len; i += kRansCta) s_pay[i] = g[i];
     }
   }
-  if (bad) atomicOr(&info->status, 1u);
+  asm volatile("cp.async.commit_group;" ::: "memory");
+  if (model_ok) {                                                   // lane t fills slots 128t .. 128t+127
+    uint32_t slot = 128u * t;
+    int lo = 0, hi = 256;                                           // s_cum[lo] <= slot < s_cum[hi]
+    while (hi - lo > 1) { const int mid = (lo + hi) >> 1; if (s_cum[mid] <= slot) lo = mid; else hi = mid; }
+    uint32_t c0 = s_cum[lo], c1 = s_cum[lo + 1];
+    for (int k = 0; k < 128; ++k, ++slot) {
+      while (slot >= c1) { ++lo; c0 = c1; c1 = s_cum[lo + 1]; }
+      s_tab[slot] = (uint32_t)lo | ((c1 - c0 - 1u) << 8) | ((slot - c0) << 20);
+    }
+  }
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
   __syncwarp();
-  const uint64_t span = min((uint64_t)kRansCta * kRansBlock, n - base);
-  for (uint64_t i = t; i < span; i += kRansCta) out[base + i] = s_out[(i / kRansBlock) * kRansPitch + (i % kRansBlock)];
+  const uint64_t myb = b0 + t, mybase = myb * kRansBlock;
+  if (mybase >= n) return;
+  const uint32_t cnt = (uint32_t)min((uint64_t)kRansBlock, n - mybase);
+  uint8_t* dst = out + mybase;
+  const uint32_t nw = nwords[myb];
+  const uint64_t o = off[myb];
+  const uint64_t rel = o - o0 + sh;                                 // this block's stream inside s_pay
+  bool bad = !model_ok || o + 4ull + 2ull * nw > payload_bytes || rel + 4ull + 2ull * nw > (uint64_t)kRansStageBytes + sh;
+  if (bad) {
+    for (uint32_t i = 0; i < cnt; ++i) dst[i] = 0;
+    atomicOr(&info->status, 1u);
+    return;
+  }
+  const uint16_t* my = reinterpret_cast<const uint16_t*>(s_pay + rel);      // 2-byte aligned: offsets and sh are even
+  uint32_t x = (uint32_t)my[0] | ((uint32_t)my[1] << 16);
+  const uint16_t* words = my + 2;
+  const uint32_t last = nw ? nw - 1u : 0u;
+  uint32_t w = 0, nxt = words[0];                                   // (nw == 0: reads the slack, never used)
+  const bool vec = (((uintptr_t)out) & 15u) == 0;
+  uint32_t i = 0;
+  for (; i + 16u <= cnt; i += 16u) {
+    uint32_t acc[4] = {0u, 0u, 0u, 0u};
+#pragma unroll
+    for (int j = 0; j < 16; ++j) {
+      const uint32_t slot = x & (kRansM - 1u);
+      const uint32_t e = s_tab[slot];
+      acc[j >> 2] |= (e & 0xffu) << (8 * (j & 3));
+      x = (((e >> 8) & 0xfffu) + 1u) * (x >> 12) + (e >> 20);
+      const bool rn = x < kRansL;                                  // renormalise: no branch (lanes diverge on every symbol)
+      x = rn ? (x << 16) | nxt : x;
+      w += rn ? 1u : 0u;
+      nxt = words[min(w, last)];
+    }
+    if (vec) {
+      *reinterpret_cast<uint4*>(dst + i) = make_uint4(acc[0], acc[1], acc[2], acc[3]);
+    } else {
+#pragma unroll
+      for (int j = 0; j < 16; ++j) dst[i + j] = (uint8_t)(acc[j >> 2] >> (8 * (j & 3)));
+    }
+  }
+  for (; i < cnt; ++i) {                                            // ragged end of the last block
+    const uint32_t slot = x & (kRansM - 1u);
+    const uint32_t e = s_tab[slot];
+    dst[i] = (uint8_t)e;
+    x = (((e >> 8) & 0xfffu) + 1u) * (x >> 12) + (e >> 20);
+    const bool rn = x < kRansL;
+    x = rn ? (x << 16) | nxt : x;
+    w += rn ? 1u : 0u;
+    nxt = words[min(w, last)];
+  }
+  if (w != nw || x != kRansL) bad = true;       // (more renormalisations than words: w > nw)
+  if (bad) atomicOr(&info->status, 1u);
 }
 
 }  // namespace
@@ -288,7 +386,7 @@ int run_rans_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_payload, u
   const int grid = (int)((nblk + kRansCta - 1) / kRansCta);
   if (grid > 0) {
     GSNFS_KERNEL(ctx, st, "rans_decode");
-    rans_decode_kernel<<<grid, kRansCta, kRansCta * kRansPitch + kRansM, st>>>(d_payload, payload_bytes, d_freq, d_nwords,
+    rans_decode_kernel<<<grid, kRansCta, kRansDecodeSmem, st>>>(d_payload, payload_bytes, d_freq, d_nwords,
                                                                               ctx->rans_off, n, d_out, d_info);
     GSNFS_LAUNCH_CHECK(ctx, st);
   }
@@ -297,7 +395,7 @@ int run_rans_decode(gsnfs_ctx* ctx, cudaStream_t st, const uint8_t* d_payload, u
 
 int rans_setup(gsnfs_ctx* ctx) {
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                          (int)(kRansCta * kRansPitch + kRansM)));
+                                          (int)kRansDecodeSmem));
   GSNFS_CUDA_OK(ctx, cudaFuncSetAttribute(rans_encode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                           (int)(kRansCta * kRansPitch)));
   return GSNFS_OK;
@@ -336,7 +434,7 @@ int static_off_for_current_device(uint64_t** out) {
     uint64_t* p = nullptr;
     if (cudaGetSymbolAddress((void**)&p, g_static_off) != cudaSuccess || !p) return GSNFS_E_CUDA;
     if (cudaFuncSetAttribute(rans_decode_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                             (int)(kRansCta * kRansPitch + kRansM)) != cudaSuccess)
+                             (int)kRansDecodeSmem) != cudaSuccess)
       return GSNFS_E_CUDA;
     g_static_off_dev[dev] = p;
   }
@@ -365,7 +463,7 @@ int gsnfs_rans_decode_static(gsnfs_stream stream, const uint8_t* d_payload, uint
   if (cudaPeekAtLastError() != cudaSuccess) return GSNFS_E_CUDA;
   const int grid = (int)((nblk + kRansCta - 1) / kRansCta);
   if (grid > 0) {
-    rans_decode_kernel<<<grid, kRansCta, kRansCta * kRansPitch + kRansM, st>>>(d_payload, payload_bytes, d_freq, d_nwords, off,
+    rans_decode_kernel<<<grid, kRansCta, kRansDecodeSmem, st>>>(d_payload, payload_bytes, d_freq, d_nwords, off,
                                                                               n, d_out, d_info);
     if (cudaPeekAtLastError() != cudaSuccess) return GSNFS_E_CUDA;
   }
