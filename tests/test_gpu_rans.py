@@ -125,6 +125,33 @@ def test_capacity_and_corruption(B, ctx):
     assert B.rlgr_info(d_info)[2] == 0 and np.array_equal(d_out.cpu().numpy(), x)
 
 
+@pytest.mark.parametrize("shift_p,shift_o", [(0, 0), (1, 0), (2, 3), (4, 8), (6, 1), (8, 16)])
+def test_decoder_accepts_any_buffer_alignment(B, ctx, shift_p, shift_o):
+    """The decoder stages the payload with 16-byte copies and stores 16 output bytes at a time when the caller's buffers allow
+    it; slices that start at other addresses (a section inside a larger buffer) take its byte-wise paths.  Same bytes out."""
+    rng = np.random.default_rng(40 + shift_p)
+    x = rng.choice([0x18, 0xff, 0x01, 0x80, 0x11, 0x22], size=100_000 + 333, p=[.5, .2, .14, .1, .05, .01]).astype(np.uint8)
+    d_f, d_nw, d_p, nbytes, nblocks, status = gpu_encode(B, ctx, x)
+    assert status == 0
+    p_buf = torch.zeros(nbytes + 64, dtype=torch.uint8, device=DEV)
+    p_view = p_buf[shift_p:shift_p + nbytes]
+    p_view.copy_(d_p[:nbytes])
+    o_buf = torch.full((len(x) + 64,), 9, dtype=torch.uint8, device=DEV)
+    o_view = o_buf[shift_o:shift_o + len(x)]
+    assert p_view.data_ptr() % 16 == shift_p % 16 and o_view.data_ptr() % 16 == shift_o % 16
+    d_info = torch.full((2,), -1, dtype=torch.int64, device=DEV)
+    B.gsnfs_rans_decode(ctx, p_view, nbytes, d_f, d_nw, len(x), o_view, d_info)
+    torch.cuda.synchronize()
+    assert B.rlgr_info(d_info)[2] == 0 and np.array_equal(o_view.cpu().numpy(), x)
+    assert bool((o_buf[:shift_o] == 9).all()) and bool((o_buf[shift_o + len(x):] == 9).all())      # nothing outside the view
+    d_info.fill_(-1)
+    o_buf.fill_(9)
+    B.gsnfs_rans_decode_static(p_view, nbytes, d_f, d_nw, len(x), o_view, d_info)
+    torch.cuda.synchronize()
+    assert B.rlgr_info(d_info)[2] == 0 and np.array_equal(o_view.cpu().numpy(), x)
+    assert bool((o_buf[:shift_o] == 9).all()) and bool((o_buf[shift_o + len(x):] == 9).all())
+
+
 def test_whole_frame_through_the_container(B):
     """A frame coded on the device (octree -> rANS, merge + RAHT + quantiser -> RLGR), framed by gsnfs_container_pack,
     parsed back, decoded on the device: voxels bit-exact, attributes as the raw-coefficient path gives them."""
